@@ -1,0 +1,471 @@
+"""Pins P1-P17: the fp64 oracle against what the
+paper and the mathematics fix -- closed forms, invariants, textbook special cases, the Keys
+kernel's printed impulse response and exact-rational brute force on tiny grids.
+
+CPU only.  Nothing here touches the CUDA path.  Expected values are typed from the closed form
+(never from the oracle's own formula) or computed with python `fractions`.
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import oracle
+
+H_PLANCK = 6.62607015e-27
+C_AA = 2.99792458e18
+HC = H_PLANCK * C_AA
+AB_FNU = 3.631e-20
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ------------------------------------------------------------------ tiny model builders
+def grid_model(m0_fn, m1_fn=None, n_phase=11, n_wave=41, p0=-5.0, dp=1.0, w0=3000.0, dw=10.0,
+               cl_coef=(0.0, 1.0, -0.2, 0.05, -0.01), wb=4302.57, wv=5428.55, lo=2800.0, hi=7000.0):
+    phase = p0 + dp * np.arange(n_phase)
+    wave = w0 + dw * np.arange(n_wave)
+    P, L = np.meshgrid(phase, wave, indexing="ij")
+    m0 = np.asarray(m0_fn(P, L), dtype=np.float64) * np.ones_like(P)
+    m1 = np.zeros_like(m0) if m1_fn is None else np.asarray(m1_fn(P, L), dtype=np.float64) * np.ones_like(P)
+    return oracle.Model(phase, wave, m0, m1, np.asarray(cl_coef, dtype=np.float64), wb, wv, lo, hi)
+
+
+def tophat(la, lb, step):
+    n = int(round((lb - la) / step)) + 1
+    w = la + step * np.arange(n)
+    return oracle.Bands(np.array([0, n]), w, np.ones(n))
+
+
+def rng_model(seed=7, **kw):
+    rng = np.random.default_rng(seed)
+    n_phase, n_wave = kw.pop("n_phase", 12), kw.pop("n_wave", 60)
+    a = rng.standard_normal((n_phase, n_wave))
+    b = rng.standard_normal((n_phase, n_wave))
+    phase = -5.0 + np.arange(n_phase)
+    wave = 3000.0 + 10.0 * np.arange(n_wave)
+    return oracle.Model(phase, wave, a, b, np.array([0.0, 0.9, -0.2, 0.05, -0.01]), 4302.57, 5428.55,
+                        2800.0, 7000.0)
+
+
+def rel(a, b):
+    return abs(a - b) / max(abs(b), 1e-300)
+
+
+# ------------------------------------------------------------------ P1
+@pytest.mark.parametrize("z,t", [(0.0, 0.3), (0.05, -2.2), (0.2, 3.9)])
+def test_p1_constant_surface_tophat(z, t):
+    """M0 = K, M1 = 0, c = 0, T = 1 on [la, lb], no zp: x0 K (lb^2 - la^2)/(2hc) (BASELINE north_star)."""
+    K, x0 = 3.25, 2.0e-5
+    m = grid_model(lambda p, l: K, n_wave=101)  # 3000..4000 A
+    la, lb = 3700.0, 3900.0  # rest-frame stays inside the grid for every z used
+    bd = tophat(la, lb, 5.0)
+    got = oracle.eval_one(m, bd, z, t, 0, None, x0, 0.7, 0.0, 0.1)
+    want = x0 * K * (lb * lb - la * la) / (2.0 * HC)
+    assert rel(got, want) < 1e-14
+
+
+# ------------------------------------------------------------------ P2 / G12
+def test_p2_linear_in_x0_affine_in_x1():
+    m = rng_model()
+    bd = tophat(3600.0, 3900.0, 5.0)
+    args = dict(z=0.1, t=1.3, b=0, zp=25.0)
+    f = lambda x0, x1: oracle.eval_one(m, bd, args["z"], args["t"], 0, 25.0, x0, x1, 0.04, -0.2)
+    assert rel(f(2e-5, 0.4), 2.0 * f(1e-5, 0.4)) < 1e-14
+    assert f(0.0, 0.4) == 0.0
+    # affine in x1: zero second difference, and m(x1=0) is the M0-only flux
+    a, b_, c_ = f(1e-5, -1.0), f(1e-5, 0.0), f(1e-5, 1.0)
+    scale = max(abs(a), abs(b_), abs(c_))
+    assert abs(a - 2.0 * b_ + c_) < 1e-13 * scale
+    m_no_m1 = oracle.Model(m.phase, m.wave, m.m0, np.zeros_like(m.m1), m.cl_coef, 4302.57, 5428.55,
+                           2800.0, 7000.0)
+    assert rel(b_, oracle.eval_one(m_no_m1, bd, 0.1, 1.3, 0, 25.0, 1e-5, 5.0, 0.04, -0.2)) < 1e-14
+
+
+# ------------------------------------------------------------------ P3
+def test_p3_c_zero_unit_colour_factor():
+    m = rng_model()
+    m_other = oracle.Model(m.phase, m.wave, m.m0, m.m1, np.array([0.3, -2.0, 1.0, 0.7, 0.2]), 4000.0,
+                           5000.0, 3100.0, 3300.0)
+    bd = tophat(3600.0, 3900.0, 5.0)
+    a = oracle.eval_one(m, bd, 0.1, 1.3, 0, None, 1e-5, 0.4, 0.0, 0.0)
+    b = oracle.eval_one(m_other, bd, 0.1, 1.3, 0, None, 1e-5, 0.4, 0.0, 0.0)
+    assert a == b  # exp(0 * CL) == 1 exactly
+
+
+# ------------------------------------------------------------------ P4
+def test_p4_exact_nodes():
+    m = rng_model()
+    for k in (0, 1, 5, 10, 11):
+        for l in (0, 1, 30, 58, 59):
+            v0, _ = m.surface(0, m.phase[k], m.wave[l])
+            v1, _ = m.surface(1, m.phase[k], m.wave[l])
+            assert abs(v0 - m.m0[k, l]) <= 1e-13 * max(1.0, abs(m.m0[k, l]))
+            assert abs(v1 - m.m1[k, l]) <= 1e-13 * max(1.0, abs(m.m1[k, l]))
+
+
+def test_p4_linear_surface_reproduced_everywhere():
+    al, be, ga = 2.0, 0.37, -1.1e-3
+    m = grid_model(lambda p, l: al + be * p + ga * l)
+    rng = np.random.default_rng(3)
+    pts = [(rng.uniform(-5, 5), rng.uniform(3000, 3400)) for _ in range(200)]
+    pts += [(-4.6, 3003.0), (4.7, 3397.0), (-5.0, 3000.0), (5.0, 3400.0), (0.2, 3001.0), (-4.9, 3200.0)]
+    for p, l in pts:
+        v, dv = m.surface(0, p, l)
+        assert abs(v - (al + be * p + ga * l)) < 1e-13 * 5.0
+        assert abs(dv - be) < 1e-12
+
+
+def test_p4_quadratic_reproduced_in_interior_cells_only():
+    m = grid_model(lambda p, l: 1.0 + 0.1 * p * p + 1e-4 * (l - 3200.0) ** 2 + 0.01 * p * (l - 3200.0))
+    f = lambda p, l: 1.0 + 0.1 * p * p + 1e-4 * (l - 3200.0) ** 2 + 0.01 * p * (l - 3200.0)
+    rng = np.random.default_rng(4)
+    for _ in range(200):
+        p, l = rng.uniform(-4, 4), rng.uniform(3010, 3390)  # interior cells of both axes
+        v, dv = m.surface(0, p, l)
+        assert abs(v - f(p, l)) < 1e-12 * 20
+        assert abs(dv - (0.2 * p + 0.01 * (l - 3200.0))) < 1e-11
+    # border cell along wavelength is linear, so a quadratic is NOT reproduced there
+    v, _ = m.surface(0, 0.5, 3005.0)
+    assert abs(v - f(0.5, 3005.0)) > 1e-4
+
+
+# ------------------------------------------------------------------ P5
+def _golden_impulse():
+    rows = []
+    with open(os.path.join(GOLDEN, "keys_impulse.txt")) as fh:
+        for line in fh:
+            line = line.strip()
+            if line and not line.startswith("#"):
+                a, b = line.split()
+                rows.append((float(a), float(b)))
+    return rows
+
+
+def test_p5_keys_impulse_response_1d():
+    n = 21
+    g = np.zeros(n)
+    g[10] = 1.0
+    for off, want in _golden_impulse():
+        v, _ = oracle.interp1(g, 100.0, 2.0, 100.0 + 2.0 * (10 + off))
+        assert abs(v - want) < 1e-15, (off, v, want)
+
+
+def test_p5_impulse_response_2d_is_product():
+    phase = np.arange(21.0)
+    wave = 1000.0 + 10.0 * np.arange(25)
+    m0 = np.zeros((21, 25))
+    m0[9, 12] = 1.0
+    m = oracle.Model(phase, wave, m0, m0 * 0.0, np.zeros(5), 4302.57, 5428.55, 2800.0, 7000.0)
+    rows = _golden_impulse()
+    for op, wp in rows[:9]:
+        for ol, wl in rows[3:13]:
+            v, _ = m.surface(0, 9.0 + op, 1120.0 + 10.0 * ol)
+            assert abs(v - wp * wl) < 1e-15
+
+
+# ------------------------------------------------------------------ P6
+def test_p6_trapezoid_linear_exact_and_quadratic_error_term():
+    x = np.array([1.0, 1.5, 4.0, 4.25, 9.0])  # non-uniform
+    g = 3.0 - 0.7 * x
+    want = 3.0 * (9.0 - 1.0) - 0.35 * (81.0 - 1.0)
+    assert abs(oracle.trapz(g, x) - want) < 1e-13
+    a, b, h = 4000.0, 6000.0, 5.0
+    lam = a + h * np.arange(int((b - a) / h) + 1)
+    got = oracle.trapz(lam * lam, lam)
+    exact = (b ** 3 - a ** 3) / 3.0
+    assert rel(got - exact, h * h * (b - a) / 6.0) < 1e-6  # = +8333.33..., rejects midpoint/Simpson
+    assert rel(got, exact + h * h * (b - a) / 6.0) < 1e-12
+
+
+# ------------------------------------------------------------------ P7
+@pytest.mark.parametrize("z,t,t0", [(0.0, 1.0, 0.0), (0.25, 3.0, -1.5), (0.1, -2.0, 1.75)])
+def test_p7_phase_mapping(z, t, t0):
+    """M0 = al + be p: pins p = (t - t0)/(1+z), including the sign of t0 (G0)."""
+    al, be, x0 = 2.0, 0.3, 1.5e-5
+    m = grid_model(lambda p, l: al + be * p, n_wave=101)
+    la, lb = 3800.0, 3950.0
+    bd = tophat(la, lb, 5.0)
+    got, dm = oracle.eval_one(m, bd, z, t, 0, None, x0, 0.0, 0.0, t0, grad=True)
+    area = (lb * lb - la * la) / (2.0 * HC)
+    want = x0 * (al + be * (t - t0) / (1.0 + z)) * area
+    assert rel(got, want) < 1e-13
+    assert rel(dm[3], -x0 * be / (1.0 + z) * area) < 1e-12  # P15 closed form for d/dt0
+
+
+# ------------------------------------------------------------------ P8
+@pytest.mark.parametrize("z", [0.0, 0.1, 0.3])
+def test_p8_wavelength_mapping(z):
+    """M0 = ga lam_rest: pins lam_rest = lam_obs/(1+z) and the observer-frame lam/(hc) factor."""
+    ga, x0, h = 1e-3, 1.0e-5, 5.0
+    m = grid_model(lambda p, l: ga * l, n_wave=151)  # 3000..4500
+    la, lb = 4000.0, 4300.0
+    bd = tophat(la, lb, h)
+    got = oracle.eval_one(m, bd, z, 0.4, 0, None, x0, 0.0, 0.0, 0.0)
+    want = x0 * ga / (1.0 + z) * ((lb ** 3 - la ** 3) / 3.0 + h * h * (lb - la) / 6.0) / HC
+    assert rel(got, want) < 1e-12
+
+
+# ------------------------------------------------------------------ P9 / P10
+def test_p9_zero_point_ratios():
+    m = rng_model()
+    w = 3600.0 + 5.0 * np.arange(61)
+    tr = np.exp(-0.5 * ((w - 3750.0) / 60.0) ** 2)
+    bd = oracle.Bands(np.array([0, 61]), w, tr)
+    raw = oracle.eval_one(m, bd, 0.1, 1.3, 0, None, 1e-5, 0.4, 0.03, 0.0)
+    m25 = oracle.eval_one(m, bd, 0.1, 1.3, 0, 25.0, 1e-5, 0.4, 0.03, 0.0)
+    m275 = oracle.eval_one(m, bd, 0.1, 1.3, 0, 27.5, 1e-5, 0.4, 0.03, 0.0)
+    assert rel(m275, 10.0 * m25) < 1e-14
+    # ZPAB written out independently with numpy's trapezoid of (AB_FNU/h) T / lam
+    zpab = np.trapezoid(AB_FNU / H_PLANCK * tr / w, w)
+    assert rel(bd.zpab(0), zpab) < 1e-14
+    assert rel(m25 / raw, 10.0 ** 10 / zpab) < 1e-14
+
+
+def test_p10_zpab_tophat_closed_form():
+    la, lb, h = 4000.0, 6000.0, 5.0
+    bd = tophat(la, lb, h)
+    lead = math.log(lb / la)
+    corr = h * h / 12.0 * (1.0 / la ** 2 - 1.0 / lb ** 2)
+    want = AB_FNU / H_PLANCK * (lead + corr)
+    assert rel(bd.zpab(0), want) < 1e-9
+    assert rel(bd.zpab(0), AB_FNU / H_PLANCK * lead) > 1e-8  # the h^2 term is resolved
+
+
+# ------------------------------------------------------------------ P11
+def test_p11_colour_law_shape():
+    coef = np.array([0.0, 0.95, -0.21, 0.06, -0.008]) * 0.9210340371976184
+    m = grid_model(lambda p, l: 1.0, cl_coef=coef)
+    B, V, lo, hi = 4302.57, 5428.55, 2800.0, 7000.0
+    assert abs(m.colour_law(B)) < 1e-15  # a0 = 0
+    P = lambda l: sum(coef[q] * l ** q for q in range(5))
+    assert rel(m.colour_law(V), P(1.0)) < 1e-14
+    assert rel(m.colour_law(5000.0), P((5000.0 - B) / (V - B))) < 1e-14
+    eps = 1e-4
+    for edge in (lo, hi):
+        a, b_, c_ = m.colour_law(edge - eps), m.colour_law(edge), m.colour_law(edge + eps)
+        assert abs(a - 2 * b_ + c_) < 1e-9  # C1: no kink in value
+        assert abs((c_ - b_) - (b_ - a)) / eps < 1e-4  # slopes agree on both sides
+    for x in (1500.0, 2000.0, 2500.0, 7500.0, 9000.0, 15000.0):  # linear outside
+        d2 = m.colour_law(x - 100.0) - 2.0 * m.colour_law(x) + m.colour_law(x + 100.0)
+        assert abs(d2) < 1e-12
+    # and genuinely curved inside
+    assert abs(m.colour_law(4900.0) - 2.0 * m.colour_law(5000.0) + m.colour_law(5100.0)) > 1e-6
+
+
+# ------------------------------------------------------------------ P12
+@pytest.mark.parametrize("z,c", [(0.0, 0.2), (0.15, -0.3)])
+def test_p12_colour_integral_within_trapezoid_bound(z, c):
+    """Constant surface, top-hat, degree-1 colour law: closed-form integral of lam exp(c(al lam + be))."""
+    K, x0, a1 = 2.0, 1e-5, 0.8
+    B, V = 4302.57, 5428.55
+    m = grid_model(lambda p, l: K, n_wave=301, cl_coef=(0.0, a1), lo=1000.0, hi=20000.0)  # 3000..6000
+    la, lb, h = 4500.0, 5500.0, 5.0
+    bd = tophat(la, lb, h)
+    got = oracle.eval_one(m, bd, z, 0.2, 0, None, x0, 0.0, c, 0.0)
+    al = c * a1 / ((1.0 + z) * (V - B))
+    be = -c * a1 * B / (V - B)
+    prim = lambda x: math.exp(al * x + be) * (x / al - 1.0 / (al * al))
+    exact = x0 * K / HC * (prim(lb) - prim(la))
+    g2 = lambda x: abs(x0 * K / HC * math.exp(al * x + be) * (2.0 * al + al * al * x))
+    bound = h * h / 12.0 * (lb - la) * max(g2(la), g2(lb))
+    assert abs(got - exact) <= bound * 1.0000001
+    assert abs(got - exact) > 0.0
+
+
+# ------------------------------------------------------------------ P13
+def test_p13_out_of_range_is_zero_and_partial_overlap():
+    K = 1.5
+    m = grid_model(lambda p, l: K, n_wave=41)  # 3000..3400, phase -5..5
+    bd = tophat(3600.0, 3800.0, 5.0)  # entirely outside at z = 0
+    assert oracle.eval_one(m, bd, 0.0, 0.0, 0, None, 1e-5, 0.0, 0.0, 0.0) == 0.0
+    bd_in = tophat(3100.0, 3300.0, 5.0)
+    assert oracle.eval_one(m, bd_in, 0.0, 5.2, 0, None, 1e-5, 0.0, 0.0, 0.0) == 0.0  # phase > last node
+    assert oracle.eval_one(m, bd_in, 0.0, -5.2, 0, None, 1e-5, 0.0, 0.0, 0.0) == 0.0
+    assert oracle.eval_one(m, bd_in, 0.0, 5.0, 0, None, 1e-5, 0.0, 0.0, 0.0) > 0.0  # closed interval
+    # partial overlap: band 3300..3500, model ends at 3400 -> trapezoid of the zero-extended integrand
+    bd_p = tophat(3300.0, 3500.0, 5.0)
+    lam = 3300.0 + 5.0 * np.arange(41)
+    g = np.where(lam <= 3400.0, 1e-5 * K * lam / HC, 0.0)
+    want = np.trapezoid(g, lam)
+    got = oracle.eval_one(m, bd_p, 0.0, 0.0, 0, None, 1e-5, 0.0, 0.0, 0.0)
+    assert rel(got, want) < 1e-14
+    # invalid band index -> NaN, not a crash
+    assert math.isnan(oracle.eval_one(m, bd_p, 0.0, 0.0, 3, None, 1e-5, 0.0, 0.0, 0.0))
+
+
+# ------------------------------------------------------------------ batched runner helpers
+def _run(m, bd, n_sn, n_samples, obs_offset, time, band, zp, z, th, flux=None, fluxerr=None, **kw):
+    return oracle.run(m, bd, n_sn=n_sn, n_samples=n_samples, obs_offset=obs_offset, time=time, band=band,
+                      zp=zp, z=z, x0=th[0], x1=th[1], c=th[2], t0=th[3], flux=flux, fluxerr=fluxerr, **kw)
+
+
+def _small_batch():
+    m = rng_model(seed=11, n_phase=14, n_wave=90)  # phase -5..8, wave 3000..3890
+    m.m0[:] = np.abs(m.m0) + 0.5  # keep fluxes away from zero
+    w1 = 3500.0 + 5.0 * np.arange(41)
+    w2 = 3650.0 + 5.0 * np.arange(31)
+    bd = oracle.Bands(np.array([0, 41, 72]), np.concatenate([w1, w2]),
+                      np.concatenate([np.exp(-0.5 * ((w1 - 3600.0) / 40.0) ** 2),
+                                      np.exp(-0.5 * ((w2 - 3725.0) / 30.0) ** 2)]))
+    obs_offset = np.array([0, 3, 8], dtype=np.int32)  # ragged: 3 and 5 observations
+    time = np.array([-1.0, 0.5, 2.25, -2.0, 0.0, 1.0, 3.0, 4.5])
+    band = np.array([0, 1, 0, 1, 0, 1, 0, 1], dtype=np.int32)
+    zp = np.full(8, 25.0)
+    z = np.array([0.02, 0.08])
+    return m, bd, obs_offset, time, band, zp, z
+
+
+# ------------------------------------------------------------------ P14
+def test_p14_chi2_identities_and_layout():
+    m, bd, oo, time, band, zp, z = _small_batch()
+    n_samples = 3
+    rng = np.random.default_rng(5)
+    th = [np.array([1e-5, 2e-5, 3e-5, 1.5e-5, 2.5e-5, 0.5e-5]), rng.normal(size=6), 0.1 * rng.normal(size=6),
+          rng.uniform(-0.5, 0.5, size=6)]
+    out = _run(m, bd, 2, n_samples, oo, time, band, zp, z, th, want_flux=True)
+    fl = out["flux"]
+    assert fl.shape == (8 * n_samples,) and np.all(np.isfinite(fl))
+    # layout: SN s block starts at obs_offset[s]*n_samples; inside, [sample][obs], obs fastest
+    for s in range(2):
+        n_obs = oo[s + 1] - oo[s]
+        for k in range(n_samples):
+            u = s * n_samples + k
+            for i in range(n_obs):
+                want = oracle.eval_one(m, bd, z[s], time[oo[s] + i], int(band[oo[s] + i]), 25.0, th[0][u],
+                                       th[1][u], th[2][u], th[3][u])
+                assert fl[oo[s] * n_samples + k * n_obs + i] == want
+    # noise-free data at sample 1 of each SN: chi2 = 0 and zero gradient there
+    data = np.concatenate([fl[oo[s] * n_samples + 1 * (oo[s + 1] - oo[s]):][: oo[s + 1] - oo[s]] for s in range(2)])
+    sig = 0.05 * np.abs(data)
+    out = _run(m, bd, 2, n_samples, oo, time, band, zp, z, th, flux=data, fluxerr=sig, want_flux=False,
+               want_chi2=True, want_dchi2=True)
+    for s in range(2):
+        assert out["chi2"][s * n_samples + 1] == 0.0
+        assert np.all(out["dchi2"][s * n_samples + 1] == 0.0)
+        assert out["chi2"][s * n_samples + 0] > 0.0
+    # data = (1+eps) model with sigma = 5% model -> N (eps/0.05)^2
+    eps = 0.01
+    th1 = [a.reshape(2, n_samples)[:, 1].copy() for a in th]
+    model = _run(m, bd, 2, 1, oo, time, band, zp, z, th1)["flux"]
+    out = _run(m, bd, 2, 1, oo, time, band, zp, z, th1, flux=(1 + eps) * model, fluxerr=0.05 * np.abs(model),
+               want_flux=False, want_chi2=True)
+    for s in range(2):
+        n_obs = oo[s + 1] - oo[s]
+        assert rel(out["chi2"][s], n_obs * (eps / 0.05) ** 2) < 1e-12
+
+
+# ------------------------------------------------------------------ P15
+def test_p15_gradient_identities_and_central_differences():
+    m, bd, oo, time, band, zp, z = _small_batch()
+    x0, x1, c, t0 = 1.7e-5, 0.6, 0.07, 0.31
+    for zz, tt, b in [(0.02, 0.5, 0), (0.08, 3.0, 1), (0.05, -2.6, 0), (0.03, 2.0 + 1e-7, 1)]:
+        f = lambda a, b_, c_, d: oracle.eval_one(m, bd, zz, tt, b, 25.0, a, b_, c_, d)
+        val, dm = oracle.eval_one(m, bd, zz, tt, b, 25.0, x0, x1, c, t0, grad=True)
+        assert rel(dm[0], val / x0) < 1e-13
+        assert rel(dm[1], f(x0, x1 + 1.0, c, t0) - f(x0, x1, c, t0)) < 1e-11
+        # central differences, step rule G14
+        hs = [1e-6 * x0, 1e-6 * max(abs(x1), 1.0), 1e-6 * max(abs(c), 1.0), 1e-6 * max(abs(t0), 1.0)]
+        th = [x0, x1, c, t0]
+        for q in range(4):
+            up, dn = list(th), list(th)
+            up[q] += hs[q]
+            dn[q] -= hs[q]
+            fd = (f(*up) - f(*dn)) / (2.0 * hs[q])
+            scale = max(abs(dm[q]), abs(val) / max(abs(th[q]), 1.0))
+            assert abs(fd - dm[q]) <= 1e-6 * scale, (q, fd, dm[q])
+
+
+def test_p15_dchi2_matches_finite_difference_of_chi2():
+    m, bd, oo, time, band, zp, z = _small_batch()
+    th = [np.array([1e-5, 2e-5]), np.array([0.3, -0.8]), np.array([0.05, -0.02]), np.array([0.2, -0.4])]
+    model = _run(m, bd, 2, 1, oo, time, band, zp, z, th)["flux"]
+    rng = np.random.default_rng(9)
+    sig = 0.05 * np.abs(model)
+    data = model + sig * rng.standard_normal(8)
+    base = _run(m, bd, 2, 1, oo, time, band, zp, z, th, flux=data, fluxerr=sig, want_flux=False, want_chi2=True,
+                want_dchi2=True)
+    for q in range(4):
+        h = 1e-6 * np.maximum(np.abs(th[q]), 1.0) if q else 1e-6 * th[0]
+        up = [a.copy() for a in th]
+        dn = [a.copy() for a in th]
+        up[q] += h
+        dn[q] -= h
+        cu = _run(m, bd, 2, 1, oo, time, band, zp, z, up, flux=data, fluxerr=sig, want_flux=False, want_chi2=True)["chi2"]
+        cd = _run(m, bd, 2, 1, oo, time, band, zp, z, dn, flux=data, fluxerr=sig, want_flux=False, want_chi2=True)["chi2"]
+        fd = (cu - cd) / (2.0 * h)
+        an = base["dchi2"][:, q]
+        assert np.all(np.abs(fd - an) <= 2e-5 * np.maximum(np.abs(an), base["chi2"] / np.maximum(np.abs(th[q]), 1.0)))
+
+
+# ------------------------------------------------------------------ P16
+def _frac_interp1(g, u):
+    """O2 in exact rational arithmetic on unit-spaced nodes 0..n-1 (independent restatement)."""
+    n = len(g)
+    if u < 0 or u > n - 1:
+        return Fraction(0)
+    i = min(int(math.floor(u)), n - 2)
+    t = u - i
+    if i == 0 or i == n - 2:
+        return (1 - t) * g[i] + t * g[i + 1]
+    # Catmull-Rom written as a Hermite cubic (a different algebraic form from the oracle's weights)
+    m_i = (g[i + 1] - g[i - 1]) / 2
+    m_j = (g[i + 2] - g[i]) / 2
+    h00 = 2 * t ** 3 - 3 * t ** 2 + 1
+    h10 = t ** 3 - 2 * t ** 2 + t
+    h01 = -2 * t ** 3 + 3 * t ** 2
+    h11 = t ** 3 - t ** 2
+    return h00 * g[i] + h10 * m_i + h01 * g[i + 1] + h11 * m_j
+
+
+@pytest.mark.parametrize("n", [3, 6])
+def test_p16_exact_rational_brute_force(n):
+    rng = np.random.default_rng(100 + n)
+    ints0 = rng.integers(-9, 10, size=(n, n))
+    ints1 = rng.integers(-9, 10, size=(n, n))
+    phase = np.arange(n, dtype=np.float64)  # 0..n-1 d
+    wave = 1000.0 + 8.0 * np.arange(n)  # step 8 A (binary-exact arithmetic)
+    m = oracle.Model(phase, wave, ints0.astype(float), ints1.astype(float), np.zeros(5), 4302.57, 5428.55,
+                     2800.0, 7000.0)
+    z = Fraction(1, 4)
+    t, t0 = Fraction(9, 4) if n == 6 else Fraction(3, 2), Fraction(-7, 8) if n == 6 else Fraction(1, 4)
+    x0, x1 = Fraction(3, 1024), Fraction(-5, 8)
+    lam_obs = [Fraction(1270), Fraction(1270) + Fraction(5 * (n - 1), 2), Fraction(1270) + Fraction(9 * (n - 1), 2)]
+    T = [Fraction(1, 2), Fraction(3, 4), Fraction(1, 4)]
+    p = (t - t0) / (1 + z)
+    g = []
+    for lam, tr in zip(lam_obs, T):
+        lr = lam / (1 + z)
+        ul = (lr - 1000) / 8
+        up = p
+        col0 = [_frac_interp1([Fraction(int(v)) for v in ints0[k]], ul) for k in range(n)]
+        col1 = [_frac_interp1([Fraction(int(v)) for v in ints1[k]], ul) for k in range(n)]
+        M0, M1 = _frac_interp1(col0, up), _frac_interp1(col1, up)
+        g.append(x0 * (M0 + x1 * M1) * tr * lam)  # hc divided out below
+    raw = sum((g[j] + g[j + 1]) / 2 * (lam_obs[j + 1] - lam_obs[j]) for j in range(2))
+    assert raw != 0
+    bd = oracle.Bands(np.array([0, 3]), np.array([float(x) for x in lam_obs]), np.array([float(x) for x in T]))
+    got = oracle.eval_one(m, bd, float(z), float(t), 0, None, float(x0), float(x1), 0.0, float(t0))
+    assert rel(got, float(raw) / HC) < 1e-14
+
+
+# ------------------------------------------------------------------ P17
+@pytest.mark.parametrize("kappa", [1e-12, 1e-6, 1e3, 1e6])
+def test_p17_scale_invariance(kappa):
+    m, bd, *_ = _small_batch()
+    mk = oracle.Model(m.phase, m.wave, m.m0 * kappa, m.m1 * kappa, m.cl_coef, 4302.57, 5428.55, 2800.0, 7000.0)
+    a = oracle.eval_one(m, bd, 0.05, 1.2, 0, 25.0, 1e-5, 0.4, 0.05, 0.1)
+    b = oracle.eval_one(mk, bd, 0.05, 1.2, 0, 25.0, 1e-5 / kappa, 0.4, 0.05, 0.1)
+    assert rel(a, b) < 1e-14
+
+
+# ------------------------------------------------------------------ constants and threading
+def test_constants_and_thread_invariance():
+    assert rel(oracle.lib().sbo_const_hc(), 1.9864458571489287e-8) < 1e-15
+    m, bd, oo, time, band, zp, z = _small_batch()
+    th = [np.array([1e-5, 2e-5]), np.array([0.3, -0.8]), np.array([0.05, -0.02]), np.array([0.2, -0.4])]
+    a = _run(m, bd, 2, 1, oo, time, band, zp, z, th, threads=1)["flux"]
+    b = _run(m, bd, 2, 1, oo, time, band, zp, z, th, threads=4)["flux"]
+    assert np.array_equal(a, b)
