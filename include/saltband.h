@@ -1,0 +1,144 @@
+/* saltband.h -- C ABI of the B200-native SALT3 batched band-flux library (libsaltband.so).
+ *
+ * The operations are those of the JAX-bandflux paper (arXiv 2504.08081; PAPER.md) as fixed by
+ * BASELINE.json `north_star` and the readings G0-G15 listed in DESIGN.md:
+ *
+ *   PAPER.md:19-23  F(p, lam) = x0 [M0(p,lam) + x1 M1(p,lam)] exp(c CL(lam)); free parameters
+ *                   x0, x1, t0, c; p is a function of redshift and t - t0
+ *   PAPER.md:38-43  bandflux = int F(lam) T(lam) lam/(hc) dlam over the band
+ *   PAPER.md:45     "trapezoidal integration along the wavelength dimension"; batching over data
+ *                   instances
+ *   PAPER.md:47     dedicated interpolation routines for the SALT3 / SALT3-NIR surfaces
+ *   north_star      p = (t - t0)/(1+z), lam_rest = lam_obs/(1+z); bicubic interpolation on the
+ *                   (phase, wavelength) grid; zero-point normalisation; chi^2 per supernova;
+ *                   analytic gradient with respect to (x0, x1, c, t0)
+ *
+ * One evaluation ("eval") = one (supernova s, parameter sample k, observation i):
+ *
+ *   m = S_i * x0 * sum_j w_j * [M0(p, l_j) + x1 M1(p, l_j)] * exp(c CL(l_j)) * T_j * lam_j/(hc)
+ *       p = (t_i - t0)/(1+z_s),  l_j = lam_j/(1+z_s),  lam_j, T_j = grid/transmission of band b_i,
+ *       w_j = trapezoid weights of that grid, S_i = 10^(0.4 zp_i)/ZPAB_b (1 if zp == NULL),
+ *       ZPAB_b = the same trapezoid of (3.631e-20 erg/s/cm^2/Hz * c/lam^2) T lam/(hc)        [G7]
+ *   M(p, l): separable cubic convolution (Keys a = -1/2) on the uniform model grid, linear in the
+ *       first/last cell of each axis, zero outside the closed grid range                [G1-G3]
+ *   CL(l): polynomial in (l - cl_wave_b)/(cl_wave_v - cl_wave_b) on [cl_lo, cl_hi], continued
+ *       linearly (value and slope) outside                                                 [G5]
+ *
+ * Conventions
+ *   - Loaders take HOST pointers and copy; compute calls take DEVICE pointers owned by the caller
+ *     (e.g. torch tensors) and a cudaStream_t passed as void*.  Compute calls only enqueue work:
+ *     no allocation visible to the caller, no host synchronisation, no retained pointers.
+ *   - dtype selects the element type of every floating-point array of a compute call (inputs and
+ *     outputs): SB_F32 (production: per-sample arithmetic in fp32) or SB_F64 (verification).
+ *   - All functions return SB_OK (0) or a negative sb_status; sb_strerror() names it.  Device data
+ *     are not validated (that would need a sync): a band index outside [0, n_bands) gives NaN for
+ *     that evaluation; fluxerr <= 0 propagates inf/NaN into chi^2; a phase or wavelength outside
+ *     the model grid is not an error and contributes zero flux [G3].
+ *   - No global mutable state.  Handles are immutable after creation; concurrent compute calls on
+ *     distinct streams with the same handles are allowed.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns SB_ECUDA.
+ */
+#ifndef SALTBAND_H
+#define SALTBAND_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sb_model sb_model; /* opaque: device-resident M0, M1 tables and the colour law */
+typedef struct sb_bands sb_bands; /* opaque: device-resident band tables, folded weights, ZPAB */
+
+typedef enum { SB_F32 = 0, SB_F64 = 1 } sb_dtype;
+
+typedef enum {
+    SB_OK = 0,
+    SB_EINVAL = -1, /* NULL pointer, bad count, non-uniform / non-increasing grid, non-finite table */
+    SB_ENOMEM = -2, /* host or device allocation failed */
+    SB_ECUDA = -3,  /* no device, or a copy / launch failed (see sb_last_cuda_error) */
+    SB_ELIMIT = -4  /* a table exceeds what the kernels stage on chip */
+} sb_status;
+
+/* sb_load_model -- PAPER.md:19-23, 47 (the M0/M1 surfaces and CL of the SALT model).
+ *   phase[n_phase], wave[n_wave]  HOST, uniform (|spacing deviation| <= 1e-9 relative), strictly
+ *                                 increasing, n_phase >= 2, n_wave >= 2 (days; Angstrom, rest frame)
+ *   m0, m1                        HOST, row-major [n_phase][n_wave], wavelength fastest, finite
+ *   cl_coef[n_cl]                 HOST, CL(l) = sum_q cl_coef[q] r^q, r = (l - cl_wave_b)/(cl_wave_v -
+ *                                 cl_wave_b); 1 <= n_cl <= 8; natural exponent exp(c*CL)    [G5]
+ *   cl_lo < cl_hi                 range (Angstrom, rest frame) outside which CL continues linearly
+ *   out                           receives the handle; free with sb_free_model.
+ * Copies everything (fp64 and fp32 device tables); the caller keeps ownership of its arrays. */
+int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int32_t n_wave,
+                  const double *m0, const double *m1, const double *cl_coef, int32_t n_cl,
+                  double cl_wave_b, double cl_wave_v, double cl_lo, double cl_hi, sb_model **out);
+
+/* sb_load_bandpasses -- PAPER.md:38-43, 47 (tabulated transmission T(lam) per filter).
+ *   CSR-packed HOST arrays: band b owns [offset[b], offset[b+1]) of wave/trans; each band has
+ *   >= 2 points, wave strictly increasing (observer frame, Angstrom; uniform spacing not
+ *   required), trans finite.  Precomputes in fp64 the trapezoid weights w_j, the
+ *   folded weights w_j T_j lam_j/(hc) and ZPAB_b [G7].  Copies; caller keeps ownership. */
+int sb_load_bandpasses(int32_t n_bands, const int64_t *offset, const double *wave,
+                       const double *trans, sb_bands **out);
+
+void sb_free_model(sb_model *m); /* NULL is allowed */
+void sb_free_bands(sb_bands *b); /* NULL is allowed */
+
+/* One batch of evaluations.  Every pointer is a DEVICE pointer owned by the caller.
+ * "unit" u = s*n_samples + k is one (supernova, parameter sample). */
+typedef struct {
+    int32_t dtype;             /* sb_dtype of time, zp, z, x0, x1, c, t0 and of all outputs */
+    int32_t n_sn;              /* supernovae, >= 0 */
+    int32_t n_samples;         /* parameter samples per supernova, >= 1 */
+    int32_t n_obs_total;       /* = obs_offset[n_sn] (host copy, so no sync is needed) */
+    const int32_t *obs_offset; /* [n_sn+1] CSR into the observation arrays; ragged allowed */
+    const void *time;          /* [n_obs_total] observer-frame time t_i (days) */
+    const int32_t *band;       /* [n_obs_total] index into sb_bands */
+    const void *zp;            /* [n_obs_total] zero point, or NULL => S_i = 1 (raw photon flux) */
+    const void *z;             /* [n_sn] redshift, > -1 */
+    const void *x0, *x1, *c, *t0; /* [n_sn*n_samples], sample fastest */
+} sb_batch;
+
+/* sb_bandflux -- the band flux m of every evaluation.
+ *   out_flux  DEVICE [n_obs_total*n_samples]: supernova s occupies the block starting at
+ *             obs_offset[s]*n_samples, laid out [n_samples][n_obs(s)], observation fastest. */
+int sb_bandflux(const sb_model *m, const sb_bands *b, const sb_batch *batch, void *out_flux,
+                void *stream);
+
+/* sb_chi2 -- chi^2 per unit: sum_i ((flux_i - m_i)/fluxerr_i)^2 over the supernova's observations
+ * (north_star; reading G10: diagonal, data errors only).  Summation order is fixed, so repeated
+ * calls are bit-identical.
+ *   flux, fluxerr  DEVICE [n_obs_total] measured flux and its 1-sigma error
+ *   out_chi2       DEVICE [n_sn*n_samples]
+ *   out_flux       DEVICE, layout as in sb_bandflux, or NULL */
+int sb_chi2(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+            const void *fluxerr, void *out_chi2, void *out_flux, void *stream);
+
+/* sb_bandflux_grad -- forward plus analytic gradient with respect to (x0, x1, c, t0), in that
+ * order (north_star; "fully differentiable").
+ *   out_flux   DEVICE, layout as in sb_bandflux, or NULL
+ *   out_dflux  DEVICE [n_obs_total*n_samples][4] d m / d(x0, x1, c, t0), same eval order, or NULL
+ *   flux, fluxerr  DEVICE [n_obs_total], required iff out_chi2 or out_dchi2 is non-NULL
+ *   out_chi2   DEVICE [n_sn*n_samples] or NULL
+ *   out_dchi2  DEVICE [n_sn*n_samples][4] = -2 sum_i (flux_i - m_i)/fluxerr_i^2 * dm_i, or NULL
+ * The derivative with respect to t0 is that of the interpolation cell selected by the phase
+ * (reading G11); it is zero outside the grid. */
+int sb_bandflux_grad(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+                     const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2,
+                     void *out_dchi2, void *stream);
+
+/* Introspection (host side, cheap). */
+int32_t sb_bands_count(const sb_bands *b);
+/* ZPAB_b as computed at load (fp64), or NaN for a bad index. */
+double sb_bands_zpab(const sb_bands *b, int32_t band);
+/* Number of kernels launched by the calling thread's most recent compute call (0 if it failed). */
+int32_t sb_last_launch_count(void);
+/* cudaError_t of the calling thread's most recent failing CUDA call (0 if none). */
+int32_t sb_last_cuda_error(void);
+const char *sb_strerror(int status);
+const char *sb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SALTBAND_H */

@@ -1,0 +1,377 @@
+// saltband.cu -- C ABI of libsaltband (include/saltband.h): loaders, argument checks, launches.
+// Product code; shares nothing with oracle/.  Build: see paper_2504_08081_b200/build.py.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "sb_internal.h"
+#include "sb_kernels.cuh"
+
+namespace {
+
+thread_local int32_t tl_launches = 0;
+thread_local int32_t tl_cuda_err = 0;
+
+bool cuda_ok(cudaError_t e)
+{
+    if (e == cudaSuccess) return true;
+    tl_cuda_err = (int32_t)e;
+    return false;
+}
+
+template <typename T> bool upload(T **dst, const std::vector<T> &src)
+{
+    *dst = nullptr;
+    size_t bytes = src.size() * sizeof(T);
+    if (bytes == 0) bytes = sizeof(T);
+    if (!cuda_ok(cudaMalloc((void **)dst, bytes))) return false;
+    if (!src.empty() && !cuda_ok(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice)))
+        return false;
+    return true;
+}
+
+bool uniform_increasing(const double *x, int32_t n)
+{
+    if (n < 2) return false;
+    for (int32_t i = 0; i < n; ++i)
+        if (!std::isfinite(x[i])) return false;
+    const double step = (x[n - 1] - x[0]) / (double)(n - 1);
+    if (!(step > 0.0)) return false;
+    for (int32_t i = 1; i < n; ++i) {
+        const double d = x[i] - x[i - 1];
+        if (!(d > 0.0) || std::fabs(d - step) > 1e-9 * step) return false;
+    }
+    return true;
+}
+
+double poly_val(const double *a, int n, double x)
+{
+    double s = 0.0;
+    for (int q = n - 1; q >= 0; --q) s = s * x + a[q];
+    return s;
+}
+double poly_der(const double *a, int n, double x)
+{
+    double s = 0.0;
+    for (int q = n - 1; q >= 1; --q) s = s * x + (double)q * a[q];
+    return s;
+}
+
+int device_smem_optin()
+{
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) return 0;
+    return v;
+}
+int device_sm_count()
+{
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+    return v;
+}
+
+} // namespace
+
+extern "C" {
+
+const char *sb_version(void) { return "saltband 0.1 (sm_100a)"; }
+
+const char *sb_strerror(int status)
+{
+    switch (status) {
+    case SB_OK: return "ok";
+    case SB_EINVAL: return "invalid argument";
+    case SB_ENOMEM: return "out of memory";
+    case SB_ECUDA: return "CUDA error (no device, or a copy/launch failed)";
+    case SB_ELIMIT: return "table exceeds on-chip staging limits";
+    default: return "unknown status";
+    }
+}
+
+int32_t sb_last_launch_count(void) { return tl_launches; }
+int32_t sb_last_cuda_error(void) { return tl_cuda_err; }
+
+int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int32_t n_wave, const double *m0,
+                  const double *m1, const double *cl_coef, int32_t n_cl, double cl_wave_b, double cl_wave_v,
+                  double cl_lo, double cl_hi, sb_model **out)
+{
+    if (out) *out = nullptr;
+    if (!phase || !wave || !m0 || !m1 || !cl_coef || !out) return SB_EINVAL;
+    if (n_phase < 2 || n_wave < 2 || n_cl < 1 || n_cl > SB_MAX_CL) return SB_EINVAL;
+    if (!uniform_increasing(phase, n_phase) || !uniform_increasing(wave, n_wave)) return SB_EINVAL;
+    if (!std::isfinite(cl_wave_b) || !std::isfinite(cl_wave_v) || cl_wave_b == cl_wave_v) return SB_EINVAL;
+    if (!std::isfinite(cl_lo) || !std::isfinite(cl_hi) || !(cl_lo < cl_hi)) return SB_EINVAL;
+    for (int q = 0; q < n_cl; ++q)
+        if (!std::isfinite(cl_coef[q])) return SB_EINVAL;
+    const size_t n = (size_t)n_phase * (size_t)n_wave;
+    for (size_t i = 0; i < n; ++i)
+        if (!std::isfinite(m0[i]) || !std::isfinite(m1[i])) return SB_EINVAL;
+    if ((long long)n_phase * ((long long)n_wave + 4) >= (1LL << 30)) return SB_ELIMIT;
+
+    sb_model *h = new (std::nothrow) sb_model();
+    if (!h) return SB_ENOMEM;
+    memset(h, 0, sizeof(*h));
+    SbModelParams &p = h->prm;
+    p.n_phase = n_phase;
+    p.n_wave = n_wave;
+    p.ld = (n_wave + 3) & ~3;
+    p.n_cl = n_cl;
+    p.p0 = phase[0];
+    p.dp = (phase[n_phase - 1] - phase[0]) / (double)(n_phase - 1);
+    p.l0 = wave[0];
+    p.dl = (wave[n_wave - 1] - wave[0]) / (double)(n_wave - 1);
+    for (int q = 0; q < SB_MAX_CL; ++q) p.cl[q] = q < n_cl ? cl_coef[q] : 0.0;
+    p.cl_b = cl_wave_b;
+    p.cl_inv_span = 1.0 / (cl_wave_v - cl_wave_b);
+    double r_lo = (cl_lo - cl_wave_b) * p.cl_inv_span, r_hi = (cl_hi - cl_wave_b) * p.cl_inv_span;
+    if (r_lo > r_hi) { double t = r_lo; r_lo = r_hi; r_hi = t; } // cl_wave_v < cl_wave_b flips the axis
+    p.r_lo = r_lo;
+    p.r_hi = r_hi;
+    p.p_lo = poly_val(p.cl, n_cl, r_lo);
+    p.s_lo = poly_der(p.cl, n_cl, r_lo);
+    p.p_hi = poly_val(p.cl, n_cl, r_hi);
+    p.s_hi = poly_der(p.cl, n_cl, r_hi);
+
+    std::vector<double> t0((size_t)n_phase * p.ld, 0.0), t1((size_t)n_phase * p.ld, 0.0);
+    for (int k = 0; k < n_phase; ++k)
+        for (int l = 0; l < n_wave; ++l) {
+            t0[(size_t)k * p.ld + l] = m0[(size_t)k * n_wave + l];
+            t1[(size_t)k * p.ld + l] = m1[(size_t)k * n_wave + l];
+        }
+    std::vector<float> f0(t0.begin(), t0.end()), f1(t1.begin(), t1.end());
+    cudaGetDevice(&h->device);
+    if (!upload(&h->m0_f64, t0) || !upload(&h->m1_f64, t1) || !upload(&h->m0_f32, f0) || !upload(&h->m1_f32, f1)) {
+        sb_free_model(h);
+        return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+    }
+    *out = h;
+    return SB_OK;
+}
+
+void sb_free_model(sb_model *m)
+{
+    if (!m) return;
+    cudaFree(m->m0_f32);
+    cudaFree(m->m1_f32);
+    cudaFree(m->m0_f64);
+    cudaFree(m->m1_f64);
+    delete m;
+}
+
+int sb_load_bandpasses(int32_t n_bands, const int64_t *offset, const double *wave, const double *trans,
+                       sb_bands **out)
+{
+    if (out) *out = nullptr;
+    if (!offset || !wave || !trans || !out || n_bands < 1) return SB_EINVAL;
+    if (offset[0] != 0) return SB_EINVAL;
+    for (int b = 0; b < n_bands; ++b)
+        if (offset[b + 1] - offset[b] < 2) return SB_EINVAL;
+    const int64_t total = offset[n_bands];
+    if (total >= (1LL << 30)) return SB_ELIMIT;
+    for (int64_t i = 0; i < total; ++i)
+        if (!std::isfinite(wave[i]) || !std::isfinite(trans[i]) || !(wave[i] > 0.0)) return SB_EINVAL;
+    for (int b = 0; b < n_bands; ++b)
+        for (int64_t i = offset[b] + 1; i < offset[b + 1]; ++i)
+            if (!(wave[i] > wave[i - 1])) return SB_EINVAL;
+
+    sb_bands *h = new (std::nothrow) sb_bands();
+    if (!h) return SB_ENOMEM;
+    memset(h, 0, sizeof(*h));
+    h->n_bands = n_bands;
+    h->n_total = (int32_t)total;
+    h->h_zpab = (double *)malloc(sizeof(double) * (size_t)n_bands);
+    if (!h->h_zpab) { delete h; return SB_ENOMEM; }
+
+    const double hc = SB_H_PLANCK * SB_C_ANGSTROM;
+    std::vector<int32_t> off(n_bands + 1);
+    std::vector<double> lam_first(n_bands), zpab_inv(n_bands), dlam(total), w(total);
+    for (int b = 0; b <= n_bands; ++b) off[b] = (int32_t)offset[b];
+    for (int b = 0; b < n_bands; ++b) {
+        const int64_t lo = offset[b], n = offset[b + 1] - lo;
+        const double *lam = wave + lo, *tr = trans + lo;
+        if ((int32_t)n > h->max_n) h->max_n = (int32_t)n;
+        if (lam[n - 1] - lam[0] > h->max_span) h->max_span = lam[n - 1] - lam[0];
+        lam_first[b] = lam[0];
+        double zp = 0.0;
+        for (int64_t j = 0; j < n; ++j) {
+            // trapezoid weight of node j: half the distance between its neighbours
+            const double left = j > 0 ? lam[j] - lam[j - 1] : 0.0;
+            const double right = j + 1 < n ? lam[j + 1] - lam[j] : 0.0;
+            const double wq = 0.5 * (left + right);
+            dlam[lo + j] = lam[j] - lam[0];
+            w[lo + j] = wq * tr[j] * lam[j] / hc; // folded: w_j T_j lam_j/(hc)
+            zp += wq * (SB_AB_FNU * SB_C_ANGSTROM / (lam[j] * lam[j])) * tr[j] * lam[j] / hc; // G7
+        }
+        h->h_zpab[b] = zp;
+        zpab_inv[b] = 1.0 / zp;
+    }
+    std::vector<float> dlam_f(dlam.begin(), dlam.end()), w_f(w.begin(), w.end());
+    cudaGetDevice(&h->device);
+    if (!upload(&h->d_off, off) || !upload(&h->d_lam_first, lam_first) || !upload(&h->d_zpab_inv, zpab_inv) ||
+        !upload(&h->d_dlam_f64, dlam) || !upload(&h->d_w_f64, w) || !upload(&h->d_dlam_f32, dlam_f) ||
+        !upload(&h->d_w_f32, w_f)) {
+        sb_free_bands(h);
+        return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+    }
+    *out = h;
+    return SB_OK;
+}
+
+void sb_free_bands(sb_bands *b)
+{
+    if (!b) return;
+    cudaFree(b->d_off);
+    cudaFree(b->d_lam_first);
+    cudaFree(b->d_zpab_inv);
+    cudaFree(b->d_dlam_f32);
+    cudaFree(b->d_w_f32);
+    cudaFree(b->d_dlam_f64);
+    cudaFree(b->d_w_f64);
+    free(b->h_zpab);
+    delete b;
+}
+
+int32_t sb_bands_count(const sb_bands *b) { return b ? b->n_bands : 0; }
+double sb_bands_zpab(const sb_bands *b, int32_t band)
+{
+    if (!b || band < 0 || band >= b->n_bands) return NAN;
+    return b->h_zpab[band];
+}
+
+} // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// Launch
+// ------------------------------------------------------------------------------------------
+namespace {
+
+template <typename T, bool GRAD, int NCL, bool STAGE, int NWARPS>
+int launch_inst(const SbKParams &kp, size_t smem, int grid, cudaStream_t st)
+{
+    auto kern = sb::sb_fused_kernel<T, GRAD, NCL, STAGE, NWARPS>;
+    if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) return SB_ECUDA;
+    kern<<<grid, NWARPS * 32, smem, st>>>(kp);
+    if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
+    tl_launches += 1;
+    return SB_OK;
+}
+
+template <typename T, bool GRAD, int NWARPS>
+int launch_typed(SbKParams &kp, const sb_bands *b, cudaStream_t st)
+{
+    const int smem_max = device_smem_optin();
+    const int n_sm = device_sm_count();
+    if (smem_max <= 0 || n_sm <= 0) return SB_ECUDA;
+    constexpr int NSET = GRAD ? 3 : 1;
+    const size_t cell_bytes = sizeof(T) * 4 * NSET;
+    const size_t red_bytes = sizeof(double) * 5 * NWARPS;
+    const size_t band_bytes = 2 * sizeof(T) * (size_t)((b->n_total + 3) & ~3);
+    // entries needed by the widest band at z >= 0 (narrower tiles still work: the kernel loops)
+    int tc_full = (int)std::ceil(b->max_span / kp.mp.dl) + 6;
+    tc_full = (tc_full + 1) & ~1;
+    if (tc_full > kp.mp.n_wave + 4) tc_full = (kp.mp.n_wave + 5) & ~1;
+    if (tc_full < 16) tc_full = 16;
+    // stage the band tables in shared memory when they fit beside >= 64-entry row buffers (fp32 only)
+    bool stage = sizeof(T) == 4 && band_bytes + red_bytes + (size_t)NWARPS * 64 * cell_bytes <= (size_t)smem_max;
+    size_t avail = (size_t)smem_max - red_bytes - (stage ? band_bytes : 0);
+    int tc = (int)(avail / ((size_t)NWARPS * cell_bytes));
+    tc &= ~1;
+    if (tc > tc_full) tc = tc_full;
+    if (tc < 16) return SB_ELIMIT;
+    kp.tile_cells = tc;
+    const size_t smem = (size_t)NWARPS * tc * cell_bytes + red_bytes + (stage ? band_bytes : 0);
+    const long long n_units = (long long)kp.n_sn * kp.n_samples;
+    int grid = (int)(n_units < (long long)n_sm ? n_units : (long long)n_sm);
+    if (grid < 1) return SB_OK;
+    const bool small_cl = kp.mp.n_cl <= 5;
+    if (stage) {
+        if (small_cl) return launch_inst<T, GRAD, 5, sizeof(T) == 4, NWARPS>(kp, smem, grid, st);
+        return launch_inst<T, GRAD, SB_MAX_CL, sizeof(T) == 4, NWARPS>(kp, smem, grid, st);
+    }
+    if (small_cl) return launch_inst<T, GRAD, 5, false, NWARPS>(kp, smem, grid, st);
+    return launch_inst<T, GRAD, SB_MAX_CL, false, NWARPS>(kp, smem, grid, st);
+}
+
+int run(const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux, const void *fluxerr,
+        void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2, void *stream, bool grad)
+{
+    tl_launches = 0;
+    if (!m || !b || !bt) return SB_EINVAL;
+    if (bt->dtype != SB_F32 && bt->dtype != SB_F64) return SB_EINVAL;
+    if (bt->n_sn < 0 || bt->n_samples < 1 || bt->n_obs_total < 0) return SB_EINVAL;
+    if ((out_chi2 || out_dchi2) && (!flux || !fluxerr)) return SB_EINVAL;
+    if (bt->n_sn == 0) return SB_OK;
+    if (!bt->obs_offset || !bt->z || !bt->x0 || !bt->x1 || !bt->c || !bt->t0) return SB_EINVAL;
+    if (bt->n_obs_total > 0 && (!bt->time || !bt->band)) return SB_EINVAL;
+    if (!out_flux && !out_dflux && !out_chi2 && !out_dchi2) return SB_EINVAL;
+    if ((long long)bt->n_sn * bt->n_samples >= (1LL << 31)) return SB_ELIMIT;
+
+    SbKParams kp;
+    memset(&kp, 0, sizeof(kp));
+    kp.mp = m->prm;
+    const bool f32 = bt->dtype == SB_F32;
+    kp.m0 = f32 ? (const void *)m->m0_f32 : (const void *)m->m0_f64;
+    kp.m1 = f32 ? (const void *)m->m1_f32 : (const void *)m->m1_f64;
+    kp.n_bands = b->n_bands;
+    kp.n_band_total = b->n_total;
+    kp.band_off = b->d_off;
+    kp.band_lam_first = b->d_lam_first;
+    kp.band_zpab_inv = b->d_zpab_inv;
+    kp.band_dlam = f32 ? (const void *)b->d_dlam_f32 : (const void *)b->d_dlam_f64;
+    kp.band_w = f32 ? (const void *)b->d_w_f32 : (const void *)b->d_w_f64;
+    kp.n_sn = bt->n_sn;
+    kp.n_samples = bt->n_samples;
+    kp.obs_offset = bt->obs_offset;
+    kp.time = bt->time;
+    kp.zp = bt->zp;
+    kp.z = bt->z;
+    kp.x0 = bt->x0;
+    kp.x1 = bt->x1;
+    kp.c = bt->c;
+    kp.t0 = bt->t0;
+    kp.band = bt->band;
+    kp.flux = flux;
+    kp.fluxerr = fluxerr;
+    kp.out_flux = out_flux;
+    kp.out_dflux = out_dflux;
+    kp.out_chi2 = out_chi2;
+    kp.out_dchi2 = out_dchi2;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (f32) {
+        if (grad) return launch_typed<float, true, 8>(kp, b, st);
+        return launch_typed<float, false, 16>(kp, b, st);
+    }
+    if (grad) return launch_typed<double, true, 8>(kp, b, st);
+    return launch_typed<double, false, 8>(kp, b, st);
+}
+
+} // namespace
+
+extern "C" {
+
+int sb_bandflux(const sb_model *m, const sb_bands *b, const sb_batch *batch, void *out_flux, void *stream)
+{
+    if (!out_flux && !(batch && batch->n_sn == 0)) { tl_launches = 0; return SB_EINVAL; }
+    return run(m, b, batch, nullptr, nullptr, out_flux, nullptr, nullptr, nullptr, stream, false);
+}
+
+int sb_chi2(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux, const void *fluxerr,
+            void *out_chi2, void *out_flux, void *stream)
+{
+    if ((!out_chi2 || !flux || !fluxerr) && !(batch && batch->n_sn == 0)) { tl_launches = 0; return SB_EINVAL; }
+    return run(m, b, batch, flux, fluxerr, out_flux, nullptr, out_chi2, nullptr, stream, false);
+}
+
+int sb_bandflux_grad(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+                     const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2,
+                     void *stream)
+{
+    return run(m, b, batch, flux, fluxerr, out_flux, out_dflux, out_chi2, out_dchi2, stream, true);
+}
+
+} // extern "C"

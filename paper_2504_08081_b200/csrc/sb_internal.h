@@ -1,0 +1,62 @@
+// sb_internal.h -- private definitions of libsaltband (handles, kernel parameter blocks).
+// Product code: shares nothing with oracle/.  Public ABI: include/saltband.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "saltband.h"
+
+#define SB_MAX_CL 8
+
+// Physical constants (CGS, Angstrom) -- PAPER.md:41 "h and c are the Planck constant and the speed
+// of light"; AB reference flux density for the zero point (G7).
+#define SB_H_PLANCK 6.62607015e-27
+#define SB_C_ANGSTROM 2.99792458e18
+#define SB_AB_FNU 3.631e-20
+
+// Model geometry + colour law, passed to kernels by value.
+struct SbModelParams {
+    int32_t n_phase, n_wave, ld, n_cl; // ld = row stride (elements) of the device tables
+    double p0, dp;                     // phase grid origin / step (days)
+    double l0, dl;                     // wavelength grid origin / step (Angstrom, rest frame)
+    double cl[SB_MAX_CL];              // colour-law coefficients, zero padded
+    double cl_b, cl_inv_span;          // reduced wavelength r = (l - cl_b) * cl_inv_span
+    double r_lo, r_hi;                 // images of cl_lo, cl_hi
+    double p_lo, s_lo, p_hi, s_hi;     // polynomial value and slope at r_lo, r_hi
+};
+
+struct sb_model {
+    SbModelParams prm;
+    float *m0_f32, *m1_f32;   // [n_phase][ld]
+    double *m0_f64, *m1_f64;  // [n_phase][ld]
+    int device;
+};
+
+struct sb_bands {
+    int32_t n_bands, n_total, max_n;
+    int32_t *d_off;        // [n_bands+1]
+    double *d_lam_first;   // [n_bands] first wavelength of each band grid
+    double *d_zpab_inv;    // [n_bands] 1 / ZPAB_b
+    float *d_dlam_f32, *d_w_f32;   // [n_total] lam_j - lam_first ; folded weight w_j T_j lam_j/(hc)
+    double *d_dlam_f64, *d_w_f64;
+    double *h_zpab;        // host copy [n_bands]
+    double max_span;       // max over bands of (lam_last - lam_first)
+    int device;
+};
+
+// Kernel parameter block.
+struct SbKParams {
+    SbModelParams mp;
+    const void *m0, *m1;              // tables of the kernel's real type
+    int32_t n_bands, n_band_total;
+    const int32_t *band_off;
+    const double *band_lam_first, *band_zpab_inv;
+    const void *band_dlam, *band_w;   // real type
+    int32_t n_sn, n_samples;
+    const int32_t *obs_offset;
+    const void *time, *zp, *z, *x0, *x1, *c, *t0;
+    const int32_t *band;
+    const void *flux, *fluxerr;       // may be NULL
+    void *out_flux, *out_dflux, *out_chi2, *out_dchi2; // may be NULL
+    int32_t tile_cells;               // coefficient-row entries per warp buffer
+};

@@ -1,0 +1,145 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the fp64 oracle, element by
+element, on the same seeded inputs (BASELINE.json configs, reduced to sizes the oracle finishes in
+seconds but spanning many CTAs, warps, tiles and ragged tails), plus edge cases.
+Tolerances: DESIGN.md reading G13 (tests/sbgpu.py); fp32 1e-5 rel + 1e-9 peak, fp64 1e-12."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+import sbgpu
+
+pytestmark = pytest.mark.gpu
+
+
+def theta_true_rep(wl):
+    return {k: v.copy() for k, v in wl.theta_true.items()}
+
+
+def prepare(config, **kw):
+    """Workload with photometry attached from the ORACLE's flux at theta_true."""
+    wl = workloads.make_workload(config, **kw)
+    ref_true = oracle.run_workload(wl, theta=theta_true_rep(wl), want_flux=True)["flux"]
+    workloads.attach_data(wl, ref_true)
+    return wl
+
+
+def oracle_all(wl, grad=False):
+    return oracle.run_workload(wl, want_flux=True, want_chi2=True, want_dflux=grad, want_dchi2=grad)
+
+
+def check_flux_chi2(wl, got, ref, fp64):
+    ns = wl.n_samples
+    tol = sbgpu.flux_tolerance(wl, ref["flux"], ns, fp64)
+    err = np.abs(got["flux"] - ref["flux"])
+    bad = np.nonzero(~(err <= tol))[0]
+    assert bad.size == 0, f"{bad.size} flux mismatches, worst ratio {np.max(err / np.maximum(tol, 1e-300)):.3g}"
+    if "chi2" in got:
+        tolc = sbgpu.chi2_tolerance(wl, ref["flux"], tol, ns, fp64)
+        errc = np.abs(got["chi2"] - ref["chi2"])
+        assert np.all(errc <= tolc), f"chi2 worst ratio {np.max(errc / np.maximum(tolc, 1e-300)):.3g}"
+    return float(np.max(err / np.maximum(tol, 1e-300)))
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_config1_full(cuda_device, fp64):
+    wl = prepare(1)
+    ref = oracle_all(wl)
+    got = sbgpu.run_gpu(wl, mode="chi2", fp64=fp64)
+    assert got["launches"] >= 1
+    check_flux_chi2(wl, got, ref, fp64)
+    only_flux = sbgpu.run_gpu(wl, mode="flux", fp64=fp64)
+    assert np.array_equal(only_flux["flux"], got["flux"])
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_config2_full_and_ragged(cuda_device, fp64):
+    wl = prepare(2)  # 1024 SN x 60 obs: full size
+    ref = oracle_all(wl)
+    got = sbgpu.run_gpu(wl, mode="chi2", fp64=fp64)
+    check_flux_chi2(wl, got, ref, fp64)
+    assert np.mean(ref["flux"] == 0.0) < 0.2
+    wlr = prepare(2, n_sn=97, ragged=True)
+    check_flux_chi2(wlr, sbgpu.run_gpu(wlr, mode="chi2", fp64=fp64), oracle_all(wlr), fp64)
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_config3_samples_axis(cuda_device, fp64):
+    wl = prepare(3, n_samples=300)  # 1 SN x 300 samples x 50 obs
+    ref = oracle_all(wl)
+    got = sbgpu.run_gpu(wl, mode="chi2", fp64=fp64)
+    check_flux_chi2(wl, got, ref, fp64)
+    # chi2 only (no flux output), as the nested-sampling likelihood is called
+    got2 = sbgpu.run_gpu(wl, mode="chi2", fp64=fp64, want_flux=False)
+    assert np.array_equal(got2["chi2"], got["chi2"])
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_config4_forward_and_gradient(cuda_device, fp64):
+    wl = prepare(4, n_sn=160)
+    ref = oracle_all(wl, grad=True)
+    got = sbgpu.run_gpu(wl, mode="grad", fp64=fp64)
+    ns = wl.n_samples
+    check_flux_chi2(wl, got, ref, fp64)
+    tol_f = sbgpu.flux_tolerance(wl, ref["flux"], ns, fp64)
+    tol_d = sbgpu.grad_tolerance(wl, ref, wl.theta, ns, fp64)
+    err = np.abs(got["dflux"] - ref["dflux"])
+    assert np.all(err <= tol_d), f"dflux worst ratio per component {np.max(err / np.maximum(tol_d, 1e-300), axis=0)}"
+    tol_g = sbgpu.dchi2_tolerance(wl, ref, tol_f, tol_d, ns, fp64)
+    errg = np.abs(got["dchi2"] - ref["dchi2"])
+    assert np.all(errg <= tol_g), f"dchi2 worst ratio {np.max(errg / np.maximum(tol_g, 1e-300), axis=0)}"
+    # the grad kernel's forward equals the forward kernel's within tolerance
+    fwd = sbgpu.run_gpu(wl, mode="chi2", fp64=fp64)
+    assert np.all(np.abs(fwd["flux"] - got["flux"]) <= 2 * tol_f)
+
+
+def test_config4_gpu_gradient_vs_oracle_central_differences(cuda_device):
+    """BASELINE.json configs[3]: analytic gradient against ORACLE central differences, step 1e-6 rel."""
+    wl = prepare(4, n_sn=24)
+    ns = wl.n_samples
+    base = oracle.run_workload(wl, want_flux=True, want_dflux=True)
+    for fp64 in (False, True):
+        got = sbgpu.run_gpu(wl, mode="grad", fp64=fp64, with_data=False)
+        tol_d = sbgpu.grad_tolerance(wl, base, wl.theta, ns, fp64)
+        peak = sbgpu.unit_peaks(wl, base["flux"], ns)
+        for q, key in enumerate(("x0", "x1", "c", "t0")):
+            th = wl.theta[key].astype(np.float64)
+            h = 1e-6 * (np.abs(th) if key == "x0" else np.maximum(np.abs(th), 1.0))
+            up = {k: v.astype(np.float64).copy() for k, v in wl.theta.items()}
+            dn = {k: v.astype(np.float64).copy() for k, v in wl.theta.items()}
+            up[key] = th + h
+            dn[key] = th - h
+            fu = oracle.run_workload(wl, theta=up)["flux"]
+            fd = oracle.run_workload(wl, theta=dn)["flux"]
+            hh = np.repeat(h, np.diff(wl.obs_offset))
+            fdiff = (fu - fd) / (2.0 * hh)
+            scale = np.repeat(np.maximum(np.abs(th), 1.0) if key != "x0" else np.abs(th), np.diff(wl.obs_offset))
+            tol = tol_d[:, q] + 1e-6 * np.maximum(np.abs(base["dflux"][:, q]), peak / scale)
+            err = np.abs(got["dflux"][:, q] - fdiff)
+            assert np.all(err <= tol), (key, fp64, float(np.max(err / tol)))
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_config5_nir_grid(cuda_device, fp64):
+    wl = prepare(5, n_sn=300)  # 24000 evals on the 71 x 1801 grid, 10 bands up to 961 samples
+    ref = oracle_all(wl)
+    got = sbgpu.run_gpu(wl, mode="chi2", fp64=fp64)
+    check_flux_chi2(wl, got, ref, fp64)
+
+
+def test_chi2_is_deterministic(cuda_device):
+    wl = prepare(2, n_sn=200)
+    a = sbgpu.run_gpu(wl, mode="chi2")
+    b = sbgpu.run_gpu(wl, mode="chi2")
+    assert np.array_equal(a["chi2"], b["chi2"]) and np.array_equal(a["flux"], b["flux"])
+
+
+def test_no_zero_point_is_raw_photon_flux(cuda_device):
+    wl = prepare(1)
+    got = sbgpu.run_gpu(wl, mode="flux", use_zp=False)
+    m, b = oracle.Model.from_dict(wl.model), oracle.Bands.from_dict(wl.bands)
+    th = wl.theta
+    want = np.array([oracle.eval_one(m, b, float(wl.z[0]), float(wl.time[i]), int(wl.band[i]), None,
+                                     float(th["x0"][0]), float(th["x1"][0]), float(th["c"][0]), float(th["t0"][0]))
+                     for i in range(wl.n_obs_total)])
+    assert np.all(np.abs(got["flux"] - want) <= 1e-5 * np.abs(want) + 1e-9 * np.max(np.abs(want)))
