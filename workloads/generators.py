@@ -214,20 +214,21 @@ _FULL = {  # n_sn, n_samples, n_obs per SN
 
 
 def make_workload(config: int, n_sn: Optional[int] = None, n_samples: Optional[int] = None,
-                  ragged: bool = False) -> Workload:
+                  ragged: bool = False, seed_offset: int = 0) -> Workload:
     """Build config `config` (1..5).  `n_sn` / `n_samples` shrink it for parity tests.
 
     The shrunk workload is a prefix of the same random streams only in distribution, not
     element-wise; parity tests always hand identical arrays to both sides, so that is fine.
     `ragged=True` draws a different observation count per supernova (between half and the
     full count) to exercise the CSR layout; BASELINE.json's configs are all regular.
+    `seed_offset` shifts the config's seed (one shard per rank in multi-GPU weak scaling).
     """
     if config not in CONFIG_IDS:
         raise ValueError(f"unknown config {config}")
     full_sn, full_samples, n_obs = _FULL[config]
     n_sn = full_sn if n_sn is None else int(n_sn)
     n_samples = full_samples if n_samples is None else int(n_samples)
-    rng = np.random.default_rng(SEED_CONFIG[config])
+    rng = np.random.default_rng(SEED_CONFIG[config] + int(seed_offset))
 
     model = make_model(nir=(config == 5))
     model.update(make_colour_law())
@@ -307,7 +308,7 @@ def make_workload(config: int, n_sn: Optional[int] = None, n_samples: Optional[i
         theta_true={k: _f32(v) for k, v in tt.items()},
         theta={k: _f32(v) for k, v in th.items()},
         noise=noise,
-        meta={"n_obs_per_sn": n_obs, "ragged": ragged, "seed": SEED_CONFIG[config]},
+        meta={"n_obs_per_sn": n_obs, "ragged": ragged, "seed": SEED_CONFIG[config] + int(seed_offset)},
     )
 
 
