@@ -111,7 +111,7 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
     const size_t n = (size_t)n_phase * (size_t)n_wave;
     for (size_t i = 0; i < n; ++i)
         if (!std::isfinite(m0[i]) || !std::isfinite(m1[i])) return SB_EINVAL;
-    if ((long long)n_phase * ((long long)n_wave + 4) >= (1LL << 30)) return SB_ELIMIT;
+    if ((long long)n_phase * ((long long)n_wave + 20) >= (1LL << 30)) return SB_ELIMIT;
 
     sb_model *h = new (std::nothrow) sb_model();
     if (!h) return SB_ENOMEM;
@@ -119,7 +119,7 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
     SbModelParams &p = h->prm;
     p.n_phase = n_phase;
     p.n_wave = n_wave;
-    p.ld = (n_wave + 3) & ~3;
+    p.ld = (n_wave + 16 + 3) & ~3; // SB_PAD_L zero columns left, >= 8 right (sb_internal.h)
     p.n_cl = n_cl;
     p.p0 = phase[0];
     p.dp = (phase[n_phase - 1] - phase[0]) / (double)(n_phase - 1);
@@ -140,8 +140,8 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
     std::vector<double> t0((size_t)n_phase * p.ld, 0.0), t1((size_t)n_phase * p.ld, 0.0);
     for (int k = 0; k < n_phase; ++k)
         for (int l = 0; l < n_wave; ++l) {
-            t0[(size_t)k * p.ld + l] = m0[(size_t)k * n_wave + l];
-            t1[(size_t)k * p.ld + l] = m1[(size_t)k * n_wave + l];
+            t0[(size_t)k * p.ld + SB_PAD_L + l] = m0[(size_t)k * n_wave + l];
+            t1[(size_t)k * p.ld + SB_PAD_L + l] = m1[(size_t)k * n_wave + l];
         }
     std::vector<float> f0(t0.begin(), t0.end()), f1(t1.begin(), t1.end());
     cudaGetDevice(&h->device);
@@ -210,11 +210,15 @@ int sb_load_bandpasses(int32_t n_bands, const int64_t *offset, const double *wav
         h->h_zpab[b] = zp;
         zpab_inv[b] = 1.0 / zp;
     }
-    std::vector<float> dlam_f(dlam.begin(), dlam.end()), w_f(w.begin(), w.end());
+    std::vector<float2> tab_f((size_t)total);
+    std::vector<double2> tab_d((size_t)total);
+    for (int64_t i = 0; i < total; ++i) {
+        tab_d[i] = make_double2(dlam[i], w[i]);
+        tab_f[i] = make_float2((float)dlam[i], (float)w[i]);
+    }
     cudaGetDevice(&h->device);
     if (!upload(&h->d_off, off) || !upload(&h->d_lam_first, lam_first) || !upload(&h->d_zpab_inv, zpab_inv) ||
-        !upload(&h->d_dlam_f64, dlam) || !upload(&h->d_w_f64, w) || !upload(&h->d_dlam_f32, dlam_f) ||
-        !upload(&h->d_w_f32, w_f)) {
+        !upload(&h->d_tab_f64, tab_d) || !upload(&h->d_tab_f32, tab_f)) {
         sb_free_bands(h);
         return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
     }
@@ -228,10 +232,8 @@ void sb_free_bands(sb_bands *b)
     cudaFree(b->d_off);
     cudaFree(b->d_lam_first);
     cudaFree(b->d_zpab_inv);
-    cudaFree(b->d_dlam_f32);
-    cudaFree(b->d_w_f32);
-    cudaFree(b->d_dlam_f64);
-    cudaFree(b->d_w_f64);
+    cudaFree(b->d_tab_f32);
+    cudaFree(b->d_tab_f64);
     free(b->h_zpab);
     delete b;
 }
@@ -262,31 +264,40 @@ int launch_inst(const SbKParams &kp, size_t smem, int grid, cudaStream_t st)
 }
 
 template <typename T, bool GRAD, int NWARPS>
-int launch_typed(SbKParams &kp, const sb_bands *b, cudaStream_t st)
+int launch_typed(SbKParams &kp, const sb_bands *b, int n_obs_total, cudaStream_t st)
 {
     const int smem_max = device_smem_optin();
     const int n_sm = device_sm_count();
     if (smem_max <= 0 || n_sm <= 0) return SB_ECUDA;
     constexpr int NSET = GRAD ? 3 : 1;
     const size_t cell_bytes = sizeof(T) * 4 * NSET;
-    const size_t red_bytes = sizeof(double) * 5 * NWARPS;
-    const size_t band_bytes = 2 * sizeof(T) * (size_t)((b->n_total + 3) & ~3);
+    // evaluation records per chunk and units per group: about `cap` evaluations per CTA pass
+    const int cap = GRAD ? 256 : 512;
+    const double mean_obs = kp.n_sn > 0 ? (double)n_obs_total / (double)kp.n_sn : 1.0;
+    int group = (int)((double)cap / (mean_obs > 1.0 ? mean_obs : 1.0));
+    if (group < 1) group = 1;
+    if (group > sb::kMaxGroup) group = sb::kMaxGroup;
+    kp.chunk_cap = cap;
+    kp.group_units = group;
     // entries needed by the widest band at z >= 0 (narrower tiles still work: the kernel loops)
-    int tc_full = (int)std::ceil(b->max_span / kp.mp.dl) + 6;
-    tc_full = (tc_full + 1) & ~1;
-    if (tc_full > kp.mp.n_wave + 4) tc_full = (kp.mp.n_wave + 5) & ~1;
-    if (tc_full < 16) tc_full = 16;
-    // stage the band tables in shared memory when they fit beside >= 64-entry row buffers (fp32 only)
-    bool stage = sizeof(T) == 4 && band_bytes + red_bytes + (size_t)NWARPS * 64 * cell_bytes <= (size_t)smem_max;
-    size_t avail = (size_t)smem_max - red_bytes - (stage ? band_bytes : 0);
+    int tc_full = (int)std::ceil(b->max_span / kp.mp.dl) + 12;
+    if (tc_full > kp.mp.n_wave + 12) tc_full = kp.mp.n_wave + 12;
+    tc_full = (tc_full + 7) & ~7;
+    if (tc_full < 32) tc_full = 32;
+    // stage the band tables in shared memory when they fit beside >= 128-entry row buffers (fp32 only)
+    const sb::SmemLayout<T, GRAD> fixed(NWARPS, 0, cap, b->n_total, false);
+    const size_t band_bytes = sb::SmemLayout<T, GRAD>(NWARPS, 0, cap, b->n_total, true).total - fixed.total;
+    const bool stage = sizeof(T) == 4 && fixed.total + band_bytes + (size_t)NWARPS * 128 * cell_bytes <= (size_t)smem_max;
+    const size_t avail = (size_t)smem_max - fixed.total - (stage ? band_bytes : 0);
     int tc = (int)(avail / ((size_t)NWARPS * cell_bytes));
-    tc &= ~1;
+    tc &= ~7;
     if (tc > tc_full) tc = tc_full;
-    if (tc < 16) return SB_ELIMIT;
+    if (tc < 32) return SB_ELIMIT;
     kp.tile_cells = tc;
-    const size_t smem = (size_t)NWARPS * tc * cell_bytes + red_bytes + (stage ? band_bytes : 0);
+    const size_t smem = sb::SmemLayout<T, GRAD>(NWARPS, tc, cap, b->n_total, stage).total;
     const long long n_units = (long long)kp.n_sn * kp.n_samples;
-    int grid = (int)(n_units < (long long)n_sm ? n_units : (long long)n_sm);
+    const long long n_groups = (n_units + group - 1) / group;
+    int grid = (int)(n_groups < (long long)n_sm ? n_groups : (long long)n_sm);
     if (grid < 1) return SB_OK;
     const bool small_cl = kp.mp.n_cl <= 5;
     if (stage) {
@@ -322,8 +333,7 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *fl
     kp.band_off = b->d_off;
     kp.band_lam_first = b->d_lam_first;
     kp.band_zpab_inv = b->d_zpab_inv;
-    kp.band_dlam = f32 ? (const void *)b->d_dlam_f32 : (const void *)b->d_dlam_f64;
-    kp.band_w = f32 ? (const void *)b->d_w_f32 : (const void *)b->d_w_f64;
+    kp.band_tab = f32 ? (const void *)b->d_tab_f32 : (const void *)b->d_tab_f64;
     kp.n_sn = bt->n_sn;
     kp.n_samples = bt->n_samples;
     kp.obs_offset = bt->obs_offset;
@@ -343,11 +353,11 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *fl
     kp.out_dchi2 = out_dchi2;
     cudaStream_t st = (cudaStream_t)stream;
     if (f32) {
-        if (grad) return launch_typed<float, true, 8>(kp, b, st);
-        return launch_typed<float, false, 16>(kp, b, st);
+        if (grad) return launch_typed<float, true, 8>(kp, b, bt->n_obs_total, st);
+        return launch_typed<float, false, 16>(kp, b, bt->n_obs_total, st);
     }
-    if (grad) return launch_typed<double, true, 8>(kp, b, st);
-    return launch_typed<double, false, 8>(kp, b, st);
+    if (grad) return launch_typed<double, true, 8>(kp, b, bt->n_obs_total, st);
+    return launch_typed<double, false, 8>(kp, b, bt->n_obs_total, st);
 }
 
 } // namespace

@@ -7,6 +7,10 @@
 #include "saltband.h"
 
 #define SB_MAX_CL 8
+// Device model tables: node l of a phase row lives at column l + SB_PAD_L; the row is zero padded
+// on both sides (>= 8 columns on the right) so that the kernel's aligned 4-node loads of a window
+// that touches the grid edge stay inside the row.  ld = round_up(n_wave + 16, 4).
+#define SB_PAD_L 8
 
 // Physical constants (CGS, Angstrom) -- PAPER.md:41 "h and c are the Planck constant and the speed
 // of light"; AB reference flux density for the zero point (G7).
@@ -27,7 +31,7 @@ struct SbModelParams {
 
 struct sb_model {
     SbModelParams prm;
-    float *m0_f32, *m1_f32;   // [n_phase][ld]
+    float *m0_f32, *m1_f32;   // [n_phase][ld], zero padded (SB_PAD_L)
     double *m0_f64, *m1_f64;  // [n_phase][ld]
     int device;
 };
@@ -37,8 +41,8 @@ struct sb_bands {
     int32_t *d_off;        // [n_bands+1]
     double *d_lam_first;   // [n_bands] first wavelength of each band grid
     double *d_zpab_inv;    // [n_bands] 1 / ZPAB_b
-    float *d_dlam_f32, *d_w_f32;   // [n_total] lam_j - lam_first ; folded weight w_j T_j lam_j/(hc)
-    double *d_dlam_f64, *d_w_f64;
+    float2 *d_tab_f32;     // [n_total] {lam_j - lam_first, folded weight w_j T_j lam_j/(hc)}
+    double2 *d_tab_f64;
     double *h_zpab;        // host copy [n_bands]
     double max_span;       // max over bands of (lam_last - lam_first)
     int device;
@@ -51,12 +55,14 @@ struct SbKParams {
     int32_t n_bands, n_band_total;
     const int32_t *band_off;
     const double *band_lam_first, *band_zpab_inv;
-    const void *band_dlam, *band_w;   // real type
+    const void *band_tab;             // interleaved {dlam_j, W_j} pairs of the kernel's real type
     int32_t n_sn, n_samples;
     const int32_t *obs_offset;
     const void *time, *zp, *z, *x0, *x1, *c, *t0;
     const int32_t *band;
     const void *flux, *fluxerr;       // may be NULL
     void *out_flux, *out_dflux, *out_chi2, *out_dchi2; // may be NULL
-    int32_t tile_cells;               // coefficient-row entries per warp buffer
+    int32_t tile_cells;               // coefficient-row entries per warp buffer (multiple of 8)
+    int32_t chunk_cap;                // evaluation records per chunk
+    int32_t group_units;              // units per CTA group (<= 16)
 };

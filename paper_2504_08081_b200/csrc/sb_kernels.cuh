@@ -1,24 +1,30 @@
 // sb_kernels.cuh -- the fused SALT3 band-flux kernel (sm_100a).
 //
-// One CTA per unit (supernova s, parameter sample k), persistent over units; one warp per
-// evaluation (observation i of that unit); lanes stride the band's wavelength samples.
+// Persistent CTAs; a CTA takes groups of G consecutive units (unit = supernova s x parameter
+// sample k) and works through the group's evaluations (one per observation of each unit) in chunks
+// of at most CAP:
+//   prologue  one THREAD per evaluation: everything that is scalar per evaluation (fp64): phase,
+//             phase weights, in-range band samples, cell window, zero point -> a record in smem.
+//   main      one WARP per evaluation (dynamic, smem counter); lanes stride the band's samples.
+//   epilogue  one thread per evaluation: coalesced result stores, chi^2 terms; then one warp per
+//             unit reduces them in a fixed order (deterministic).
 // Steps (citations in include/saltband.h):
-//   a1  p = (t - t0)/(1+z) per evaluation (fp64 scalar prologue); per sample the fractional cell
-//       coordinate u_j = (lam_j/(1+z) - L0)/dL, computed RELATIVE to the evaluation's first cell as
-//       one FFMA  t_j = dlam_j * a + b  (dlam_j = lam_j - lam_first is exact in fp32).
+//   a1  p = (t - t0)/(1+z) per evaluation; per sample the fractional cell coordinate relative to
+//       the evaluation's first cell as ONE FFMA  t_j = dlam_j * a + b  (dlam_j = lam_j - lam_first
+//       is exact in fp32).
 //   a2  bicubic interpolation, separable: the <= 4 phase rows of M0 and M1 are collapsed once per
-//       evaluation into a 1-D row R[l] = sum_k wp_k (M0 + x1 M1)[kp+k][l]; each cell of that row
-//       is then converted to the cubic's coefficients about the cell centre (an exact
-//       re-association of the Keys a=-1/2 / Catmull-Rom weights; linear in border cells), stored
-//       as one float4 per cell in this warp's shared-memory row buffer.  A sample is 1 LDS.128 +
-//       3 FFMA.
+//       evaluation into a 1-D row R[l] = sum_k wp_k (M0 + x1 M1)[kp+k][l] (float4 loads: 4 nodes
+//       per lane, 120 cells per warp pass, 3 shuffles for the halo); each cell of that row is
+//       converted to the cubic's coefficients about the cell centre (an exact re-association of
+//       the Keys a=-1/2 / Catmull-Rom weights; linear in border cells) and stored as one float4
+//       per cell in this warp's shared-memory row buffer (XOR-swizzled: conflict-free stores).
+//       A sample is then 1 LDS.128 + 3 FFMA.
 //   a3  colour law: degree-(NCL-1) Horner in the reduced wavelength, linear continuation by
-//       clamping, one ex2 per sample (coefficients pre-scaled by c*log2(e) in fp32 mode).
-//   a4/a5  folded weight W_j = w_j T_j lam_j/(hc) (trapezoid weight folded at load), FFMA
-//       accumulate per lane, warp-shuffle butterfly.
-//   a6  zero point S = 10^(0.4 zp)/ZPAB_b in fp64 per evaluation.
-//   a7  chi^2 per unit: per-warp partial sums in observation order, fixed-order CTA sum (fp64
-//       accumulators; deterministic).
+//       clamping, one ex2 per sample (coefficients pre-scaled by c*log2(e) in fp32 forward mode).
+//   a4/a5  folded weight W_j = w_j T_j lam_j/(hc) (trapezoid weight folded at load), interleaved
+//       with dlam_j (one LDS.64), FFMA accumulate per lane, warp-shuffle butterfly.
+//   a6  zero point S = 10^(0.4 zp)/ZPAB_b in fp64 per evaluation (prologue).
+//   a7  chi^2 per unit in fp64, fixed summation order.
 //   a8  analytic gradient: three coefficient sets (value row, M1-only row, d/dphase row) and four
 //       accumulators give d m/d(x0, x1, c, t0).
 #pragma once
@@ -27,15 +33,27 @@
 namespace sb {
 
 constexpr int kWarpSize = 32;
-constexpr int kCellsPerPass = 29; // a 32-node pass yields 29 cells (3-node halo via shuffles)
+constexpr int kCellsPerPass = 120; // lanes 1..30 produce 4 cells each; lanes 0 and 31 carry the halo
+constexpr int kMaxGroup = 16;      // units per CTA group
 
 template <typename T> struct Vec4;
 template <> struct Vec4<float> { using type = float4; };
 template <> struct Vec4<double> { using type = double4; };
+template <typename T> struct Vec2;
+template <> struct Vec2<float> { using type = float2; };
+template <> struct Vec2<double> { using type = double2; };
 
 template <typename T> __device__ __forceinline__ typename Vec4<T>::type make_v4(T a, T b, T c, T d);
 template <> __device__ __forceinline__ float4 make_v4<float>(float a, float b, float c, float d) { return make_float4(a, b, c, d); }
 template <> __device__ __forceinline__ double4 make_v4<double>(double a, double b, double c, double d) { return make_double4(a, b, c, d); }
+
+__device__ __forceinline__ float4 ldg_v4(const float *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
+__device__ __forceinline__ double4 ldg_v4(const double *p)
+{
+    const double2 a = __ldg(reinterpret_cast<const double2 *>(p));
+    const double2 b = __ldg(reinterpret_cast<const double2 *>(p) + 1);
+    return make_double4(a.x, a.y, b.x, b.y);
+}
 
 // Split t into the nearest integer and the signed remainder s = t - rint(t), |s| <= 1/2.
 // fp32: magic-number rounding on the FMA pipe (no F2I/FRND on the quarter-rate XU pipe).
@@ -74,19 +92,30 @@ template <typename T> __device__ __forceinline__ T warp_sum(T v)
     return v;
 }
 
-// Number of j in [0, n) with f(j) < thr for a non-decreasing f; warp-cooperative 32-ary search.
+// Number of j in [0, n) with f(j) < thr (or <= thr) for a non-decreasing f; one thread.
+template <typename F>
+__device__ __forceinline__ int count_less(int n, double thr, F f, bool or_equal)
+{
+    int lo = 0, hi = n;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        const double v = f(mid);
+        const bool less = or_equal ? (v <= thr) : (v < thr);
+        if (less) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+// Same count, warp-cooperative 32-ary search (used only when a band needs several tiles).
 template <typename F, typename T>
-__device__ __forceinline__ int warp_count_less(int n, T thr, int lane, F f, bool or_equal)
+__device__ __forceinline__ int warp_count_less(int n, T thr, int lane, F f)
 {
     int lo = 0, len = n;
     while (len > 0) {
         int step = (len + kWarpSize - 1) / kWarpSize;
         int j = lo + lane * step; // probe the first element of each of 32 sub-ranges
         bool less = false;
-        if (j < lo + len) {
-            T v = f(j);
-            less = or_equal ? (v <= thr) : (v < thr);
-        }
+        if (j < lo + len) less = f(j) < thr;
         unsigned m = __ballot_sync(0xffffffffu, less);
         int cnt = __popc(m); // probes 0..cnt-1 are "less": the boundary is inside sub-range cnt-1
         if (cnt == 0) return lo;
@@ -98,10 +127,18 @@ __device__ __forceinline__ int warp_count_less(int n, T thr, int lane, F f, bool
     return lo;
 }
 
-// Coefficients of one cell's polynomial about the cell centre, s in [-1/2, 1/2].
-//   g = global cell index, nodes rm = R[g-1], r0 = R[g], r1 = R[g+1], r2 = R[g+2] (clamped loads).
-//   Interior (1 <= g <= n-3): Catmull-Rom.  g = 0 or n-2: linear (G2).  g = -1 and
-//   g = n-1 continue the adjacent border line (reached only within rounding of the grid edge).
+// Interior cell: Catmull-Rom cubic through (rm, r0, r1, r2) about the cell centre, s in [-1/2, 1/2].
+template <typename T>
+__device__ __forceinline__ typename Vec4<T>::type cell_coef_interior(T rm, T r0, T r1, T r2)
+{
+    const T s1 = r0 + r1, s2 = rm + r2, d1 = r1 - r0, d2 = r2 - rm;
+    return make_v4<T>(fma_t(s1, (T)0.5625, s2 * (T)-0.0625), fma_t(d1, (T)1.375, d2 * (T)-0.125),
+                      (s2 - s1) * (T)0.25, fma_t(d1, (T)-1.5, d2 * (T)0.5));
+}
+
+// General cell g of an n-node row (nodes outside the row are zero padding and never used):
+//   1 <= g <= n-3 Catmull-Rom; g = 0 or n-2 linear (G2); g = -1 and g = n-1 continue the
+//   adjacent border line (reached only within rounding of the grid edge); anything else is zero.
 template <typename T>
 __device__ __forceinline__ typename Vec4<T>::type cell_coef(int g, int n, T rm, T r0, T r1, T r2)
 {
@@ -110,9 +147,7 @@ __device__ __forceinline__ typename Vec4<T>::type cell_coef(int g, int n, T rm, 
     if (g == -1) { T d = r2 - r1; return make_v4<T>(r1 - h * d, d, 0, 0); }
     if (g == n - 1) { T d = r0 - rm; return make_v4<T>(r0 + h * d, d, 0, 0); }
     if (g == 0 || g == n - 2) return make_v4<T>(h * (r0 + r1), r1 - r0, 0, 0);
-    T s1 = r0 + r1, s2 = rm + r2, d1 = r1 - r0, d2 = r2 - rm;
-    return make_v4<T>(((T)9 * s1 - s2) * (T)0.0625, ((T)11 * d1 - d2) * (T)0.125, (s2 - s1) * (T)0.25,
-                      (d2 - (T)3 * d1) * h);
+    return cell_coef_interior<T>(rm, r0, r1, r2);
 }
 
 template <typename T>
@@ -120,6 +155,10 @@ __device__ __forceinline__ T poly3(const typename Vec4<T>::type &a, T s)
 {
     return fma_t(fma_t(fma_t(a.w, s, a.z), s, a.y), s, a.x);
 }
+
+// Row-buffer slot of entry q: XOR swizzle inside groups of 8 slots so that the four 128-bit stores
+// of a collapse pass (lane l writes entries 4l..4l+3) are bank-conflict free.
+__device__ __forceinline__ int swz(int q) { return q ^ ((q >> 3) & 3); }
 
 // Cubic-convolution weights (Keys a = -1/2) and their derivatives, or the linear border pair.
 __device__ __forceinline__ void phase_weights(double tau, bool border, double inv_dp, double w[4], double d[4])
@@ -140,12 +179,40 @@ __device__ __forceinline__ void phase_weights(double tau, bool border, double in
     d[3] = 0.5 * (3.0 * t2 - 2.0 * tau) * inv_dp;
 }
 
+// ---- shared-memory records -----------------------------------------------------------------
+// Per unit (supernova x sample) of the current group.
+template <typename T> struct UnitRec {
+    T cl[SB_MAX_CL];      // colour-law coefficients (fp32 forward mode: times c*log2e)
+    T s_lo, s_hi;         // continuation slopes (same scaling)
+    T al;                 // reduced wavelength per observer-frame Angstrom: r_j = dlam_j*al + be
+    T c_exp;              // gradient mode: exponent argument = CL * c_exp
+    T x1, a_t;            // a_t: model cells per observer-frame Angstrom
+    double x0, opz, t0, cc;
+    long long out_base;   // first element of this unit in out_flux
+    int32_t sn, o_lo, n_obs, e_begin;
+};
+
+// Per evaluation of the current chunk; written by one thread, read by one warp.
+template <typename T> struct EvalRecBase {
+    int32_t j_lo, j_hi;   // in-range samples [j_lo, j_hi) (absolute index into the band tables)
+    int32_t col0;         // first table column loaded by lane 0 of pass 0 (multiple of 4)
+    int32_t n_entries;    // coefficient entries (cells) needed; 0 = nothing to integrate
+    int32_t rowoff[4];    // element offset of the four phase rows
+    T w0[4], w1[4];       // phase weights on M0 and on M1 (forward mode: w1 already times x1)
+    T b_t, be;            // t_j = dlam_j*a_t + b_t ; r_j = dlam_j*al + be
+    int32_t unit, obs;    // group-local unit, global observation index
+    double scale;         // zero-point factor S
+};
+template <typename T, bool GRAD> struct EvalRec : EvalRecBase<T> {};
+template <typename T> struct EvalRec<T, true> : EvalRecBase<T> {
+    T d0[4], d1[4];       // d/dp weights on M0 and on M1 (d1 already times x1)
+};
+
 template <typename T, int NCL> struct Colour {
-    T a[NCL];        // polynomial coefficients (fp32 fwd mode: times c*log2e)
+    T a[NCL];        // polynomial coefficients
     T r_lo, r_hi;    // clamp range of the reduced wavelength
     T s_lo, s_hi;    // continuation slopes (same scaling as a[])
     T al, be;        // r_j = dlam_j * al + be
-    // returns CL(r) in the scaling of a[]
     __device__ __forceinline__ T eval(T dl) const
     {
         T r = fma_t(dl, al, be);
@@ -159,269 +226,423 @@ template <typename T, int NCL> struct Colour {
     }
 };
 
+template <typename T, bool GRAD> struct SmemLayout {
+    // byte offsets of the carve-up; every block is 16-byte aligned
+    size_t rowbuf, recs, res, units, uacc, misc, bands, total;
+    __host__ __device__ SmemLayout(int nwarps, int tile_cells, int cap, int n_band_total, bool stage)
+    {
+        constexpr int NSET = GRAD ? 3 : 1;
+        constexpr int NRES = GRAD ? 5 : 1;
+        size_t o = 0;
+        rowbuf = o; o += (size_t)nwarps * tile_cells * NSET * sizeof(typename Vec4<T>::type);
+        recs = o; o += (size_t)cap * sizeof(EvalRec<T, GRAD>);
+        res = o; o += (size_t)cap * NRES * sizeof(double);
+        units = o; o += (size_t)kMaxGroup * sizeof(UnitRec<T>);
+        uacc = o; o += (size_t)kMaxGroup * 5 * sizeof(double);
+        misc = o; o += 16;
+        bands = o; o += stage ? (size_t)((n_band_total + 1) & ~1) * sizeof(typename Vec2<T>::type) : 0;
+        total = o;
+    }
+};
+
+// ---- prologue: one thread per evaluation ----------------------------------------------------
+// Fills the evaluation's record, or (nothing to integrate / bad band index) its result directly.
+template <typename T, bool GRAD>
+__device__ __forceinline__ void eval_prologue(const SbKParams &P, const UnitRec<T> *units, int nu, int e,
+                                              EvalRec<T, GRAD> &R, double *res,
+                                              const typename Vec2<T>::type *tab)
+{
+    constexpr int NRES = GRAD ? 5 : 1;
+    const SbModelParams &mp = P.mp;
+    int gu = 0;
+    while (gu + 1 < nu && e >= units[gu + 1].e_begin) ++gu;
+    const UnitRec<T> &U = units[gu];
+    const int o = U.o_lo + (e - U.e_begin);
+    R.unit = gu;
+    R.obs = o;
+    R.n_entries = 0;
+#pragma unroll
+    for (int k = 0; k < NRES; ++k) res[k] = 0.0;
+    const int b = __ldg(P.band + o);
+    if ((unsigned)b >= (unsigned)P.n_bands) {
+#pragma unroll
+        for (int k = 0; k < NRES; ++k) res[k] = __longlong_as_double(0x7ff8000000000000LL);
+        return;
+    }
+    const int nP = mp.n_phase, nW = mp.n_wave;
+    const double inv_dp = 1.0 / mp.dp, inv_dl = 1.0 / mp.dl;
+    const int boff = __ldg(P.band_off + b);
+    const int nb = __ldg(P.band_off + b + 1) - boff;
+    const double lam_first = __ldg(P.band_lam_first + b);
+    const double opz = U.opz, inv_opz = 1.0 / opz;
+    // ---- a1: phase
+    const double p = ((double)static_cast<const T *>(P.time)[o] - U.t0) / opz;
+    const double up = (p - mp.p0) * inv_dp;
+    if (!((up >= 0.0) && (up <= (double)(nP - 1)))) return;
+    // in-range band samples [j_lo, j_hi): 0 <= u_j <= nW-1; membership is decided in fp64
+    // (dlam_j is exact for fp32-representable grids)
+    const double dl_lo = mp.l0 * opz - lam_first;
+    const double dl_hi = (mp.l0 + (double)(nW - 1) * mp.dl) * opz - lam_first;
+    auto probe = [&](int j) { return (double)tab[boff + j].x; };
+    const int j_lo = count_less(nb, dl_lo, probe, false);
+    const int j_hi = count_less(nb, dl_hi, probe, true);
+    if (j_lo >= j_hi) return;
+    // ---- a2: phase weights
+    const int kp = min((int)floor(up), nP - 2);
+    const double tau = up - (double)kp;
+    const bool pborder = (kp == 0) || (kp == nP - 2);
+    double wv[4], wd[4];
+    phase_weights(tau, pborder, inv_dp, wv, wd);
+    const double x1 = (double)U.x1;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        R.rowoff[k] = min(max(kp - 1 + k, 0), nP - 1) * mp.ld;
+        R.w0[k] = (T)wv[k];
+        R.w1[k] = GRAD ? (T)wv[k] : (T)(wv[k] * x1);
+        if constexpr (GRAD) {
+            R.d0[k] = (T)wd[k];
+            R.d1[k] = (T)(wd[k] * x1);
+        }
+    }
+    // ---- a1: wavelength geometry relative to the first cell of the window
+    const double a_d = inv_opz * inv_dl;                          // cells per observer-frame Angstrom
+    const double ub = (lam_first * inv_opz - mp.l0) * inv_dl;     // u of dlam = 0
+    const double u_first = (double)tab[boff + j_lo].x * a_d + ub;
+    const double u_last = (double)tab[boff + j_hi - 1].x * a_d + ub;
+    const int i_first = min(max((int)floor(u_first), 0), nW - 2);
+    const int i_last = min(max((int)floor(u_last), 0), nW - 2);
+    // window of cells i_first-1 .. i_last+1 (one spare cell each side for fp32 rounding of t_j);
+    // entry q <-> cell g0 + q, g0 aligned so that table columns are loaded as aligned float4
+    const int col0 = ((i_first - 1 + SB_PAD_L) & ~3) - 4;
+    const int g0 = col0 + 4 - SB_PAD_L;
+    R.col0 = col0;
+    R.n_entries = i_last + 1 - g0 + 1;
+    R.j_lo = boff + j_lo;
+    R.j_hi = boff + j_hi;
+    R.b_t = (T)(ub - (double)g0 - 0.5); // t_j = u_j - g0 - 1/2, rint(t_j) = entry, remainder in [-1/2, 1/2]
+    R.be = (T)((lam_first * inv_opz - mp.cl_b) * mp.cl_inv_span);
+    double S = 1.0;
+    if (P.zp != nullptr) S = exp10(0.4 * (double)static_cast<const T *>(P.zp)[o]) * __ldg(P.band_zpab_inv + b);
+    R.scale = S;
+}
+
+// ---- main: one warp integrates one evaluation -------------------------------------------------
+template <typename T, bool GRAD, int NCL>
+__device__ __forceinline__ void eval_warp(const SbKParams &P, const UnitRec<T> &U, const EvalRec<T, GRAD> &R,
+                                          typename Vec4<T>::type *rowbuf, int TC,
+                                          const typename Vec2<T>::type *__restrict__ tab, int lane, double *res)
+{
+    using V4 = typename Vec4<T>::type;
+    using V2 = typename Vec2<T>::type;
+    constexpr int NSET = GRAD ? 3 : 1;
+    const SbModelParams &mp = P.mp;
+    const int nW = mp.n_wave;
+    const T *__restrict__ M0 = static_cast<const T *>(P.m0);
+    const T *__restrict__ M1 = static_cast<const T *>(P.m1);
+
+    const int n_entries = R.n_entries, col0 = R.col0, j_hi = R.j_hi;
+    const int g0 = col0 + 4 - SB_PAD_L;
+    const int col_max = col0 + 4 + n_entries + 1; // last node column any needed cell touches
+    T w0[4], w1[4], d0[4], d1[4];
+    const T *p0[4], *p1[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        w0[k] = R.w0[k];
+        w1[k] = R.w1[k];
+        if constexpr (GRAD) { d0[k] = R.d0[k]; d1[k] = R.d1[k]; }
+        p0[k] = M0 + R.rowoff[k];
+        p1[k] = M1 + R.rowoff[k];
+    }
+    const T x1_t = U.x1;
+    const T a_t = U.a_t, b_t = R.b_t;
+    Colour<T, NCL> col;
+#pragma unroll
+    for (int q = 0; q < NCL; ++q) col.a[q] = U.cl[q];
+    col.r_lo = (T)mp.r_lo;
+    col.r_hi = (T)mp.r_hi;
+    col.s_lo = U.s_lo;
+    col.s_hi = U.s_hi;
+    col.al = U.al;
+    col.be = R.be;
+    const T c_exp = U.c_exp;
+
+    T accF = 0, accB = 0, accC = 0, accD = 0;
+    int ja = R.j_lo;
+    for (int q0 = 0;; q0 += TC - 8) {
+        const int q_end = min(q0 + TC, n_entries);
+        // ---- a2: collapse the phase rows (4 nodes per lane), convert to per-cell cubic coefficients
+        for (int qp = q0; qp < q_end; qp += kCellsPerPass) {
+            const int c = col0 + qp + 4 * lane; // this lane's nodes: columns c..c+3 = cells' left nodes
+            T r[4] = {0, 0, 0, 0}, r1[4] = {0, 0, 0, 0}, rd[4] = {0, 0, 0, 0};
+            if (c <= col_max) {
+                V4 v0[4], v1[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    v0[k] = ldg_v4(p0[k] + c);
+                    v1[k] = ldg_v4(p1[k] + c);
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const T a0[4] = {v0[k].x, v0[k].y, v0[k].z, v0[k].w};
+                    const T a1[4] = {v1[k].x, v1[k].y, v1[k].z, v1[k].w};
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        r[e] = fma_t(w0[k], a0[e], r[e]);
+                        if constexpr (GRAD) {
+                            r1[e] = fma_t(w1[k], a1[e], r1[e]);
+                            rd[e] = fma_t(d0[k], a0[e], rd[e]);
+                            rd[e] = fma_t(d1[k], a1[e], rd[e]);
+                        } else {
+                            r[e] = fma_t(w1[k], a1[e], r[e]);
+                        }
+                    }
+                }
+                if constexpr (GRAD) {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) r[e] = fma_t(x1_t, r1[e], r[e]);
+                }
+            }
+            const int qb = qp + 4 * (lane - 1);       // first entry this lane produces (lanes 1..30)
+            const int gb = g0 + qb;                   // its cell index
+            const bool special = (g0 + qp <= 0) || (g0 + qp + kCellsPerPass + 3 >= nW - 2); // warp-uniform
+            const bool writer = (lane >= 1) && (lane <= 30);
+            auto emit = [&](const T(&x)[4], int set) {
+                const T am = __shfl_up_sync(0xffffffffu, x[3], 1);
+                const T ap = __shfl_down_sync(0xffffffffu, x[0], 1);
+                const T ap2 = __shfl_down_sync(0xffffffffu, x[1], 1);
+                const T n[7] = {am, x[0], x[1], x[2], x[3], ap, ap2};
+                V4 cf[4];
+                if (!special) {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) cf[e] = cell_coef_interior<T>(n[e], n[e + 1], n[e + 2], n[e + 3]);
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) cf[e] = cell_coef<T>(gb + e, nW, n[e], n[e + 1], n[e + 2], n[e + 3]);
+                }
+                if (writer) {
+#pragma unroll
+                    for (int e = 0; e < 4; ++e)
+                        if (qb + e < q_end) rowbuf[(size_t)swz(qb + e - q0) * NSET + set] = cf[e];
+                }
+            };
+            emit(r, 0);
+            if constexpr (GRAD) {
+                emit(r1, 1);
+                emit(rd, 2);
+            }
+        }
+        __syncwarp();
+        // ---- samples of this tile: rint(t_j) in [q0, q0+TC-2]
+        int jb = j_hi;
+        if (q_end < n_entries) {
+            const T thr = (T)(q0 + TC) - (T)1.5;
+            auto probe = [&](int j) { return fma_t(tab[ja + j].x, a_t, b_t); };
+            jb = ja + warp_count_less(j_hi - ja, thr, lane, probe);
+        }
+        const V4 *rb = rowbuf;
+#pragma unroll 4
+        for (int j = ja + lane; j < jb; j += kWarpSize) {
+            const V2 dw = tab[j];
+            const T dl = dw.x, wj = dw.y;
+            int idx;
+            T s;
+            split_rn(fma_t(dl, a_t, b_t), idx, s);
+            const int slot = swz(idx - q0);
+            const V4 cf = rb[slot * NSET];
+            const T val = poly3<T>(cf, s);
+            const T cl = col.eval(dl);
+            if constexpr (GRAD) {
+                const T ew = exp_scaled(cl * c_exp) * wj;
+                const T v1 = poly3<T>(rb[slot * NSET + 1], s);
+                const T vd = poly3<T>(rb[slot * NSET + 2], s);
+                const T f = ew * val;
+                accF += f;
+                accB = fma_t(ew, v1, accB);
+                accC = fma_t(f, cl, accC);
+                accD = fma_t(ew, vd, accD);
+            } else {
+                accF = fma_t(exp_scaled(cl) * wj, val, accF);
+            }
+        }
+        ja = jb;
+        __syncwarp();
+        if (q_end >= n_entries) break;
+    }
+    // ---- a5: wavelength integral (warp butterfly), a6: zero point
+    accF = warp_sum(accF);
+    if constexpr (GRAD) {
+        accB = warp_sum(accB);
+        accC = warp_sum(accC);
+        accD = warp_sum(accD);
+    }
+    if (lane == 0) {
+        const double S = R.scale, x0 = U.x0;
+        res[0] = S * x0 * (double)accF;
+        if constexpr (GRAD) {
+            res[1] = S * (double)accF;
+            res[2] = S * x0 * (double)accB;
+            res[3] = S * x0 * (double)accC;
+            res[4] = -S * x0 * (double)accD / U.opz;
+        }
+    }
+}
+
+// ---- the kernel -------------------------------------------------------------------------------
 template <typename T, bool GRAD, int NCL, bool STAGE, int NWARPS>
 __global__ void __launch_bounds__(NWARPS * kWarpSize, 1) sb_fused_kernel(const __grid_constant__ SbKParams P)
 {
     using V4 = typename Vec4<T>::type;
+    using V2 = typename Vec2<T>::type;
     constexpr int NSET = GRAD ? 3 : 1; // coefficient sets per cell: value [, M1-only, d/dphase]
+    constexpr int NRES = GRAD ? 5 : 1; // results per evaluation: m [, dm/d(x0, x1, c, t0)]
+    constexpr int NT = NWARPS * kWarpSize;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const SbModelParams &mp = P.mp;
-    const int TC = P.tile_cells;
-
-    // ---- shared memory carve-up: [warp row buffers][reduction scratch][band tables]
-    V4 *rowbuf = reinterpret_cast<V4 *>(smem_raw) + (size_t)warp * TC * NSET;
-    double *red = reinterpret_cast<double *>(smem_raw + (size_t)NWARPS * TC * NSET * sizeof(V4));
-    const T *tab_dlam = static_cast<const T *>(P.band_dlam);
-    const T *tab_w = static_cast<const T *>(P.band_w);
+    const int TC = P.tile_cells, CAP = P.chunk_cap, G = P.group_units;
+    const SmemLayout<T, GRAD> L(NWARPS, TC, CAP, P.n_band_total, STAGE);
+    V4 *rowbuf = reinterpret_cast<V4 *>(smem_raw + L.rowbuf) + (size_t)warp * TC * NSET;
+    EvalRec<T, GRAD> *recs = reinterpret_cast<EvalRec<T, GRAD> *>(smem_raw + L.recs);
+    double *res = reinterpret_cast<double *>(smem_raw + L.res);
+    UnitRec<T> *units = reinterpret_cast<UnitRec<T> *>(smem_raw + L.units);
+    double *uacc = reinterpret_cast<double *>(smem_raw + L.uacc);
+    int *misc = reinterpret_cast<int *>(smem_raw + L.misc); // [0] work counter, [1] evaluations in the group
+    const V2 *tab = static_cast<const V2 *>(P.band_tab);
     if (STAGE) {
-        T *s_dlam = reinterpret_cast<T *>(red + NWARPS * 5);
-        T *s_w = s_dlam + ((P.n_band_total + 3) & ~3);
-        for (int i = tid; i < P.n_band_total; i += NWARPS * kWarpSize) {
-            s_dlam[i] = tab_dlam[i];
-            s_w[i] = tab_w[i];
-        }
-        tab_dlam = s_dlam;
-        tab_w = s_w;
+        V2 *s_tab = reinterpret_cast<V2 *>(smem_raw + L.bands);
+        for (int i = tid; i < P.n_band_total; i += NT) s_tab[i] = tab[i];
+        tab = s_tab;
         __syncthreads();
     }
-    const T *__restrict__ M0 = static_cast<const T *>(P.m0);
-    const T *__restrict__ M1 = static_cast<const T *>(P.m1);
-    const T *__restrict__ g_time = static_cast<const T *>(P.time);
-    const T *__restrict__ g_zp = static_cast<const T *>(P.zp);
-    const T *__restrict__ g_flux = static_cast<const T *>(P.flux);
-    const T *__restrict__ g_err = static_cast<const T *>(P.fluxerr);
     T *o_flux = static_cast<T *>(P.out_flux);
     T *o_dflux = static_cast<T *>(P.out_dflux);
+    const T *__restrict__ g_flux = static_cast<const T *>(P.flux);
+    const T *__restrict__ g_err = static_cast<const T *>(P.fluxerr);
     const bool want_chi = (P.out_chi2 != nullptr) || (P.out_dchi2 != nullptr);
-
-    const int nP = mp.n_phase, nW = mp.n_wave, ld = mp.ld;
-    const double inv_dp = 1.0 / mp.dp, inv_dl = 1.0 / mp.dl;
     const long long n_units = (long long)P.n_sn * P.n_samples;
+    const long long n_groups = (n_units + G - 1) / G;
 
-    for (long long unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
-        const int sn = (int)(unit / P.n_samples);
-        const int ks = (int)(unit - (long long)sn * P.n_samples);
-        const int o_lo = __ldg(P.obs_offset + sn);
-        const int n_obs = __ldg(P.obs_offset + sn + 1) - o_lo;
-        const double z = (double)static_cast<const T *>(P.z)[sn];
-        const double x0 = (double)static_cast<const T *>(P.x0)[unit];
-        const double x1 = (double)static_cast<const T *>(P.x1)[unit];
-        const double cc = (double)static_cast<const T *>(P.c)[unit];
-        const double t0 = (double)static_cast<const T *>(P.t0)[unit];
-        const double opz = 1.0 + z;
-        const double inv_opz = 1.0 / opz;
-        const double a_d = inv_opz * inv_dl; // cells per observer-frame Angstrom
-        const T a_t = (T)a_d;
-
-        // colour law for this unit (a3).  Forward fp32: fold c*log2e into the coefficients.
-        Colour<T, NCL> col;
-        const double cscale = GRAD ? 1.0 : cc * exp_arg_scale<T>();
+    for (long long group = blockIdx.x; group < n_groups; group += gridDim.x) {
+        const long long u0 = group * G;
+        const int nu = (int)min((long long)G, n_units - u0);
+        // ---- unit records (one thread per unit)
+        if (tid < nu) {
+            const long long unit = u0 + tid;
+            UnitRec<T> &U = units[tid];
+            const int sn = (int)(unit / P.n_samples);
+            const int ks = (int)(unit - (long long)sn * P.n_samples);
+            const int o_lo = __ldg(P.obs_offset + sn);
+            const int n_obs = __ldg(P.obs_offset + sn + 1) - o_lo;
+            const double z = (double)static_cast<const T *>(P.z)[sn];
+            const double cc = (double)static_cast<const T *>(P.c)[unit];
+            const double opz = 1.0 + z, inv_opz = 1.0 / opz;
+            U.sn = sn;
+            U.o_lo = o_lo;
+            U.n_obs = n_obs;
+            U.out_base = (long long)o_lo * P.n_samples + (long long)ks * n_obs;
+            U.x0 = (double)static_cast<const T *>(P.x0)[unit];
+            U.x1 = static_cast<const T *>(P.x1)[unit];
+            U.t0 = (double)static_cast<const T *>(P.t0)[unit];
+            U.cc = cc;
+            U.opz = opz;
+            U.a_t = (T)(inv_opz / mp.dl);
+            U.al = (T)(inv_opz * mp.cl_inv_span);
+            // colour law of this unit (a3).  Forward fp32: fold c*log2e into the coefficients.
+            const double cscale = GRAD ? 1.0 : cc * exp_arg_scale<T>();
 #pragma unroll
-        for (int q = 0; q < NCL; ++q) col.a[q] = (T)(mp.cl[q] * cscale);
-        col.r_lo = (T)mp.r_lo;
-        col.r_hi = (T)mp.r_hi;
-        col.s_lo = (T)(mp.s_lo * cscale);
-        col.s_hi = (T)(mp.s_hi * cscale);
-        const double al_d = inv_opz * mp.cl_inv_span;
-        col.al = (T)al_d;
-        const T c_exp = (T)(cc * exp_arg_scale<T>()); // GRAD: arg = CL * c_exp
-
-        const long long out_base = (long long)o_lo * P.n_samples + (long long)ks * n_obs;
-        double chi = 0.0, dchi0 = 0.0, dchi1 = 0.0, dchi2 = 0.0, dchi3 = 0.0;
-
-        for (int i = warp; i < n_obs; i += NWARPS) {
-            const int o = o_lo + i;
-            const int b = __ldg(P.band + o);
-            double m = 0.0, dm0 = 0.0, dm1 = 0.0, dm2 = 0.0, dm3 = 0.0;
-            if ((unsigned)b >= (unsigned)P.n_bands) {
-                m = dm0 = dm1 = dm2 = dm3 = __longlong_as_double(0x7ff8000000000000LL);
-            } else {
-                const int boff = __ldg(P.band_off + b);
-                const int nb = __ldg(P.band_off + b + 1) - boff;
-                const double lam_first = __ldg(P.band_lam_first + b);
-                const T *dlam = tab_dlam + boff;
-                const T *wtab = tab_w + boff;
-                // ---- a1: phase
-                const double p = ((double)g_time[o] - t0) / opz;
-                const double up = (p - mp.p0) * inv_dp;
-                // in-range band samples [j_lo, j_hi): 0 <= u_j <= nW-1
-                const double dl_lo = mp.l0 * opz - lam_first;
-                const double dl_hi = (mp.l0 + (double)(nW - 1) * mp.dl) * opz - lam_first;
-                int j_lo = 0, j_hi = 0;
-                const bool phase_ok = (up >= 0.0) && (up <= (double)(nP - 1));
-                if (phase_ok) {
-                    // membership is decided in fp64 (dlam_j is exact for fp32-representable grids)
-                    auto probe = [&](int j) { return (double)dlam[j]; };
-                    j_lo = warp_count_less(nb, dl_lo, lane, probe, false);
-                    j_hi = warp_count_less(nb, dl_hi, lane, probe, true);
-                }
-                if (j_lo < j_hi) {
-                    int kp = min((int)floor(up), nP - 2);
-                    const double tau = up - (double)kp;
-                    const bool pborder = (kp == 0) || (kp == nP - 2);
-                    double wv[4], wd[4];
-                    phase_weights(tau, pborder, inv_dp, wv, wd);
-                    int row[4];
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) row[k] = min(max(kp - 1 + k, 0), nP - 1) * ld;
-                    T w0[4], w1[4], d0[4], d1[4];
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        w0[k] = (T)wv[k];
-                        w1[k] = GRAD ? (T)wv[k] : (T)(wv[k] * x1);
-                        d0[k] = (T)wd[k];
-                        d1[k] = (T)(wd[k] * x1);
-                    }
-                    const T x1_t = (T)x1;
-                    // ---- a1: wavelength geometry relative to the first cell
-                    const double ub = (lam_first * inv_opz - mp.l0) * inv_dl; // u of dlam = 0
-                    const double u_first = (double)dlam[j_lo] * a_d + ub;
-                    const double u_last = (double)dlam[j_hi - 1] * a_d + ub;
-                    const int i_first = min(max((int)floor(u_first), 0), nW - 2);
-                    const int i_last = min(max((int)floor(u_last), 0), nW - 2);
-                    const int n_entries = i_last - i_first + 3; // cells i_first-1 .. i_last+1
-                    const T b_t = (T)(ub - (double)i_first + 0.5); // t_j = u_j - (i_first-1) - 1/2
-                    col.be = (T)((lam_first * inv_opz - mp.cl_b) * mp.cl_inv_span);
-
-                    T accF = 0, accB = 0, accC = 0, accD = 0;
-                    int ja = j_lo;
-                    for (int q0 = 0; ja < j_hi; q0 += TC - 2) {
-                        const int q_end = min(q0 + TC, n_entries);
-                        // ---- a2: collapse phase rows, convert to per-cell cubic coefficients
-                        for (int qs = q0; qs < q_end; qs += kCellsPerPass) {
-                            const int g_lane = i_first - 1 + qs + lane - 1; // lane l: node of cell qs+l-1
-                            const int node = min(max(g_lane, 0), nW - 1);
-                            T r = 0, r1 = 0, rd = 0;
-#pragma unroll
-                            for (int k = 0; k < 4; ++k) {
-                                const T v0 = __ldg(M0 + row[k] + node);
-                                const T v1 = __ldg(M1 + row[k] + node);
-                                r = fma_t(w0[k], v0, r);
-                                if (GRAD) {
-                                    r1 = fma_t(w1[k], v1, r1);
-                                    rd = fma_t(d0[k], v0, rd);
-                                    rd = fma_t(d1[k], v1, rd);
-                                } else {
-                                    r = fma_t(w1[k], v1, r);
-                                }
-                            }
-                            if (GRAD) r = fma_t(x1_t, r1, r);
-                            const int q = qs + lane - 1; // entry this lane produces (lanes 1..29)
-                            {
-                                T am = __shfl_up_sync(0xffffffffu, r, 1);
-                                T ap = __shfl_down_sync(0xffffffffu, r, 1);
-                                T a2 = __shfl_down_sync(0xffffffffu, r, 2);
-                                V4 cf = cell_coef<T>(g_lane, nW, am, r, ap, a2);
-                                if (lane >= 1 && lane <= kCellsPerPass && q < q_end) rowbuf[(q - q0) * NSET] = cf;
-                            }
-                            if (GRAD) {
-                                T am = __shfl_up_sync(0xffffffffu, r1, 1);
-                                T ap = __shfl_down_sync(0xffffffffu, r1, 1);
-                                T a2 = __shfl_down_sync(0xffffffffu, r1, 2);
-                                V4 cf = cell_coef<T>(g_lane, nW, am, r1, ap, a2);
-                                if (lane >= 1 && lane <= kCellsPerPass && q < q_end) rowbuf[(q - q0) * NSET + 1] = cf;
-                                am = __shfl_up_sync(0xffffffffu, rd, 1);
-                                ap = __shfl_down_sync(0xffffffffu, rd, 1);
-                                a2 = __shfl_down_sync(0xffffffffu, rd, 2);
-                                cf = cell_coef<T>(g_lane, nW, am, rd, ap, a2);
-                                if (lane >= 1 && lane <= kCellsPerPass && q < q_end) rowbuf[(q - q0) * NSET + 2] = cf;
-                            }
-                        }
-                        __syncwarp();
-                        // ---- samples of this tile: rint(t_j) in [q0, q0+TC-2]
-                        int jb = j_hi;
-                        if (q_end < n_entries) {
-                            const T thr = (T)(q0 + TC) - (T)1.5;
-                            auto probe = [&](int j) { return fma_t(dlam[ja + j], a_t, b_t); };
-                            jb = ja + warp_count_less(j_hi - ja, thr, lane, probe, false);
-                        }
-                        const V4 *rb = rowbuf - (size_t)q0 * NSET;
-#pragma unroll 4
-                        for (int j = ja + lane; j < jb; j += kWarpSize) {
-                            const T dl = dlam[j];
-                            const T wj = wtab[j];
-                            int idx;
-                            T s;
-                            split_rn(fma_t(dl, a_t, b_t), idx, s);
-                            const V4 cf = rb[idx * NSET];
-                            const T val = poly3<T>(cf, s);
-                            const T cl = col.eval(dl);
-                            if (GRAD) {
-                                const T ew = exp_scaled(cl * c_exp) * wj;
-                                const T v1 = poly3<T>(rb[idx * NSET + 1], s);
-                                const T vd = poly3<T>(rb[idx * NSET + 2], s);
-                                const T f = ew * val;
-                                accF += f;
-                                accB = fma_t(ew, v1, accB);
-                                accC = fma_t(f, cl, accC);
-                                accD = fma_t(ew, vd, accD);
-                            } else {
-                                accF = fma_t(exp_scaled(cl) * wj, val, accF);
-                            }
-                        }
-                        ja = jb;
-                        __syncwarp();
-                        if (q_end >= n_entries) break;
-                    }
-                    // ---- a5: wavelength integral (warp butterfly), a6: zero point
-                    accF = warp_sum(accF);
-                    double S = 1.0;
-                    if (g_zp != nullptr) S = exp10(0.4 * (double)g_zp[o]) * __ldg(P.band_zpab_inv + b);
-                    m = S * x0 * (double)accF;
-                    if (GRAD) {
-                        accB = warp_sum(accB);
-                        accC = warp_sum(accC);
-                        accD = warp_sum(accD);
-                        dm0 = S * (double)accF;
-                        dm1 = S * x0 * (double)accB;
-                        dm2 = S * x0 * (double)accC;
-                        dm3 = -S * x0 * (double)accD * inv_opz;
-                    }
-                }
-            }
-            // ---- outputs of this evaluation
-            if (lane == 0) {
-                if (o_flux) o_flux[out_base + i] = (T)m;
-                if (GRAD && o_dflux) {
-                    V4 *dst = reinterpret_cast<V4 *>(o_dflux) + (out_base + i);
-                    *dst = make_v4<T>((T)dm0, (T)dm1, (T)dm2, (T)dm3);
-                }
-            }
-            if (want_chi) { // a7 (every lane carries the same partial)
-                const double f = (double)g_flux[o], e = (double)g_err[o];
-                const double rr = (f - m) / e;
-                chi += rr * rr;
-                if (GRAD) {
-                    const double g = -2.0 * (f - m) / (e * e);
-                    dchi0 += g * dm0;
-                    dchi1 += g * dm1;
-                    dchi2 += g * dm2;
-                    dchi3 += g * dm3;
-                }
-            }
+            for (int q = 0; q < SB_MAX_CL; ++q) U.cl[q] = (T)(mp.cl[q] * cscale);
+            U.s_lo = (T)(mp.s_lo * cscale);
+            U.s_hi = (T)(mp.s_hi * cscale);
+            U.c_exp = (T)(cc * exp_arg_scale<T>());
         }
-        if (want_chi) { // fixed-order sum over warps: deterministic
-            if (lane == 0) {
-                red[warp * 5 + 0] = chi;
-                red[warp * 5 + 1] = dchi0;
-                red[warp * 5 + 2] = dchi1;
-                red[warp * 5 + 3] = dchi2;
-                red[warp * 5 + 4] = dchi3;
+        if (tid < kMaxGroup * 5) uacc[tid] = 0.0;
+        __syncthreads();
+        if (tid == 0) {
+            int acc = 0;
+            for (int u = 0; u < nu; ++u) {
+                units[u].e_begin = acc;
+                acc += units[u].n_obs;
+            }
+            misc[1] = acc;
+        }
+        __syncthreads();
+        const int n_ev = misc[1];
+
+        for (int c0 = 0; c0 < n_ev; c0 += CAP) {
+            const int nc = min(CAP, n_ev - c0);
+            // ---- prologue: one thread per evaluation
+            for (int el = tid; el < nc; el += NT)
+                eval_prologue<T, GRAD>(P, units, nu, c0 + el, recs[el], res + (size_t)el * NRES, tab);
+            if (tid == 0) misc[0] = 0;
+            __syncthreads();
+            // ---- main: warps pull evaluations
+            for (;;) {
+                int el = 0;
+                if (lane == 0) el = atomicAdd(&misc[0], 1);
+                el = __shfl_sync(0xffffffffu, el, 0);
+                if (el >= nc) break;
+                const EvalRec<T, GRAD> &R = recs[el];
+                if (R.n_entries > 0)
+                    eval_warp<T, GRAD, NCL>(P, units[R.unit], R, rowbuf, TC, tab, lane, res + (size_t)el * NRES);
             }
             __syncthreads();
-            if (tid < 5) {
-                double s = 0.0;
-                for (int w = 0; w < NWARPS; ++w) s += red[w * 5 + tid];
-                if (tid == 0) {
-                    if (P.out_chi2) static_cast<T *>(P.out_chi2)[unit] = (T)s;
-                } else if (GRAD && P.out_dchi2) {
-                    static_cast<T *>(P.out_dchi2)[unit * 4 + (tid - 1)] = (T)s;
+            // ---- epilogue: results out (coalesced within a unit), chi^2 terms in place (a7)
+            for (int el = tid; el < nc; el += NT) {
+                const EvalRec<T, GRAD> &R = recs[el];
+                const UnitRec<T> &U = units[R.unit];
+                double *rr = res + (size_t)el * NRES;
+                const long long oi = U.out_base + (R.obs - U.o_lo);
+                const double m = rr[0];
+                if (o_flux) o_flux[oi] = (T)m;
+                if constexpr (GRAD) {
+                    if (o_dflux) reinterpret_cast<V4 *>(o_dflux)[oi] = make_v4<T>((T)rr[1], (T)rr[2], (T)rr[3], (T)rr[4]);
+                }
+                if (want_chi) {
+                    const double f = (double)g_flux[R.obs], e = (double)g_err[R.obs];
+                    const double q = (f - m) / e;
+                    rr[0] = q * q;
+                    if constexpr (GRAD) {
+                        const double g = -2.0 * (f - m) / (e * e);
+                        rr[1] *= g;
+                        rr[2] *= g;
+                        rr[3] *= g;
+                        rr[4] *= g;
+                    }
                 }
             }
             __syncthreads();
+            if (want_chi) { // one warp per unit, lanes stride its terms, fixed butterfly: deterministic
+                for (int u = warp; u < nu; u += NWARPS) {
+                    const int lo = max(units[u].e_begin, c0) - c0;
+                    const int hi = min(units[u].e_begin + units[u].n_obs, c0 + nc) - c0;
+                    double s[NRES];
+#pragma unroll
+                    for (int k = 0; k < NRES; ++k) s[k] = 0.0;
+                    for (int el = lo + lane; el < hi; el += kWarpSize) {
+#pragma unroll
+                        for (int k = 0; k < NRES; ++k) s[k] += res[(size_t)el * NRES + k];
+                    }
+#pragma unroll
+                    for (int k = 0; k < NRES; ++k) s[k] = warp_sum(s[k]);
+                    if (lane == 0) {
+#pragma unroll
+                        for (int k = 0; k < NRES; ++k) uacc[u * 5 + k] += s[k];
+                    }
+                }
+                __syncthreads();
+            }
         }
+        if (want_chi && tid < nu) {
+            const long long unit = u0 + tid;
+            if (P.out_chi2) static_cast<T *>(P.out_chi2)[unit] = (T)uacc[tid * 5];
+            if constexpr (GRAD) {
+                if (P.out_dchi2)
+                    reinterpret_cast<V4 *>(P.out_dchi2)[unit] =
+                        make_v4<T>((T)uacc[tid * 5 + 1], (T)uacc[tid * 5 + 2], (T)uacc[tid * 5 + 3], (T)uacc[tid * 5 + 4]);
+            }
+        }
+        __syncthreads();
     }
 }
 
