@@ -283,7 +283,8 @@ int launch_typed(SbKParams &kp, const sb_bands *b, int n_obs_total, cudaStream_t
     int tc_full = (int)std::ceil(b->max_span / kp.mp.dl) + 12;
     if (tc_full > kp.mp.n_wave + 12) tc_full = kp.mp.n_wave + 12;
     tc_full = (tc_full + 7) & ~7;
-    if (tc_full < 32) tc_full = 32;
+    if (tc_full < 64) tc_full = 64;
+    if (tc_full > 360) tc_full = 360; // kPassesPerTile collapse passes of 120 entries per tile
     // stage the band tables in shared memory when they fit beside >= 128-entry row buffers (fp32 only)
     const sb::SmemLayout<T, GRAD> fixed(NWARPS, 0, cap, b->n_total, false);
     const size_t band_bytes = sb::SmemLayout<T, GRAD>(NWARPS, 0, cap, b->n_total, true).total - fixed.total;
@@ -292,7 +293,7 @@ int launch_typed(SbKParams &kp, const sb_bands *b, int n_obs_total, cudaStream_t
     int tc = (int)(avail / ((size_t)NWARPS * cell_bytes));
     tc &= ~7;
     if (tc > tc_full) tc = tc_full;
-    if (tc < 32) return SB_ELIMIT;
+    if (tc < 64) return SB_ELIMIT;
     kp.tile_cells = tc;
     const size_t smem = sb::SmemLayout<T, GRAD>(NWARPS, tc, cap, b->n_total, stage).total;
     const long long n_units = (long long)kp.n_sn * kp.n_samples;

@@ -28,6 +28,8 @@
 //   a8  analytic gradient: three coefficient sets (value row, M1-only row, d/dphase row) and four
 //       accumulators give d m/d(x0, x1, c, t0).
 #pragma once
+#include <type_traits>
+
 #include "sb_internal.h"
 
 namespace sb {
@@ -53,21 +55,6 @@ __device__ __forceinline__ double4 ldg_v4(const double *p)
     const double2 a = __ldg(reinterpret_cast<const double2 *>(p));
     const double2 b = __ldg(reinterpret_cast<const double2 *>(p) + 1);
     return make_double4(a.x, a.y, b.x, b.y);
-}
-
-// Split t into the nearest integer and the signed remainder s = t - rint(t), |s| <= 1/2.
-// fp32: magic-number rounding on the FMA pipe (no F2I/FRND on the quarter-rate XU pipe).
-__device__ __forceinline__ void split_rn(float t, int &idx, float &s)
-{
-    const float magic = 12582912.0f; // 1.5 * 2^23: valid for |t| < 2^22
-    float r = __fadd_rn(t, magic);
-    idx = __float_as_int(r) - 0x4B400000;
-    s = __fsub_rn(t, __fsub_rn(r, magic));
-}
-__device__ __forceinline__ void split_rn(double t, int &idx, double &s)
-{
-    idx = __double2int_rn(t);
-    s = t - (double)idx;
 }
 
 __device__ __forceinline__ float fma_t(float a, float b, float c) { return __fmaf_rn(a, b, c); }
@@ -156,10 +143,8 @@ __device__ __forceinline__ T poly3(const typename Vec4<T>::type &a, T s)
     return fma_t(fma_t(fma_t(a.w, s, a.z), s, a.y), s, a.x);
 }
 
-// Row-buffer slot of entry q: XOR swizzle inside groups of 8 slots so that the four 128-bit stores
-// of a collapse pass (lane l writes entries 4l..4l+3) are bank-conflict free.
-__device__ __forceinline__ int swz(int q) { return q ^ ((q >> 3) & 3); }
-
+// Row-buffer slot of entry q: q ^ ((q >> 3) & 3) -- an XOR swizzle inside groups of 8 slots so that the
+// four 128-bit stores of a collapse pass (lane l writes entries 4l..4l+3) are bank-conflict free.
 // Cubic-convolution weights (Keys a = -1/2) and their derivatives, or the linear border pair.
 __device__ __forceinline__ void phase_weights(double tau, bool border, double inv_dp, double w[4], double d[4])
 {
@@ -178,6 +163,12 @@ __device__ __forceinline__ void phase_weights(double tau, bool border, double in
     d[2] = 0.5 * (-9.0 * t2 + 8.0 * tau + 1.0) * inv_dp;
     d[3] = 0.5 * (3.0 * t2 - 2.0 * tau) * inv_dp;
 }
+
+// Colour-law evaluation modes of one evaluation (decided in the prologue, warp-uniform):
+//   CM_GENERIC  clamp + polynomial + linear continuation (any sample anywhere)
+//   CM_INSIDE   every in-range sample lies inside [cl_lo, cl_hi]: polynomial only
+//   CM_LINEAR   every sample lies on one side outside the range: CL = lin_a + lin_b * dlam
+enum { CM_GENERIC = 0, CM_INSIDE = 1, CM_LINEAR = 2 };
 
 // ---- shared-memory records -----------------------------------------------------------------
 // Per unit (supernova x sample) of the current group.
@@ -202,28 +193,13 @@ template <typename T> struct EvalRecBase {
     T b_t, be;            // t_j = dlam_j*a_t + b_t ; r_j = dlam_j*al + be
     int32_t unit, obs;    // group-local unit, global observation index
     double scale;         // zero-point factor S
+    T lin_a, lin_b;       // CM_LINEAR: CL_j = lin_a + lin_b * dlam_j (scaled like UnitRec::cl)
+    int32_t cmode;        // colour-law mode of this evaluation (CM_*)
+    int32_t pad_;
 };
 template <typename T, bool GRAD> struct EvalRec : EvalRecBase<T> {};
 template <typename T> struct EvalRec<T, true> : EvalRecBase<T> {
     T d0[4], d1[4];       // d/dp weights on M0 and on M1 (d1 already times x1)
-};
-
-template <typename T, int NCL> struct Colour {
-    T a[NCL];        // polynomial coefficients
-    T r_lo, r_hi;    // clamp range of the reduced wavelength
-    T s_lo, s_hi;    // continuation slopes (same scaling as a[])
-    T al, be;        // r_j = dlam_j * al + be
-    __device__ __forceinline__ T eval(T dl) const
-    {
-        T r = fma_t(dl, al, be);
-        T rc = fmin(fmax(r, r_lo), r_hi);
-        T d = r - rc;
-        T slope = d > (T)0 ? s_hi : s_lo;
-        T p = a[NCL - 1];
-#pragma unroll
-        for (int q = NCL - 2; q >= 0; --q) p = fma_t(p, rc, a[q]);
-        return fma_t(slope, d, p);
-    }
 };
 
 template <typename T, bool GRAD> struct SmemLayout {
@@ -320,21 +296,123 @@ __device__ __forceinline__ void eval_prologue(const SbKParams &P, const UnitRec<
     R.j_lo = boff + j_lo;
     R.j_hi = boff + j_hi;
     R.b_t = (T)(ub - (double)g0 - 0.5); // t_j = u_j - g0 - 1/2, rint(t_j) = entry, remainder in [-1/2, 1/2]
-    R.be = (T)((lam_first * inv_opz - mp.cl_b) * mp.cl_inv_span);
+    const double al_d = inv_opz * mp.cl_inv_span;
+    const double be_d = (lam_first * inv_opz - mp.cl_b) * mp.cl_inv_span;
+    R.be = (T)be_d;
+    // ---- a3: colour-law mode of this evaluation (reduced wavelength is monotone in j)
+    {
+        const double r_a = (double)tab[boff + j_lo].x * al_d + be_d;
+        const double r_b = (double)tab[boff + j_hi - 1].x * al_d + be_d;
+        const double r_min = fmin(r_a, r_b), r_max = fmax(r_a, r_b);
+        const double margin = 1e-4; // far above the fp32 rounding of r_j, so every lane agrees with the mode
+        const double cscale = GRAD ? 1.0 : U.cc * exp_arg_scale<T>();
+        int cmode = CM_GENERIC;
+        double lin_a = 0.0, lin_b = 0.0;
+        if (r_min >= mp.r_lo + margin && r_max <= mp.r_hi - margin) {
+            cmode = CM_INSIDE;
+        } else if (r_min >= mp.r_hi + margin) {
+            cmode = CM_LINEAR;
+            lin_a = (mp.p_hi + mp.s_hi * (be_d - mp.r_hi)) * cscale;
+            lin_b = mp.s_hi * al_d * cscale;
+        } else if (r_max <= mp.r_lo - margin) {
+            cmode = CM_LINEAR;
+            lin_a = (mp.p_lo + mp.s_lo * (be_d - mp.r_lo)) * cscale;
+            lin_b = mp.s_lo * al_d * cscale;
+        }
+        R.cmode = cmode;
+        R.lin_a = (T)lin_a;
+        R.lin_b = (T)lin_b;
+    }
     double S = 1.0;
     if (P.zp != nullptr) S = exp10(0.4 * (double)static_cast<const T *>(P.zp)[o]) * __ldg(P.band_zpab_inv + b);
     R.scale = S;
 }
 
+// ---- shared-memory access through 32-bit addresses (no generic-pointer arithmetic in the loops)
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void sts_v4(uint32_t a, const float4 &v)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void sts_v4(uint32_t a, const double4 &v)
+{
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v.x), "d"(v.y) : "memory");
+    asm volatile("st.shared.v2.f64 [%0+16], {%1, %2};" ::"r"(a), "d"(v.z), "d"(v.w) : "memory");
+}
+__device__ __forceinline__ void lds_v4(uint32_t a, float4 &v)
+{
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+}
+__device__ __forceinline__ void lds_v4(uint32_t a, double4 &v)
+{
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+16];" : "=d"(v.z), "=d"(v.w) : "r"(a));
+}
+
+// Split t into a row-buffer key and the signed remainder s = t - rint(t), |s| <= 1/2.
+//   fp32: magic-number rounding on the FMA pipe (no F2I/FRND on the quarter-rate XU pipe); the key
+//   is the raw bit pattern of t + 1.5*2^23, i.e. rint(t) + kKeyBias<float>.   fp64: key = rint(t).
+// The slot of entry q is swz(q); since the bias and the tile origin are multiples of 32, swz(key)
+// = swz(q) + bias, and the bias is folded into the base address once per tile.
+template <typename T> struct KeyBias;
+template <> struct KeyBias<float> { static constexpr uint32_t value = 0x4B400000u; };
+template <> struct KeyBias<double> { static constexpr uint32_t value = 0u; };
+__device__ __forceinline__ void split_key(float t, uint32_t &key, float &s)
+{
+    const float magic = 12582912.0f; // 1.5 * 2^23: valid for |t| < 2^22
+    const float r = __fadd_rn(t, magic);
+    key = __float_as_uint(r);
+    s = __fsub_rn(t, __fsub_rn(r, magic));
+}
+__device__ __forceinline__ void split_key(double t, uint32_t &key, double &s)
+{
+    const int i = __double2int_rn(t);
+    key = (uint32_t)i;
+    s = t - (double)i;
+}
+__device__ __forceinline__ uint32_t swz_key(uint32_t k) { return k ^ ((k >> 3) & 3u); }
+
+template <typename T, int NCL> struct Colour {
+    T a[NCL];        // polynomial coefficients
+    T r_lo, r_hi;    // clamp range of the reduced wavelength
+    T s_lo, s_hi;    // continuation slopes (same scaling as a[])
+    T al, be;        // r_j = dlam_j * al + be
+    T lin_a, lin_b;  // CM_LINEAR
+    template <int CM> __device__ __forceinline__ T eval(T dl) const
+    {
+        if constexpr (CM == CM_LINEAR) {
+            return fma_t(dl, lin_b, lin_a);
+        } else if constexpr (CM == CM_INSIDE) {
+            const T r = fma_t(dl, al, be);
+            T p = a[NCL - 1];
+#pragma unroll
+            for (int q = NCL - 2; q >= 0; --q) p = fma_t(p, r, a[q]);
+            return p;
+        } else {
+            const T r = fma_t(dl, al, be);
+            const T rc = fmin(fmax(r, r_lo), r_hi);
+            const T d = r - rc;
+            const T slope = d > (T)0 ? s_hi : s_lo;
+            T p = a[NCL - 1];
+#pragma unroll
+            for (int q = NCL - 2; q >= 0; --q) p = fma_t(p, rc, a[q]);
+            return fma_t(slope, d, p);
+        }
+    }
+};
+
 // ---- main: one warp integrates one evaluation -------------------------------------------------
+constexpr int kPassesPerTile = 3; // a tile is at most 3 collapse passes (360 entries)
+
 template <typename T, bool GRAD, int NCL>
 __device__ __forceinline__ void eval_warp(const SbKParams &P, const UnitRec<T> &U, const EvalRec<T, GRAD> &R,
-                                          typename Vec4<T>::type *rowbuf, int TC,
+                                          uint32_t rowbuf_s, int TC,
                                           const typename Vec2<T>::type *__restrict__ tab, int lane, double *res)
 {
     using V4 = typename Vec4<T>::type;
     using V2 = typename Vec2<T>::type;
     constexpr int NSET = GRAD ? 3 : 1;
+    constexpr uint32_t kSlot = (uint32_t)sizeof(V4) * NSET; // bytes per row-buffer entry
     const SbModelParams &mp = P.mp;
     const int nW = mp.n_wave;
     const T *__restrict__ M0 = static_cast<const T *>(P.m0);
@@ -350,8 +428,8 @@ __device__ __forceinline__ void eval_warp(const SbKParams &P, const UnitRec<T> &
         w0[k] = R.w0[k];
         w1[k] = R.w1[k];
         if constexpr (GRAD) { d0[k] = R.d0[k]; d1[k] = R.d1[k]; }
-        p0[k] = M0 + R.rowoff[k];
-        p1[k] = M1 + R.rowoff[k];
+        p0[k] = M0 + (R.rowoff[k] + col0 + 4 * lane);
+        p1[k] = M1 + (R.rowoff[k] + col0 + 4 * lane);
     }
     const T x1_t = U.x1;
     const T a_t = U.a_t, b_t = R.b_t;
@@ -364,22 +442,29 @@ __device__ __forceinline__ void eval_warp(const SbKParams &P, const UnitRec<T> &
     col.s_hi = U.s_hi;
     col.al = U.al;
     col.be = R.be;
+    col.lin_a = R.lin_a;
+    col.lin_b = R.lin_b;
     const T c_exp = U.c_exp;
+    const int cmode = R.cmode;
 
     T accF = 0, accB = 0, accC = 0, accD = 0;
     int ja = R.j_lo;
-    for (int q0 = 0;; q0 += TC - 8) {
+    const int tile_step = (TC - 8) & ~31; // tile origins stay multiples of 32 (see split_key)
+    for (int q0 = 0;; q0 += tile_step) {
         const int q_end = min(q0 + TC, n_entries);
         // ---- a2: collapse the phase rows (4 nodes per lane), convert to per-cell cubic coefficients
-        for (int qp = q0; qp < q_end; qp += kCellsPerPass) {
+#pragma unroll
+        for (int ps = 0; ps < kPassesPerTile; ++ps) {
+            const int qp = q0 + ps * kCellsPerPass;
+            if (qp >= q_end) break;
             const int c = col0 + qp + 4 * lane; // this lane's nodes: columns c..c+3 = cells' left nodes
             T r[4] = {0, 0, 0, 0}, r1[4] = {0, 0, 0, 0}, rd[4] = {0, 0, 0, 0};
             if (c <= col_max) {
                 V4 v0[4], v1[4];
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                    v0[k] = ldg_v4(p0[k] + c);
-                    v1[k] = ldg_v4(p1[k] + c);
+                    v0[k] = ldg_v4(p0[k] + ps * kCellsPerPass);
+                    v1[k] = ldg_v4(p1[k] + ps * kCellsPerPass);
                 }
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
@@ -406,11 +491,14 @@ __device__ __forceinline__ void eval_warp(const SbKParams &P, const UnitRec<T> &
             const int gb = g0 + qb;                   // its cell index
             const bool special = (g0 + qp <= 0) || (g0 + qp + kCellsPerPass + 3 >= nW - 2); // warp-uniform
             const bool writer = (lane >= 1) && (lane <= 30);
-            auto emit = [&](const T(&x)[4], int set) {
-                const T am = __shfl_up_sync(0xffffffffu, x[3], 1);
-                const T ap = __shfl_down_sync(0xffffffffu, x[0], 1);
-                const T ap2 = __shfl_down_sync(0xffffffffu, x[1], 1);
-                const T n[7] = {am, x[0], x[1], x[2], x[3], ap, ap2};
+            // lane l's four entries live in one 8-slot swizzle group half: slots (qb-q0)+e ^ x, x fixed
+            const uint32_t qrel = (uint32_t)(qb - q0);
+            const uint32_t x = (qrel >> 3) & 3u;
+            auto emit = [&](const T(&n4)[4], int set) {
+                const T am = __shfl_up_sync(0xffffffffu, n4[3], 1);
+                const T ap = __shfl_down_sync(0xffffffffu, n4[0], 1);
+                const T ap2 = __shfl_down_sync(0xffffffffu, n4[1], 1);
+                const T n[7] = {am, n4[0], n4[1], n4[2], n4[3], ap, ap2};
                 V4 cf[4];
                 if (!special) {
 #pragma unroll
@@ -422,7 +510,7 @@ __device__ __forceinline__ void eval_warp(const SbKParams &P, const UnitRec<T> &
                 if (writer) {
 #pragma unroll
                     for (int e = 0; e < 4; ++e)
-                        if (qb + e < q_end) rowbuf[(size_t)swz(qb + e - q0) * NSET + set] = cf[e];
+                        if (qb + e < q_end) sts_v4(rowbuf_s + ((qrel + e) ^ x) * kSlot + set * (uint32_t)sizeof(V4), cf[e]);
                 }
             };
             emit(r, 0);
@@ -439,34 +527,49 @@ __device__ __forceinline__ void eval_warp(const SbKParams &P, const UnitRec<T> &
             auto probe = [&](int j) { return fma_t(tab[ja + j].x, a_t, b_t); };
             jb = ja + warp_count_less(j_hi - ja, thr, lane, probe);
         }
-        const V4 *rb = rowbuf;
+        const uint32_t base = rowbuf_s - (KeyBias<T>::value + (uint32_t)q0) * kSlot;
+        auto samples = [&](auto cm_tag) {
+            constexpr int CM = decltype(cm_tag)::value;
 #pragma unroll 4
-        for (int j = ja + lane; j < jb; j += kWarpSize) {
-            const V2 dw = tab[j];
-            const T dl = dw.x, wj = dw.y;
-            int idx;
-            T s;
-            split_rn(fma_t(dl, a_t, b_t), idx, s);
-            const int slot = swz(idx - q0);
-            const V4 cf = rb[slot * NSET];
-            const T val = poly3<T>(cf, s);
-            const T cl = col.eval(dl);
-            if constexpr (GRAD) {
-                const T ew = exp_scaled(cl * c_exp) * wj;
-                const T v1 = poly3<T>(rb[slot * NSET + 1], s);
-                const T vd = poly3<T>(rb[slot * NSET + 2], s);
-                const T f = ew * val;
-                accF += f;
-                accB = fma_t(ew, v1, accB);
-                accC = fma_t(f, cl, accC);
-                accD = fma_t(ew, vd, accD);
-            } else {
-                accF = fma_t(exp_scaled(cl) * wj, val, accF);
+            for (int j = ja + lane; j < jb; j += kWarpSize) {
+                const V2 dw = tab[j];
+                const T dl = dw.x, wj = dw.y;
+                uint32_t key;
+                T s;
+                split_key(fma_t(dl, a_t, b_t), key, s);
+                const uint32_t addr = swz_key(key) * kSlot + base;
+                V4 cf;
+                lds_v4(addr, cf);
+                const T val = poly3<T>(cf, s);
+                const T cl = col.template eval<CM>(dl);
+                if constexpr (GRAD) {
+                    V4 c1, cd;
+                    lds_v4(addr + (uint32_t)sizeof(V4), c1);
+                    lds_v4(addr + 2u * (uint32_t)sizeof(V4), cd);
+                    const T ew = exp_scaled(cl * c_exp) * wj;
+                    const T v1 = poly3<T>(c1, s);
+                    const T vd = poly3<T>(cd, s);
+                    const T f = ew * val;
+                    accF += f;
+                    accB = fma_t(ew, v1, accB);
+                    accC = fma_t(f, cl, accC);
+                    accD = fma_t(ew, vd, accD);
+                } else {
+                    accF = fma_t(exp_scaled(cl) * wj, val, accF);
+                }
             }
-        }
+        };
+        if (cmode == CM_INSIDE) samples(std::integral_constant<int, CM_INSIDE>{});
+        else if (cmode == CM_LINEAR) samples(std::integral_constant<int, CM_LINEAR>{});
+        else samples(std::integral_constant<int, CM_GENERIC>{});
         ja = jb;
         __syncwarp();
         if (q_end >= n_entries) break;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            p0[k] += tile_step;
+            p1[k] += tile_step;
+        }
     }
     // ---- a5: wavelength integral (warp butterfly), a6: zero point
     accF = warp_sum(accF);
@@ -502,7 +605,7 @@ __global__ void __launch_bounds__(NWARPS * kWarpSize, 1) sb_fused_kernel(const _
     const SbModelParams &mp = P.mp;
     const int TC = P.tile_cells, CAP = P.chunk_cap, G = P.group_units;
     const SmemLayout<T, GRAD> L(NWARPS, TC, CAP, P.n_band_total, STAGE);
-    V4 *rowbuf = reinterpret_cast<V4 *>(smem_raw + L.rowbuf) + (size_t)warp * TC * NSET;
+    const uint32_t rowbuf_s = smem_addr(smem_raw + L.rowbuf) + (uint32_t)warp * (uint32_t)TC * (uint32_t)(NSET * sizeof(V4));
     EvalRec<T, GRAD> *recs = reinterpret_cast<EvalRec<T, GRAD> *>(smem_raw + L.recs);
     double *res = reinterpret_cast<double *>(smem_raw + L.res);
     UnitRec<T> *units = reinterpret_cast<UnitRec<T> *>(smem_raw + L.units);
@@ -584,7 +687,7 @@ __global__ void __launch_bounds__(NWARPS * kWarpSize, 1) sb_fused_kernel(const _
                 if (el >= nc) break;
                 const EvalRec<T, GRAD> &R = recs[el];
                 if (R.n_entries > 0)
-                    eval_warp<T, GRAD, NCL>(P, units[R.unit], R, rowbuf, TC, tab, lane, res + (size_t)el * NRES);
+                    eval_warp<T, GRAD, NCL>(P, units[R.unit], R, rowbuf_s, TC, tab, lane, res + (size_t)el * NRES);
             }
             __syncthreads();
             // ---- epilogue: results out (coalesced within a unit), chi^2 terms in place (a7)
