@@ -52,6 +52,17 @@ typedef struct sb_bands sb_bands; /* opaque: device-resident band tables, folded
 
 typedef enum { SB_F32 = 0, SB_F64 = 1 } sb_dtype;
 
+/* Formulation bits, OR-ed into sb_batch.dtype (optional; 0 = the library picks the fastest that
+ * applies).  Both formulations compute the same sums for every evaluation; they differ in what is
+ * shared between evaluations (G_geom / G_col):
+ *   SB_FORM_DIRECT   one warp per evaluation, geometry and colour factor recomputed per evaluation
+ *                    (G = 1); any band grid, fp32 or fp64, forward or gradient.
+ *   SB_FORM_GROUPED  the observations of a unit that share a band are integrated together, sharing
+ *                    the rest-frame geometry and the colour factor; fp32 forward calls with uniform
+ *                    band grids only -- a call that demands it where it does not apply returns
+ *                    SB_ELIMIT. */
+enum { SB_FORM_DIRECT = 0x100, SB_FORM_GROUPED = 0x200 };
+
 typedef enum {
     SB_OK = 0,
     SB_EINVAL = -1, /* NULL pointer, bad count, non-uniform / non-increasing grid, non-finite table */
@@ -87,7 +98,8 @@ void sb_free_bands(sb_bands *b); /* NULL is allowed */
 /* One batch of evaluations.  Every pointer is a DEVICE pointer owned by the caller.
  * "unit" u = s*n_samples + k is one (supernova, parameter sample). */
 typedef struct {
-    int32_t dtype;             /* sb_dtype of time, zp, z, x0, x1, c, t0 and of all outputs */
+    int32_t dtype;             /* sb_dtype of time, zp, z, x0, x1, c, t0 and of all outputs,
+                                  optionally OR-ed with one SB_FORM_* bit */
     int32_t n_sn;              /* supernovae, >= 0 */
     int32_t n_samples;         /* parameter samples per supernova, >= 1 */
     int32_t n_obs_total;       /* = obs_offset[n_sn] (host copy, so no sync is needed) */

@@ -8,6 +8,8 @@ a missing GPU makes every compute call raise.
 from .api import (  # noqa: F401
     SB_F32,
     SB_F64,
+    SB_FORM_DIRECT,
+    SB_FORM_GROUPED,
     Bands,
     Model,
     SaltbandError,

@@ -12,6 +12,7 @@ from typing import Optional
 import numpy as np
 
 SB_F32, SB_F64 = 0, 1
+SB_FORM_DIRECT, SB_FORM_GROUPED = 0x100, 0x200  # optional formulation bits OR-ed into dtype
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "libsaltband.so")
@@ -177,7 +178,7 @@ def _batch(dtype: int, n_sn: int, n_samples: int, obs_offset, time, band, zp, z,
            n_obs_total: int):
     import torch
 
-    ft = torch.float32 if dtype == SB_F32 else torch.float64
+    ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
     n_units = n_sn * n_samples
     return _Batch(
         dtype, n_sn, n_samples, n_obs_total,
@@ -199,7 +200,7 @@ def sb_bandflux(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples:
     """include/saltband.h: sb_bandflux.  out_flux: [n_obs_total*n_samples] CUDA tensor (written)."""
     import torch
 
-    ft = torch.float32 if dtype == SB_F32 else torch.float64
+    ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
     bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total)
     rc = _load().sb_bandflux(model._h, bands._h, C.byref(bt), _ptr(out_flux, ft, n_obs_total * n_samples, "out_flux"),
                              _stream())
@@ -211,7 +212,7 @@ def sb_chi2(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int
     """include/saltband.h: sb_chi2.  out_chi2: [n_sn*n_samples]; out_flux optional."""
     import torch
 
-    ft = torch.float32 if dtype == SB_F32 else torch.float64
+    ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
     bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total)
     rc = _load().sb_chi2(model._h, bands._h, C.byref(bt), _ptr(flux, ft, n_obs_total, "flux"),
                          _ptr(fluxerr, ft, n_obs_total, "fluxerr"),
@@ -226,7 +227,7 @@ def sb_bandflux_grad(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_sam
     """include/saltband.h: sb_bandflux_grad.  Gradient order: (x0, x1, c, t0)."""
     import torch
 
-    ft = torch.float32 if dtype == SB_F32 else torch.float64
+    ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
     bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total)
     n_ev, n_units = n_obs_total * n_samples, n_sn * n_samples
     rc = _load().sb_bandflux_grad(

@@ -9,6 +9,7 @@
 
 #include "sb_internal.h"
 #include "sb_kernels.cuh"
+#include "sb_hoist.cuh"
 
 namespace {
 
@@ -149,6 +150,17 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
         sb_free_model(h);
         return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
     }
+    if (n_wave + 34 <= SBH_LDN && n_phase >= 4) { // interleaved {M0, M1} table of the band-grouped kernel
+        std::vector<float2> t01((size_t)n_phase * SBH_LDN, make_float2(0.f, 0.f));
+        for (int k = 0; k < n_phase; ++k)
+            for (int l = 0; l < n_wave; ++l)
+                t01[(size_t)k * SBH_LDN + SBH_PAD_L + l] =
+                    make_float2((float)m0[(size_t)k * n_wave + l], (float)m1[(size_t)k * n_wave + l]);
+        if (!upload(&h->m01_f32, t01)) {
+            sb_free_model(h);
+            return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+        }
+    }
     *out = h;
     return SB_OK;
 }
@@ -160,6 +172,7 @@ void sb_free_model(sb_model *m)
     cudaFree(m->m1_f32);
     cudaFree(m->m0_f64);
     cudaFree(m->m1_f64);
+    cudaFree(m->m01_f32);
     delete m;
 }
 
@@ -210,6 +223,17 @@ int sb_load_bandpasses(int32_t n_bands, const int64_t *offset, const double *wav
         h->h_zpab[b] = zp;
         zpab_inv[b] = 1.0 / zp;
     }
+    // uniform band grids (all of them) enable the band-grouped kernel: lam_j = lam_first + j h_b
+    std::vector<double> hstep(n_bands);
+    std::vector<float> w_f(w.begin(), w.end());
+    h->all_uniform = 1;
+    for (int b = 0; b < n_bands; ++b) {
+        const int64_t lo = offset[b], n = offset[b + 1] - lo;
+        const double *lam = wave + lo;
+        hstep[b] = (lam[n - 1] - lam[0]) / (double)(n - 1);
+        for (int64_t j = 0; j < n; ++j)
+            if (std::fabs(lam[j] - (lam[0] + (double)j * hstep[b])) > 1e-9 * lam[j]) h->all_uniform = 0;
+    }
     std::vector<float2> tab_f((size_t)total);
     std::vector<double2> tab_d((size_t)total);
     for (int64_t i = 0; i < total; ++i) {
@@ -218,7 +242,8 @@ int sb_load_bandpasses(int32_t n_bands, const int64_t *offset, const double *wav
     }
     cudaGetDevice(&h->device);
     if (!upload(&h->d_off, off) || !upload(&h->d_lam_first, lam_first) || !upload(&h->d_zpab_inv, zpab_inv) ||
-        !upload(&h->d_tab_f64, tab_d) || !upload(&h->d_tab_f32, tab_f)) {
+        !upload(&h->d_tab_f64, tab_d) || !upload(&h->d_tab_f32, tab_f) || !upload(&h->d_w_f32, w_f) ||
+        !upload(&h->d_dlam_f64, dlam) || !upload(&h->d_h, hstep)) {
         sb_free_bands(h);
         return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
     }
@@ -234,6 +259,9 @@ void sb_free_bands(sb_bands *b)
     cudaFree(b->d_zpab_inv);
     cudaFree(b->d_tab_f32);
     cudaFree(b->d_tab_f64);
+    cudaFree(b->d_w_f32);
+    cudaFree(b->d_dlam_f64);
+    cudaFree(b->d_h);
     free(b->h_zpab);
     delete b;
 }
@@ -309,11 +337,90 @@ int launch_typed(SbKParams &kp, const sb_bands *b, int n_obs_total, cudaStream_t
     return launch_inst<T, GRAD, SB_MAX_CL, false, NWARPS>(kp, smem, grid, st);
 }
 
-int run(const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux, const void *fluxerr,
+// Band-grouped kernel (sb_hoist.cuh): fp32 forward, uniform band grids.  Returns 1 when it is not
+// applicable (the caller then runs the per-evaluation kernel), SB_OK or an error otherwise.
+int launch_hoisted(const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux, const void *fluxerr,
+                   void *out_flux, void *out_chi2, cudaStream_t st)
+{
+    constexpr int NCL = 5;
+    if (!m->m01_f32 || !b->all_uniform || m->prm.n_cl > NCL || b->n_bands > 64) return 1;
+    const int smem_max = device_smem_optin();
+    const int n_sm = device_sm_count();
+    if (smem_max <= 0 || n_sm <= 0) return SB_ECUDA;
+    const long long n_units = (long long)bt->n_sn * bt->n_samples;
+    const double mean_obs = bt->n_sn > 0 ? (double)bt->n_obs_total / (double)bt->n_sn : 1.0;
+    // units per group: enough groups for every SM (>= 4 per CTA), at most kMaxSeg, about <= cap observations
+    const int cap = 4096;
+    long long g = n_units / ((long long)n_sm * 4);
+    if (g > sbh::kMaxSeg) g = sbh::kMaxSeg;
+    if ((double)g * mean_obs > (double)cap) g = (long long)((double)cap / mean_obs);
+    if (g < 1) g = 1;
+    const sbh::HSmem L(b->n_total, cap);
+    if (L.total > (size_t)smem_max || L.total > 100 * 1024) return 1;
+
+    unsigned char *ws = nullptr; // workspace: group counter + z-order permutation (stream-ordered)
+    const size_t ws_bytes = 256 + sizeof(int32_t) * (size_t)bt->n_sn;
+    if (!cuda_ok(cudaMallocAsync((void **)&ws, ws_bytes, st))) return SB_ECUDA;
+    SbHParams hp;
+    memset(&hp, 0, sizeof(hp));
+    hp.mp = m->prm;
+    hp.m01 = m->m01_f32;
+    hp.n_bands = b->n_bands;
+    hp.n_band_total = b->n_total;
+    hp.band_off = b->d_off;
+    hp.band_lam_first = b->d_lam_first;
+    hp.band_zpab_inv = b->d_zpab_inv;
+    hp.band_h = b->d_h;
+    hp.band_dlam = b->d_dlam_f64;
+    hp.band_w = b->d_w_f32;
+    hp.n_sn = bt->n_sn;
+    hp.n_samples = bt->n_samples;
+    hp.obs_offset = bt->obs_offset;
+    hp.time = (const float *)bt->time;
+    hp.zp = (const float *)bt->zp;
+    hp.z = (const float *)bt->z;
+    hp.x0 = (const float *)bt->x0;
+    hp.x1 = (const float *)bt->x1;
+    hp.c = (const float *)bt->c;
+    hp.t0 = (const float *)bt->t0;
+    hp.band = bt->band;
+    hp.flux = (const float *)flux;
+    hp.fluxerr = (const float *)fluxerr;
+    hp.out_flux = (float *)out_flux;
+    hp.out_chi2 = (float *)out_chi2;
+    hp.counter = reinterpret_cast<unsigned int *>(ws);
+    hp.perm = reinterpret_cast<const int32_t *>(ws + 256);
+    hp.group_units = (int)g;
+    hp.cap = cap;
+    int rc = SB_OK;
+    sbh::sb_zorder_kernel<<<1, 1024, 0, st>>>(hp.z, hp.n_sn, reinterpret_cast<int32_t *>(ws + 256), hp.counter);
+    if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
+    if (rc == SB_OK) {
+        tl_launches += 1;
+        auto kern = sbh::sb_hoist_kernel<NCL, SBH_LDN>;
+        const long long n_groups = (n_units + g - 1) / g;
+        const int grid = (int)(n_groups < (long long)n_sm ? n_groups : (long long)n_sm);
+        if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total))) rc = SB_ECUDA;
+        if (rc == SB_OK) {
+            kern<<<grid, sbh::kThreads, L.total, st>>>(hp);
+            if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
+            else tl_launches += 1;
+        }
+    }
+    if (!cuda_ok(cudaFreeAsync(ws, st)) && rc == SB_OK) rc = SB_ECUDA;
+    return rc;
+}
+
+int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void *flux, const void *fluxerr,
         void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2, void *stream, bool grad)
 {
     tl_launches = 0;
-    if (!m || !b || !bt) return SB_EINVAL;
+    if (!m || !b || !bt_in) return SB_EINVAL;
+    sb_batch batch = *bt_in; // split the formulation bits off the dtype
+    const int32_t form = batch.dtype & (SB_FORM_DIRECT | SB_FORM_GROUPED);
+    batch.dtype &= ~(SB_FORM_DIRECT | SB_FORM_GROUPED);
+    const sb_batch *bt = &batch;
+    if (form == (SB_FORM_DIRECT | SB_FORM_GROUPED)) return SB_EINVAL;
     if (bt->dtype != SB_F32 && bt->dtype != SB_F64) return SB_EINVAL;
     if (bt->n_sn < 0 || bt->n_samples < 1 || bt->n_obs_total < 0) return SB_EINVAL;
     if ((out_chi2 || out_dchi2) && (!flux || !fluxerr)) return SB_EINVAL;
@@ -353,6 +460,11 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *fl
     kp.out_chi2 = out_chi2;
     kp.out_dchi2 = out_dchi2;
     cudaStream_t st = (cudaStream_t)stream;
+    if (f32 && !grad && form != SB_FORM_DIRECT && bt->n_obs_total > 0) {
+        const int rc = launch_hoisted(m, b, bt, flux, fluxerr, out_flux, out_chi2, st);
+        if (rc != 1) return rc;
+    }
+    if (form == SB_FORM_GROUPED) return SB_ELIMIT; // the grouped formulation was demanded but does not apply
     if (f32) {
         if (grad) return launch_typed<float, true, 8>(kp, b, bt->n_obs_total, st);
         return launch_typed<float, false, 16>(kp, b, bt->n_obs_total, st);

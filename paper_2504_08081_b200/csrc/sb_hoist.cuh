@@ -1,0 +1,579 @@
+// sb_hoist.cuh -- the band-grouped ("hoisted") fused SALT3 band-flux kernel (sm_100a), fp32 forward.
+//
+// Same arithmetic per evaluation as sb_kernels.cuh, but the work
+// item is one (unit, band): the observations of a unit that share a band share the rest-frame
+// wavelength geometry and the colour factor (they depend on z, c and the band only -- PAPER.md:19-23,
+// 38-43), so those are computed once per band sample and reused by up to kOB observations
+// (G_geom = G_col = observations per (unit, band), up to 8 per pass).
+//
+// Mapping.  Persistent CTAs (one per SM, 16 warps) pull GROUPS of units that are neighbours in
+// redshift (the z-order permutation is built by sb_zorder_kernel in the same call), and inside a group
+// warps pull ITEMS (band, unit) in band-major order, so that at any time all warps of an SM read the
+// same ~(71 rows x 240 columns) window of the M0/M1 table: it stays in L1 and HBM/L2 see only the
+// per-observation records.  Inside an item a LANE owns one model cell per pass (29 cells per pass):
+//   a2  the lane loads its node of the 4 phase rows of {M0, M1} (one coalesced LDG.64 per row of the
+//       interleaved table), collapses them with the observation's phase weights (8 FFMA), gets the 3
+//       neighbouring nodes by warp shuffles and converts them to the cell's cubic in tau in [0,1)
+//       (Catmull-Rom = Keys a = -1/2; linear in the border cells, reading G2).  The coefficients of up
+//       to 8 observations stay in REGISTERS: no row buffer, no gathers.
+//   a1/a3/a4  the lane walks the 2-5 band samples that fall into its cell: tau and the reduced
+//       wavelength advance by constant steps, the colour factor exp(c CL) (one ex2) times the folded
+//       weight W_j (one LDS) is computed once and shared by the observations;
+//   a5  per observation 3 FFMA (Horner) + 1 FFMA (accumulate); warp butterfly at the end;
+//   a6/a7  epilogue per unit in fp64: zero point, flux store (coalesced), chi^2 in a fixed order.
+// Requirements (checked by the host, otherwise sb_kernels.cuh runs): fp32, forward only, every band
+// grid uniform, n_phase >= 4, n_wave + 34 <= LDN, n_cl <= NCL, band weights fit in shared memory.
+#pragma once
+#include "sb_internal.h"
+#include "sb_kernels.cuh"
+
+namespace sbh {
+
+constexpr int kWarps = 16;
+constexpr int kThreads = kWarps * 32;
+constexpr int kMaxSeg = 32;  // segments (units) per round
+constexpr int kOB = 8;       // observations sharing one pass
+constexpr int kPass = 29;    // cells per pass: lanes 1..29 own a cell, lanes 0, 30, 31 carry the halo
+constexpr int kZBins = 2048; // redshift bins of the z-order permutation
+
+// One segment = a contiguous run of observations of one unit (a whole unit unless it exceeds the
+// round capacity); lives in shared memory for the duration of a round.
+struct HSeg {
+    double x0, t0, opz, inv_opz, cc;
+    long long out_base;  // out_flux index of the segment's first observation
+    int32_t unit;        // global unit index (supernova * n_samples + sample)
+    int32_t sn;
+    int32_t o_lo;        // first global observation index of the segment
+    int32_t n;           // observations in the segment
+    int32_t e_begin;     // first slot in the round's result array
+    int32_t first, last; // first / last segment of its unit
+    float x1;
+    float cl[SB_MAX_CL]; // colour-law coefficients times c*log2(e)
+    float s_lo, s_hi;    // continuation slopes, same scaling
+    float p_lo, p_hi;    // polynomial value at the range ends, same scaling
+};
+
+struct HUnitTmp {
+    int32_t unit, sn, o_lo, n;
+};
+
+struct WScratch {
+    float wts[kOB][8];   // per observation: phase weights on M0 [0..3] and on M1 (times x1) [4..7]
+    int32_t rowoff[kOB]; // byte offset of the first of the 4 phase rows
+    int32_t slot[kOB];   // result slot of the observation
+    int32_t queue[64];   // observations of the item waiting for a chunk
+};
+
+struct HSmem {
+    size_t w, res, segs, utmp, scr, misc, total;
+    __host__ __device__ HSmem(int n_band_total, int cap)
+    {
+        size_t o = 0;
+        w = o; o += (size_t)((n_band_total + 3) & ~3) * sizeof(float);
+        res = o; o += (size_t)((cap + 3) & ~3) * sizeof(float);
+        o = (o + 15) & ~(size_t)15;
+        segs = o; o += (size_t)kMaxSeg * sizeof(HSeg);
+        utmp = o; o += (size_t)kMaxSeg * sizeof(HUnitTmp);
+        scr = o; o += (size_t)kWarps * sizeof(WScratch);
+        misc = o; o += 64;
+        total = o;
+    }
+};
+
+// ---- z-order permutation (counting sort of the supernovae by 1/(1+z)) + group counter reset -------
+// One CTA.  Order inside a bin is arbitrary (atomics): results do not depend on it, each unit is
+// computed independently of its neighbours.
+__global__ void __launch_bounds__(1024, 1) sb_zorder_kernel(const float *__restrict__ z, int n_sn, int32_t *perm,
+                                                            unsigned int *counter)
+{
+    __shared__ int hist[kZBins];
+    __shared__ int lane_tot[32];
+    const int tid = threadIdx.x;
+    if (tid == 0) *counter = 0u;
+    for (int i = tid; i < kZBins; i += blockDim.x) hist[i] = 0;
+    __syncthreads();
+    auto bin_of = [&](int i) {
+        const float key = 1.0f / (1.0f + __ldg(z + i)); // window position scales with 1/(1+z)
+        int b = (int)(key * (float)kZBins);
+        if (!(key > 0.0f)) b = 0;
+        return min(max(b, 0), kZBins - 1);
+    };
+    for (int i = tid; i < n_sn; i += blockDim.x) atomicAdd(&hist[bin_of(i)], 1);
+    __syncthreads();
+    if (tid < 32) { // exclusive scan: 64 bins per lane, then across lanes
+        constexpr int PER = kZBins / 32;
+        int s = 0;
+        for (int k = 0; k < PER; ++k) s += hist[tid * PER + k];
+        int incl = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (tid >= o) incl += v;
+        }
+        int run = incl - s;
+        for (int k = 0; k < PER; ++k) {
+            const int c = hist[tid * PER + k];
+            hist[tid * PER + k] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < n_sn; i += blockDim.x) perm[atomicAdd(&hist[bin_of(i)], 1)] = i;
+}
+
+// ---- colour law of one item: exponent argument (log2 units) as a function of the reduced wavelength
+template <int NCL> struct HColour {
+    float a[NCL];
+    float r_lo, r_hi, s_lo, s_hi;
+    float lin_a, lin_b; // CM_LINEAR: arg = lin_a + lin_b * r
+    template <int CM> __device__ __forceinline__ float arg(float r) const
+    {
+        if constexpr (CM == sb::CM_LINEAR) {
+            return __fmaf_rn(r, lin_b, lin_a);
+        } else if constexpr (CM == sb::CM_INSIDE) {
+            float p = a[NCL - 1];
+#pragma unroll
+            for (int q = NCL - 2; q >= 0; --q) p = __fmaf_rn(p, r, a[q]);
+            return p;
+        } else {
+            const float rc = fminf(fmaxf(r, r_lo), r_hi);
+            const float d = r - rc;
+            const float slope = d > 0.0f ? s_hi : s_lo;
+            float p = a[NCL - 1];
+#pragma unroll
+            for (int q = NCL - 2; q >= 0; --q) p = __fmaf_rn(p, rc, a[q]);
+            return __fmaf_rn(slope, d, p);
+        }
+    }
+};
+
+// Geometry of one item (unit, band): warp-uniform values.
+struct HGeo {
+    int32_t n_in;     // in-range band samples
+    int32_t ncell;    // model cells spanned
+    int32_t g_first;  // first cell
+    int32_t wbase;    // index of the first in-range sample in the staged weight table
+    int32_t cmode;
+    float c0;         // u of the first in-range sample minus g_first
+    float ha_hi, ha_lo, inv_ha; // cells per band sample (split in two floats), its inverse
+    float hal, r_first;         // reduced-wavelength step per sample, value at the first sample
+};
+
+__device__ __forceinline__ float4 lds_f4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+
+// One chunk: NOB observations of the item integrated together.
+template <int NOB, int NCL, int LDN>
+__device__ __forceinline__ void run_chunk(const SbHParams &P, const HSeg &S, const HGeo &G, const HColour<NCL> &col,
+                                          WScratch &W, const float *__restrict__ s_w, float *__restrict__ res,
+                                          int lane)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    constexpr int ROWB = LDN * (int)sizeof(float2); // bytes per phase row (compile time: immediate offsets)
+    const SbModelParams &mp = P.mp;
+    const int nW = mp.n_wave, nP = mp.n_phase;
+
+    // ---- a1/a2 per observation (lane o < NOB): phase, phase weights, row offset
+    if (lane < NOB) {
+        const int oi = W.queue[lane];
+        const int o = S.o_lo + oi;
+        const double p = ((double)__ldg(P.time + o) - S.t0) * S.inv_opz;
+        const double up = (p - mp.p0) / mp.dp;
+        float w[4] = {0.f, 0.f, 0.f, 0.f};
+        int kp = 0;
+        if ((up >= 0.0) && (up <= (double)(nP - 1))) { // outside the phase grid: zero flux (G3)
+            kp = min((int)floor(up), nP - 2);
+            const double tau = up - (double)kp;
+            double wv[4], wd[4];
+            sb::phase_weights(tau, (kp == 0) || (kp == nP - 2), 1.0, wv, wd);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) w[k] = (float)wv[k];
+        }
+        const int rb = min(max(kp - 1, 0), nP - 4); // rows rb..rb+3 are loaded
+        const int shift = (kp - 1) - rb;            // -1 at the first cell, +1 at the last, else 0
+        float ws[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int src = k - shift;               // slot k holds the weight of row rb + k
+            float v = 0.f;
+            if (src == 0) v = w[0];
+            if (src == 1) v = w[1];
+            if (src == 2) v = w[2];
+            if (src == 3) v = w[3];
+            ws[k] = (src >= 0 && src <= 3) ? v : 0.f;
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            W.wts[lane][k] = ws[k];
+            W.wts[lane][4 + k] = ws[k] * S.x1;
+        }
+        W.rowoff[lane] = rb * ROWB;
+        W.slot[lane] = S.e_begin + oi;
+    }
+    __syncwarp();
+
+    int rowoff[NOB];
+#pragma unroll
+    for (int o = 0; o < NOB; ++o) rowoff[o] = W.rowoff[o];
+    float acc[NOB];
+#pragma unroll
+    for (int o = 0; o < NOB; ++o) acc[o] = 0.f;
+
+    // column pointer of this lane for pass 0: node (g_first - 1 + lane)
+    const char *colp = reinterpret_cast<const char *>(P.m01) + (size_t)(G.g_first - 1 + SBH_PAD_L + lane) * sizeof(float2);
+    const int n_pass = (G.ncell + kPass - 1) / kPass;
+    const float c0 = G.c0, inv_ha = G.inv_ha, ha_hi = G.ha_hi, ha_lo = G.ha_lo, hal = G.hal, r_first = G.r_first;
+    const int n_in = G.n_in, ncell = G.ncell;
+
+    for (int q = 0; q < n_pass; ++q) {
+        // ---- a2: collapse the phase rows and convert to per-cell cubic coefficients (registers)
+        const int gq = kPass * q + lane - 1; // this lane's cell relative to g_first
+        const int g = G.g_first + gq;
+        const bool special = (G.g_first + kPass * q <= 0) || (G.g_first + kPass * q + kPass >= nW - 2); // warp-uniform
+        const bool border = special && ((g <= 0) || (g >= nW - 2));
+        float cf[NOB][4];
+#pragma unroll
+        for (int o = 0; o < NOB; ++o) {
+            const char *p = colp + rowoff[o];
+            const float2 v0 = __ldg(reinterpret_cast<const float2 *>(p));
+            const float2 v1 = __ldg(reinterpret_cast<const float2 *>(p + ROWB));
+            const float2 v2 = __ldg(reinterpret_cast<const float2 *>(p + 2 * ROWB));
+            const float2 v3 = __ldg(reinterpret_cast<const float2 *>(p + 3 * ROWB));
+            const float4 wa = lds_f4(&W.wts[o][0]);
+            const float4 wb = lds_f4(&W.wts[o][4]);
+            float node = wa.x * v0.x;
+            node = __fmaf_rn(wa.y, v1.x, node);
+            node = __fmaf_rn(wa.z, v2.x, node);
+            node = __fmaf_rn(wa.w, v3.x, node);
+            node = __fmaf_rn(wb.x, v0.y, node);
+            node = __fmaf_rn(wb.y, v1.y, node);
+            node = __fmaf_rn(wb.z, v2.y, node);
+            node = __fmaf_rn(wb.w, v3.y, node);
+            const float rm = __shfl_up_sync(FULL, node, 1);
+            const float r1 = __shfl_down_sync(FULL, node, 1);
+            const float r2 = __shfl_down_sync(FULL, node, 2);
+            // Catmull-Rom in tau: c0 = r0, c1 = (r1 - rm)/2, c3 = 1.5 (r0 - r1) + (r2 - rm)/2,
+            // c2 = (r1 - r0) - c1 - c3
+            const float d10 = node - r1;
+            float c1 = 0.5f * (r1 - rm);
+            float c3 = __fmaf_rn(1.5f, d10, 0.5f * (r2 - rm));
+            float c2 = (-d10 - c1) - c3;
+            if (border) { // linear border cell (G2)
+                c1 = -d10;
+                c2 = 0.f;
+                c3 = 0.f;
+            }
+            cf[o][0] = node;
+            cf[o][1] = c1;
+            cf[o][2] = c2;
+            cf[o][3] = c3;
+        }
+        colp += kPass * sizeof(float2);
+
+        // ---- a1: the band samples of this lane's cell: j' in [js, je)
+        const bool valid = (lane >= 1) && (lane <= kPass) && (gq < ncell);
+        const float gf = (float)gq;
+        int js = (int)ceilf((gf - c0) * inv_ha);
+        js = min(max(js, 0), n_in);
+        if (gq <= 0) js = 0;
+        int je = __shfl_down_sync(FULL, js, 1);
+        if (gq >= ncell - 1) je = n_in;
+        const int cnt = valid ? max(je - js, 0) : 0;
+        const float jsf = (float)js;
+        float tau = __fmaf_rn(jsf, ha_lo, __fmaf_rn(jsf, ha_hi, -gf)) + c0; // u_js - g
+        float r = __fmaf_rn(jsf, hal, r_first);
+        const float *wp = s_w + (G.wbase + js);
+        const int km = __reduce_max_sync(FULL, cnt);
+
+        // ---- a3/a4/a5: samples
+        auto samples = [&](auto cm_tag) {
+            constexpr int CM = decltype(cm_tag)::value;
+            for (int k = 0; k < km; ++k) {
+                float w = 0.f;
+                if (k < cnt) w = wp[k];
+                const float ew = sb::exp_scaled(col.template arg<CM>(r)) * w;
+#pragma unroll
+                for (int o = 0; o < NOB; ++o) {
+                    const float val = __fmaf_rn(__fmaf_rn(__fmaf_rn(cf[o][3], tau, cf[o][2]), tau, cf[o][1]), tau, cf[o][0]);
+                    acc[o] = __fmaf_rn(ew, val, acc[o]);
+                }
+                tau += ha_hi;
+                r += hal;
+            }
+        };
+        if (G.cmode == sb::CM_INSIDE) samples(std::integral_constant<int, sb::CM_INSIDE>{});
+        else if (G.cmode == sb::CM_LINEAR) samples(std::integral_constant<int, sb::CM_LINEAR>{});
+        else samples(std::integral_constant<int, sb::CM_GENERIC>{});
+    }
+    // ---- a5: wavelength integral (butterfly); raw integrals to the round's result array
+#pragma unroll
+    for (int o = 0; o < NOB; ++o) acc[o] = sb::warp_sum(acc[o]);
+    if (lane == 0) {
+#pragma unroll
+        for (int o = 0; o < NOB; ++o) res[W.slot[o]] = acc[o];
+    }
+    __syncwarp();
+}
+
+template <int NCL, int LDN>
+__device__ __forceinline__ void run_chunk_n(int n, const SbHParams &P, const HSeg &S, const HGeo &G,
+                                            const HColour<NCL> &col, WScratch &W, const float *s_w, float *res, int lane)
+{
+    switch (n) {
+    case 1: run_chunk<1, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
+    case 2: run_chunk<2, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
+    case 3: run_chunk<3, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
+    case 4: run_chunk<4, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
+    case 5: run_chunk<5, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
+    case 6: run_chunk<6, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
+    case 7: run_chunk<7, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
+    default: run_chunk<8, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
+    }
+}
+
+// One item: the observations of segment S in band b.
+template <int NCL, int LDN>
+__device__ __forceinline__ void run_item(const SbHParams &P, const HSeg &S, int b, WScratch &W, const float *s_w,
+                                         float *res, int lane)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    const SbModelParams &mp = P.mp;
+    const int nW = mp.n_wave;
+    // ---- geometry of (z, band): in-range samples decided in fp64 (G9), window of model cells
+    const int boff = __ldg(P.band_off + b);
+    const int nb = __ldg(P.band_off + b + 1) - boff;
+    const double lam_first = __ldg(P.band_lam_first + b);
+    const double h = __ldg(P.band_h + b);
+    const double opz = S.opz, inv_opz = S.inv_opz;
+    const double dl_lo = mp.l0 * opz - lam_first;
+    const double dl_hi = (mp.l0 + (double)(nW - 1) * mp.dl) * opz - lam_first;
+    const double *__restrict__ dlam = P.band_dlam + boff;
+    int j_lo = (int)fmin(fmax(ceil(dl_lo / h), 0.0), (double)nb);
+    while (j_lo > 0 && __ldg(dlam + j_lo - 1) >= dl_lo) --j_lo;
+    while (j_lo < nb && __ldg(dlam + j_lo) < dl_lo) ++j_lo;
+    int j_hi = (int)fmin(fmax(floor(dl_hi / h) + 1.0, 0.0), (double)nb);
+    while (j_hi < nb && __ldg(dlam + j_hi) <= dl_hi) ++j_hi;
+    while (j_hi > 0 && __ldg(dlam + j_hi - 1) > dl_hi) --j_hi;
+    if (j_lo >= j_hi) return; // band entirely outside the model grid: results stay 0 (G3)
+
+    HGeo G;
+    const double a_d = inv_opz / mp.dl;                        // cells per observer-frame Angstrom
+    const double ub = (lam_first * inv_opz - mp.l0) / mp.dl;   // u of dlam = 0
+    const double ha = h * a_d;                                 // cells per band sample
+    const double u_lo = (double)j_lo * ha + ub;
+    const double u_hi = (double)(j_hi - 1) * ha + ub;
+    const int g_first = min(max((int)floor(u_lo), 0), nW - 2);
+    const int g_last = min(max((int)floor(u_hi), 0), nW - 2);
+    G.n_in = j_hi - j_lo;
+    G.g_first = g_first;
+    G.ncell = g_last - g_first + 1;
+    G.wbase = boff + j_lo;
+    G.c0 = (float)(u_lo - (double)g_first);
+    G.ha_hi = (float)ha;
+    G.ha_lo = (float)(ha - (double)G.ha_hi);
+    G.inv_ha = (float)(1.0 / ha);
+    const double al_d = inv_opz * mp.cl_inv_span;
+    const double be_d = (lam_first * inv_opz - mp.cl_b) * mp.cl_inv_span;
+    const double hal = h * al_d;
+    const double r_a = (double)j_lo * hal + be_d, r_b = (double)(j_hi - 1) * hal + be_d;
+    G.hal = (float)hal;
+    G.r_first = (float)r_a;
+    // ---- a3: colour-law mode of the item (reduced wavelength is monotone in j)
+    HColour<NCL> col;
+#pragma unroll
+    for (int q = 0; q < NCL; ++q) col.a[q] = S.cl[q];
+    col.r_lo = (float)mp.r_lo;
+    col.r_hi = (float)mp.r_hi;
+    col.s_lo = S.s_lo;
+    col.s_hi = S.s_hi;
+    col.lin_a = 0.f;
+    col.lin_b = 0.f;
+    {
+        const double r_min = fmin(r_a, r_b), r_max = fmax(r_a, r_b);
+        const double margin = 1e-4;
+        int cmode = sb::CM_GENERIC;
+        if (r_min >= mp.r_lo + margin && r_max <= mp.r_hi - margin) {
+            cmode = sb::CM_INSIDE;
+        } else if (r_min >= mp.r_hi + margin) { // arg = p_hi + s_hi (r - r_hi)
+            cmode = sb::CM_LINEAR;
+            col.lin_b = S.s_hi;
+            col.lin_a = (float)((double)S.p_hi - (double)S.s_hi * mp.r_hi);
+        } else if (r_max <= mp.r_lo - margin) {
+            cmode = sb::CM_LINEAR;
+            col.lin_b = S.s_lo;
+            col.lin_a = (float)((double)S.p_lo - (double)S.s_lo * mp.r_lo);
+        }
+        G.cmode = cmode;
+    }
+
+    // ---- the observations of this band, in order, in chunks of kOB
+    int qn = 0;
+    for (int base = 0; base < S.n; base += 32) {
+        const int oi = base + lane;
+        bool match = false;
+        if (oi < S.n) match = __ldg(P.band + S.o_lo + oi) == b;
+        const unsigned m = __ballot_sync(FULL, match);
+        if (match) W.queue[qn + __popc(m & ((1u << lane) - 1u))] = oi;
+        qn += __popc(m);
+        __syncwarp();
+        while (qn >= kOB) {
+            run_chunk<kOB, NCL, LDN>(P, S, G, col, W, s_w, res, lane);
+            const int rest = qn - kOB; // <= 31
+            int v = 0;
+            if (lane < rest) v = W.queue[kOB + lane];
+            __syncwarp();
+            if (lane < rest) W.queue[lane] = v;
+            __syncwarp();
+            qn = rest;
+        }
+    }
+    if (qn > 0) run_chunk_n<NCL, LDN>(qn, P, S, G, col, W, s_w, res, lane);
+}
+
+// ---- the kernel ---------------------------------------------------------------------------------
+template <int NCL, int LDN>
+__global__ void __launch_bounds__(kThreads, 1) sb_hoist_kernel(const __grid_constant__ SbHParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const SbModelParams &mp = P.mp;
+    const HSmem L(P.n_band_total, P.cap);
+    float *s_w = reinterpret_cast<float *>(smem_raw + L.w);
+    float *res = reinterpret_cast<float *>(smem_raw + L.res);
+    HSeg *segs = reinterpret_cast<HSeg *>(smem_raw + L.segs);
+    HUnitTmp *utmp = reinterpret_cast<HUnitTmp *>(smem_raw + L.utmp);
+    WScratch *scr = reinterpret_cast<WScratch *>(smem_raw + L.scr);
+    int *misc = reinterpret_cast<int *>(smem_raw + L.misc);       // [0] group, [1] n_seg, [2] n_ev, [3] next unit, [4] next offset, [5] item counter
+    double *carry = reinterpret_cast<double *>(smem_raw + L.misc + 32); // chi^2 of a unit split over rounds
+
+    for (int i = tid; i < P.n_band_total; i += kThreads) s_w[i] = __ldg(P.band_w + i);
+    const long long n_units = (long long)P.n_sn * P.n_samples;
+    const int G = P.group_units, CAP = P.cap;
+    const long long n_groups = (n_units + G - 1) / G;
+    const bool want_chi = P.out_chi2 != nullptr;
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) misc[0] = (int)atomicAdd(P.counter, 1u);
+        __syncthreads();
+        const long long group = (long long)(unsigned)misc[0];
+        if (group >= n_groups) break;
+        const long long pos0 = group * G;
+        const int npos = (int)min((long long)G, n_units - pos0);
+        if (tid < npos) { // unit -> supernova (z-ordered), observation range
+            const long long pos = pos0 + tid;
+            const int si = (int)(pos / P.n_samples);
+            const int ks = (int)(pos - (long long)si * P.n_samples);
+            const int sn = P.perm ? __ldg(P.perm + si) : si;
+            HUnitTmp t;
+            t.sn = sn;
+            t.unit = sn * P.n_samples + ks;
+            t.o_lo = __ldg(P.obs_offset + sn);
+            t.n = __ldg(P.obs_offset + sn + 1) - t.o_lo;
+            utmp[tid] = t;
+        }
+        if (tid == 0) { misc[3] = 0; misc[4] = 0; }
+        __syncthreads();
+
+        for (;;) {
+            const int cur_u = misc[3];
+            __syncthreads();
+            if (cur_u >= npos) break;
+            // ---- round: consecutive units whose observations fit the result array (a unit larger
+            // than the array is processed alone, CAP observations at a time)
+            if (tid == 0) {
+                int u = misc[3], off = misc[4], n_ev = 0, n_seg = 0;
+                while (u < npos && n_seg < kMaxSeg) {
+                    const int rem = utmp[u].n - off;
+                    HSeg &S = segs[n_seg];
+                    if (rem <= CAP - n_ev) {
+                        S.unit = u; S.o_lo = off; S.n = rem; S.e_begin = n_ev; S.first = (off == 0); S.last = 1;
+                        n_ev += rem; ++n_seg; ++u; off = 0;
+                    } else if (n_ev == 0) {
+                        S.unit = u; S.o_lo = off; S.n = CAP; S.e_begin = 0; S.first = (off == 0); S.last = 0;
+                        n_ev = CAP; ++n_seg; off += CAP;
+                        break;
+                    } else {
+                        break;
+                    }
+                }
+                misc[1] = n_seg; misc[2] = n_ev; misc[3] = u; misc[4] = off; misc[5] = 0;
+            }
+            __syncthreads();
+            const int n_seg = misc[1], n_ev = misc[2];
+            if (tid < n_seg) { // segment parameters (S.unit / S.o_lo hold group-local values until here)
+                HSeg &S = segs[tid];
+                const HUnitTmp t = utmp[S.unit];
+                const int off = S.o_lo;
+                const int ks = t.unit - t.sn * P.n_samples;
+                S.unit = t.unit;
+                S.sn = t.sn;
+                S.o_lo = t.o_lo + off;
+                S.out_base = (long long)t.o_lo * P.n_samples + (long long)ks * t.n + off;
+                const double z = (double)__ldg(P.z + t.sn);
+                const double cc = (double)__ldg(P.c + t.unit);
+                S.opz = 1.0 + z;
+                S.inv_opz = 1.0 / S.opz;
+                S.x0 = (double)__ldg(P.x0 + t.unit);
+                S.x1 = __ldg(P.x1 + t.unit);
+                S.t0 = (double)__ldg(P.t0 + t.unit);
+                S.cc = cc;
+                const double cscale = cc * 1.4426950408889634; // exponent in log2 units (ex2)
+#pragma unroll
+                for (int q = 0; q < SB_MAX_CL; ++q) S.cl[q] = (float)(mp.cl[q] * cscale);
+                S.s_lo = (float)(mp.s_lo * cscale);
+                S.s_hi = (float)(mp.s_hi * cscale);
+                S.p_lo = (float)(mp.p_lo * cscale);
+                S.p_hi = (float)(mp.p_hi * cscale);
+            }
+            for (int e = tid; e < n_ev; e += kThreads) res[e] = 0.f;
+            __syncthreads();
+
+            // ---- main: warps pull items (band-major: all warps work on the same band window)
+            const int n_items = P.n_bands * n_seg;
+            for (;;) {
+                int it = 0;
+                if (lane == 0) it = atomicAdd(&misc[5], 1);
+                it = __shfl_sync(0xffffffffu, it, 0);
+                if (it >= n_items) break;
+                const int b = it / n_seg, sg = it - b * n_seg;
+                if (segs[sg].n > 0) run_item<NCL, LDN>(P, segs[sg], b, scr[warp], s_w, res, lane);
+            }
+            __syncthreads();
+
+            // ---- epilogue: one warp per segment; a6 zero point (fp64), flux out (coalesced), a7 chi^2
+            for (int sg = warp; sg < n_seg; sg += kWarps) {
+                const HSeg &S = segs[sg];
+                double sum = 0.0;
+                for (int i = lane; i < S.n; i += 32) {
+                    const int o = S.o_lo + i;
+                    const int b = __ldg(P.band + o);
+                    double m;
+                    if ((unsigned)b >= (unsigned)P.n_bands) {
+                        m = __longlong_as_double(0x7ff8000000000000LL);
+                    } else {
+                        double sc = 1.0;
+                        if (P.zp != nullptr) sc = exp10(0.4 * (double)__ldg(P.zp + o)) * __ldg(P.band_zpab_inv + b);
+                        m = sc * S.x0 * (double)res[S.e_begin + i];
+                    }
+                    if (P.out_flux) P.out_flux[S.out_base + i] = (float)m;
+                    if (want_chi) {
+                        const double f = (double)__ldg(P.flux + o), e = (double)__ldg(P.fluxerr + o);
+                        const double qv = (f - m) / e;
+                        sum += qv * qv;
+                    }
+                }
+                if (want_chi) {
+                    sum = sb::warp_sum(sum);
+                    if (lane == 0) {
+                        const double total = (S.first ? 0.0 : *carry) + sum;
+                        if (S.last) P.out_chi2[S.unit] = (float)total;
+                        else *carry = total;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+} // namespace sbh

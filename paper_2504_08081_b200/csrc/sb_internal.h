@@ -29,10 +29,17 @@ struct SbModelParams {
     double p_lo, s_lo, p_hi, s_hi;     // polynomial value and slope at r_lo, r_hi
 };
 
+// Interleaved {M0, M1} fp32 table of the band-grouped kernel (sb_hoist.cuh): [n_phase][SBH_LDN]
+// float2, node l at column l + SBH_PAD_L, zero padded.  The row stride is a compile-time constant so
+// that the four phase rows of a cell are reached with immediate offsets from one pointer.
+#define SBH_PAD_L 2
+#define SBH_LDN 1856
+
 struct sb_model {
     SbModelParams prm;
     float *m0_f32, *m1_f32;   // [n_phase][ld], zero padded (SB_PAD_L)
     double *m0_f64, *m1_f64;  // [n_phase][ld]
+    float2 *m01_f32;          // [n_phase][SBH_LDN] or NULL when n_wave + 34 > SBH_LDN
     int device;
 };
 
@@ -45,6 +52,11 @@ struct sb_bands {
     double2 *d_tab_f64;
     double *h_zpab;        // host copy [n_bands]
     double max_span;       // max over bands of (lam_last - lam_first)
+    // band-grouped kernel (sb_hoist.cuh): only when every band grid is uniform
+    int32_t all_uniform;   // 1 when |lam_j - (lam_first + j h_b)| <= 1e-9 lam_j for every band
+    float *d_w_f32;        // [n_total] folded weights
+    double *d_dlam_f64;    // [n_total] lam_j - lam_first
+    double *d_h;           // [n_bands] uniform step h_b
     int device;
 };
 
@@ -65,4 +77,24 @@ struct SbKParams {
     int32_t tile_cells;               // coefficient-row entries per warp buffer (multiple of 8)
     int32_t chunk_cap;                // evaluation records per chunk
     int32_t group_units;              // units per CTA group (<= 16)
+};
+
+// Kernel parameter block of the band-grouped kernel (sb_hoist.cuh), fp32 forward.
+struct SbHParams {
+    SbModelParams mp;
+    const float2 *m01;                // [n_phase][SBH_LDN] {M0, M1}
+    int32_t n_bands, n_band_total;
+    const int32_t *band_off;
+    const double *band_lam_first, *band_zpab_inv, *band_h, *band_dlam;
+    const float *band_w;
+    int32_t n_sn, n_samples;
+    const int32_t *obs_offset;
+    const float *time, *zp, *z, *x0, *x1, *c, *t0;
+    const int32_t *band;
+    const float *flux, *fluxerr;      // may be NULL
+    float *out_flux, *out_chi2;       // may be NULL
+    const int32_t *perm;              // z-ordered supernova indices (workspace) or NULL
+    unsigned int *counter;            // group counter (workspace, zeroed by sb_zorder_kernel)
+    int32_t group_units;              // units per group (<= 32)
+    int32_t cap;                      // observations per round
 };

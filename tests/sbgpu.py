@@ -19,8 +19,9 @@ def load_handles(wl):
 
 def run_gpu(wl, *, mode: str = "chi2", fp64: bool = False, theta: Optional[Dict[str, np.ndarray]] = None,
             use_zp: bool = True, handles=None, want_flux: bool = True, want_dflux: bool = True,
-            with_data: bool = True) -> Dict[str, np.ndarray]:
-    """mode: 'flux' (sb_bandflux), 'chi2' (sb_chi2), 'grad' (sb_bandflux_grad).  Returns host fp64 arrays."""
+            with_data: bool = True, form: Optional[str] = None) -> Dict[str, np.ndarray]:
+    """mode: 'flux' (sb_bandflux), 'chi2' (sb_chi2), 'grad' (sb_bandflux_grad).  form: None (library's
+    choice), 'direct' or 'grouped' (include/saltband.h SB_FORM_*).  Returns host fp64 arrays."""
     import torch
 
     import paper_2504_08081_b200 as sb
@@ -28,6 +29,7 @@ def run_gpu(wl, *, mode: str = "chi2", fp64: bool = False, theta: Optional[Dict[
     dev = torch.device("cuda:0")
     ft = torch.float64 if fp64 else torch.float32
     dt = sb.SB_F64 if fp64 else sb.SB_F32
+    dt |= {None: 0, "direct": sb.SB_FORM_DIRECT, "grouped": sb.SB_FORM_GROUPED}[form]
     model, bands = handles if handles is not None else load_handles(wl)
     th = wl.theta if theta is None else theta
     n_units = len(th["x0"])
