@@ -150,7 +150,7 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
         sb_free_model(h);
         return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
     }
-    if (n_wave + 34 <= SBH_LDN && n_phase >= 4) { // interleaved {M0, M1} table of the band-grouped kernel
+    if (n_wave + 48 <= SBH_LDN && n_phase >= 4) { // interleaved {M0, M1} table of the band-grouped kernel
         std::vector<float2> t01((size_t)n_phase * SBH_LDN, make_float2(0.f, 0.f));
         for (int k = 0; k < n_phase; ++k)
             for (int l = 0; l < n_wave; ++l)

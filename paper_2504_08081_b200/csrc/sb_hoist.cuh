@@ -22,7 +22,7 @@
 //   a5  per observation 3 FFMA (Horner) + 1 FFMA (accumulate); warp butterfly at the end;
 //   a6/a7  epilogue per unit in fp64: zero point, flux store (coalesced), chi^2 in a fixed order.
 // Requirements (checked by the host, otherwise sb_kernels.cuh runs): fp32, forward only, every band
-// grid uniform, n_phase >= 4, n_wave + 34 <= LDN, n_cl <= NCL, band weights fit in shared memory.
+// grid uniform, n_phase >= 4, n_wave + 48 <= LDN, n_cl <= NCL, band weights fit in shared memory.
 #pragma once
 #include "sb_internal.h"
 #include "sb_kernels.cuh"
@@ -33,7 +33,6 @@ constexpr int kWarps = 16;
 constexpr int kThreads = kWarps * 32;
 constexpr int kMaxSeg = 32;  // segments (units) per round
 constexpr int kOB = 8;       // observations sharing one pass
-constexpr int kPass = 29;    // cells per pass: lanes 1..29 own a cell, lanes 0, 30, 31 carry the halo
 constexpr int kZBins = 2048; // redshift bins of the z-order permutation
 
 // One segment = a contiguous run of observations of one unit (a whole unit unless it exceeds the
@@ -58,9 +57,6 @@ struct HUnitTmp {
 };
 
 struct WScratch {
-    float wts[kOB][8];   // per observation: phase weights on M0 [0..3] and on M1 (times x1) [4..7]
-    int32_t rowoff[kOB]; // byte offset of the first of the 4 phase rows
-    int32_t slot[kOB];   // result slot of the observation
     int32_t queue[64];   // observations of the item waiting for a chunk
 };
 
@@ -159,143 +155,139 @@ struct HGeo {
     float hal, r_first;         // reduced-wavelength step per sample, value at the first sample
 };
 
-__device__ __forceinline__ float4 lds_f4(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+// Sum NV values per lane across the warp so that lane L ends with the total of value (L >> SH),
+// SH = 5 - log2(NV): log2(NV) halving steps (each lane keeps the half selected by one lane bit and
+// sends the other half to its partner), then plain butterflies over the remaining lane bits.
+template <int NV> __device__ __forceinline__ float warp_reduce_transpose(float (&v)[NV], int lane)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    static_assert(NV == 4 || NV == 8 || NV == 16 || NV == 32, "NV must be a power of two in [4, 32]");
+    int mask = 16;
+#pragma unroll
+    for (int n = NV; n > 1; n >>= 1) {
+        const bool hi = (lane & mask) != 0;
+#pragma unroll
+        for (int i = 0; i < n / 2; ++i) {
+            const float keep = hi ? v[i + n / 2] : v[i];
+            const float send = hi ? v[i] : v[i + n / 2];
+            v[i] = keep + __shfl_xor_sync(FULL, send, mask);
+        }
+        mask >>= 1;
+    }
+    float r = v[0];
+#pragma unroll
+    for (int m = 16 / NV; m > 0; m >>= 1) r += __shfl_xor_sync(FULL, r, m);
+    return r;
+}
 
-// One chunk: NOB observations of the item integrated together.
+// One chunk: up to NOB (a power of two) observations of the item integrated together; n valid.
+//
+// The band integral of observation o is  sum_j ew_j sum_m w_m(tau_j) R_o[i_j + m]  (R_o = the
+// phase-collapsed row, w_m = Keys weights, ew_j = colour factor x folded band weight).  Exchanging the
+// sums (an exact re-association) gives  sum_l At[l] R_o[l]  with the NODE WEIGHTS
+// At[l] = sum_j ew_j w_{l - i_j}(tau_j), which do not depend on the observation: they are built once
+// per chunk from the per-cell moments sum ew tau^p, and every observation then costs 8 FFMA per model
+// node (4 phase rows x {M0, M1}) with the phase weights applied after the warp reduction.
 template <int NOB, int NCL, int LDN>
-__device__ __forceinline__ void run_chunk(const SbHParams &P, const HSeg &S, const HGeo &G, const HColour<NCL> &col,
-                                          WScratch &W, const float *__restrict__ s_w, float *__restrict__ res,
-                                          int lane)
+__device__ __forceinline__ void run_chunk(int n, const SbHParams &P, const HSeg &S, const HGeo &G,
+                                          const HColour<NCL> &col, WScratch &W, const float *__restrict__ s_w,
+                                          float *__restrict__ res, int lane)
 {
     constexpr unsigned FULL = 0xffffffffu;
     constexpr int ROWB = LDN * (int)sizeof(float2); // bytes per phase row (compile time: immediate offsets)
+    constexpr int NV = 4 * NOB;                     // accumulators per lane: D[o][k], k = phase row
+    constexpr int SH = NV == 32 ? 0 : NV == 16 ? 1 : NV == 8 ? 2 : 3; // lane -> value index shift
     const SbModelParams &mp = P.mp;
     const int nW = mp.n_wave, nP = mp.n_phase;
 
-    // ---- a1/a2 per observation (lane o < NOB): phase, phase weights, row offset
-    if (lane < NOB) {
-        const int oi = W.queue[lane];
+    // ---- a1/a2 per observation: lane (o, k) = ((lane >> SH) >> 2, (lane >> SH) & 3) holds the weight
+    // of phase row rb + k of observation o; everything scalar per observation is fp64
+    const int my_o = (lane >> SH) >> 2, my_k = (lane >> SH) & 3;
+    float my_w = 0.f;
+    int my_rowoff = 0, my_slot = -1;
+    if (my_o < n) {
+        const int oi = W.queue[my_o];
         const int o = S.o_lo + oi;
         const double p = ((double)__ldg(P.time + o) - S.t0) * S.inv_opz;
         const double up = (p - mp.p0) / mp.dp;
-        float w[4] = {0.f, 0.f, 0.f, 0.f};
         int kp = 0;
+        double wv[4] = {0.0, 0.0, 0.0, 0.0}, wd[4];
         if ((up >= 0.0) && (up <= (double)(nP - 1))) { // outside the phase grid: zero flux (G3)
             kp = min((int)floor(up), nP - 2);
-            const double tau = up - (double)kp;
-            double wv[4], wd[4];
-            sb::phase_weights(tau, (kp == 0) || (kp == nP - 2), 1.0, wv, wd);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) w[k] = (float)wv[k];
+            sb::phase_weights(up - (double)kp, (kp == 0) || (kp == nP - 2), 1.0, wv, wd);
         }
         const int rb = min(max(kp - 1, 0), nP - 4); // rows rb..rb+3 are loaded
-        const int shift = (kp - 1) - rb;            // -1 at the first cell, +1 at the last, else 0
-        float ws[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const int src = k - shift;               // slot k holds the weight of row rb + k
-            float v = 0.f;
-            if (src == 0) v = w[0];
-            if (src == 1) v = w[1];
-            if (src == 2) v = w[2];
-            if (src == 3) v = w[3];
-            ws[k] = (src >= 0 && src <= 3) ? v : 0.f;
-        }
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            W.wts[lane][k] = ws[k];
-            W.wts[lane][4 + k] = ws[k] * S.x1;
-        }
-        W.rowoff[lane] = rb * ROWB;
-        W.slot[lane] = S.e_begin + oi;
+        const int src = my_k - ((kp - 1) - rb);     // row rb + k carries Keys weight index src
+        double w = 0.0;
+        if (src == 0) w = wv[0];
+        if (src == 1) w = wv[1];
+        if (src == 2) w = wv[2];
+        if (src == 3) w = wv[3];
+        my_w = (float)w;
+        my_rowoff = rb * ROWB;
+        my_slot = S.e_begin + oi;
     }
-    __syncwarp();
-
     int rowoff[NOB];
 #pragma unroll
-    for (int o = 0; o < NOB; ++o) rowoff[o] = W.rowoff[o];
-    float acc[NOB];
+    for (int o = 0; o < NOB; ++o) rowoff[o] = __shfl_sync(FULL, my_rowoff, (o * 4) << SH);
+    float D[NV];
 #pragma unroll
-    for (int o = 0; o < NOB; ++o) acc[o] = 0.f;
+    for (int i = 0; i < NV; ++i) D[i] = 0.f;
 
-    // column pointer of this lane for pass 0: node (g_first - 1 + lane)
-    const char *colp = reinterpret_cast<const char *>(P.m01) + (size_t)(G.g_first - 1 + SBH_PAD_L + lane) * sizeof(float2);
-    const int n_pass = (G.ncell + kPass - 1) / kPass;
+    // pass q: lane l <-> NODE column nbcol + 32 q + l of the table (a 256-byte aligned window: every
+    // LDG.64 of the warp touches exactly two 128-byte lines) and <-> CELL (node + 1).  Node n takes
+    // w_{-1} of cell n+1 (this lane), w_0 of cell n (lane - 1), w_1 of cell n-1 (lane - 2) and w_2 of
+    // cell n-2 (lane - 3); lanes 0..2 take them from the previous pass (carried in registers).
+    const int col_first = G.g_first - 1 + SBH_PAD_L;          // column of the first node needed
+    const int nbcol = col_first & ~15;
+    const int n_pass = (G.g_first + G.ncell + 1 + SBH_PAD_L - nbcol) / 32 + 1; // last node: g_last + 2
+    const char *colp = reinterpret_cast<const char *>(P.m01) + (ptrdiff_t)(nbcol + lane) * (ptrdiff_t)sizeof(float2);
     const float c0 = G.c0, inv_ha = G.inv_ha, ha_hi = G.ha_hi, ha_lo = G.ha_lo, hal = G.hal, r_first = G.r_first;
     const int n_in = G.n_in, ncell = G.ncell;
+    const float x1 = S.x1;
+    auto jstart = [&](int x) { // first band sample (relative to the first in-range one) of cell x
+        int j = (int)ceilf(((float)x - c0) * inv_ha);
+        j = min(max(j, 0), n_in);
+        if (x <= 0) j = 0;
+        if (x >= ncell) j = n_in;
+        return j;
+    };
+    constexpr int NA = NOB > 4 ? NOB / 2 : NOB; // observations whose loads are issued before the sample loop
+    float pa0 = 0.f, pa1 = 0.f, pa2 = 0.f;      // w_0, w_1, w_2 of the previous pass's cells
+    int gq = nbcol - SBH_PAD_L + 1 + lane - G.g_first; // this lane's cell relative to g_first
 
     for (int q = 0; q < n_pass; ++q) {
-        // ---- a2: collapse the phase rows and convert to per-cell cubic coefficients (registers)
-        const int gq = kPass * q + lane - 1; // this lane's cell relative to g_first
-        const int g = G.g_first + gq;
-        const bool special = (G.g_first + kPass * q <= 0) || (G.g_first + kPass * q + kPass >= nW - 2); // warp-uniform
-        const bool border = special && ((g <= 0) || (g >= nW - 2));
-        float cf[NOB][4];
+        // ---- a2 loads, first batch: this lane's node of the 4 phase rows ({M0, M1} pairs)
+        float2 rawa[NA][4];
 #pragma unroll
-        for (int o = 0; o < NOB; ++o) {
+        for (int o = 0; o < NA; ++o) {
             const char *p = colp + rowoff[o];
-            const float2 v0 = __ldg(reinterpret_cast<const float2 *>(p));
-            const float2 v1 = __ldg(reinterpret_cast<const float2 *>(p + ROWB));
-            const float2 v2 = __ldg(reinterpret_cast<const float2 *>(p + 2 * ROWB));
-            const float2 v3 = __ldg(reinterpret_cast<const float2 *>(p + 3 * ROWB));
-            const float4 wa = lds_f4(&W.wts[o][0]);
-            const float4 wb = lds_f4(&W.wts[o][4]);
-            float node = wa.x * v0.x;
-            node = __fmaf_rn(wa.y, v1.x, node);
-            node = __fmaf_rn(wa.z, v2.x, node);
-            node = __fmaf_rn(wa.w, v3.x, node);
-            node = __fmaf_rn(wb.x, v0.y, node);
-            node = __fmaf_rn(wb.y, v1.y, node);
-            node = __fmaf_rn(wb.z, v2.y, node);
-            node = __fmaf_rn(wb.w, v3.y, node);
-            const float rm = __shfl_up_sync(FULL, node, 1);
-            const float r1 = __shfl_down_sync(FULL, node, 1);
-            const float r2 = __shfl_down_sync(FULL, node, 2);
-            // Catmull-Rom in tau: c0 = r0, c1 = (r1 - rm)/2, c3 = 1.5 (r0 - r1) + (r2 - rm)/2,
-            // c2 = (r1 - r0) - c1 - c3
-            const float d10 = node - r1;
-            float c1 = 0.5f * (r1 - rm);
-            float c3 = __fmaf_rn(1.5f, d10, 0.5f * (r2 - rm));
-            float c2 = (-d10 - c1) - c3;
-            if (border) { // linear border cell (G2)
-                c1 = -d10;
-                c2 = 0.f;
-                c3 = 0.f;
-            }
-            cf[o][0] = node;
-            cf[o][1] = c1;
-            cf[o][2] = c2;
-            cf[o][3] = c3;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) rawa[o][k] = __ldg(reinterpret_cast<const float2 *>(p + k * ROWB));
         }
-        colp += kPass * sizeof(float2);
 
-        // ---- a1: the band samples of this lane's cell: j' in [js, je)
-        const bool valid = (lane >= 1) && (lane <= kPass) && (gq < ncell);
-        const float gf = (float)gq;
-        int js = (int)ceilf((gf - c0) * inv_ha);
-        js = min(max(js, 0), n_in);
-        if (gq <= 0) js = 0;
-        int je = __shfl_down_sync(FULL, js, 1);
-        if (gq >= ncell - 1) je = n_in;
-        const int cnt = valid ? max(je - js, 0) : 0;
+        // ---- a1: the band samples of this lane's cell
+        const int js = jstart(gq), je = jstart(gq + 1);
+        const int cnt = je - js;
         const float jsf = (float)js;
-        float tau = __fmaf_rn(jsf, ha_lo, __fmaf_rn(jsf, ha_hi, -gf)) + c0; // u_js - g
+        float tau = __fmaf_rn(jsf, ha_lo, __fmaf_rn(jsf, ha_hi, -(float)gq)) + c0; // u_js - cell
         float r = __fmaf_rn(jsf, hal, r_first);
         const float *wp = s_w + (G.wbase + js);
         const int km = __reduce_max_sync(FULL, cnt);
 
-        // ---- a3/a4/a5: samples
+        // ---- a3/a4: moments of the cell: S_p = sum_k ew_k tau_k^p
+        float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
         auto samples = [&](auto cm_tag) {
             constexpr int CM = decltype(cm_tag)::value;
             for (int k = 0; k < km; ++k) {
                 float w = 0.f;
                 if (k < cnt) w = wp[k];
                 const float ew = sb::exp_scaled(col.template arg<CM>(r)) * w;
-#pragma unroll
-                for (int o = 0; o < NOB; ++o) {
-                    const float val = __fmaf_rn(__fmaf_rn(__fmaf_rn(cf[o][3], tau, cf[o][2]), tau, cf[o][1]), tau, cf[o][0]);
-                    acc[o] = __fmaf_rn(ew, val, acc[o]);
-                }
+                const float t2 = tau * tau;
+                s0 += ew;
+                s1 = __fmaf_rn(ew, tau, s1);
+                s2 = __fmaf_rn(ew, t2, s2);
+                s3 = __fmaf_rn(ew, t2 * tau, s3);
                 tau += ha_hi;
                 r += hal;
             }
@@ -303,14 +295,66 @@ __device__ __forceinline__ void run_chunk(const SbHParams &P, const HSeg &S, con
         if (G.cmode == sb::CM_INSIDE) samples(std::integral_constant<int, sb::CM_INSIDE>{});
         else if (G.cmode == sb::CM_LINEAR) samples(std::integral_constant<int, sb::CM_LINEAR>{});
         else samples(std::integral_constant<int, sb::CM_GENERIC>{});
-    }
-    // ---- a5: wavelength integral (butterfly); raw integrals to the round's result array
+
+        // ---- moments -> weights on the cell's four nodes (Keys a = -1/2; linear in border cells, G2)
+        const int g = G.g_first + gq;
+        float am = 0.5f * (__fmaf_rn(2.0f, s2, -s3) - s1);
+        float a0 = __fmaf_rn(1.5f, s3, __fmaf_rn(-2.5f, s2, s0));
+        float a1 = 0.5f * (__fmaf_rn(4.0f, s2, s1) - 3.0f * s3);
+        float a2 = 0.5f * (s3 - s2);
+        if (g <= 0 || g >= nW - 2) {
+            am = 0.f;
+            a0 = s0 - s1;
+            a1 = s1;
+            a2 = 0.f;
+        }
+        // node weight of this lane's node
+        auto from_left = [&](float cur, float prev, int d) {
+            const float a = __shfl_up_sync(FULL, cur, d);
+            const float b = __shfl_sync(FULL, prev, (lane - d) & 31);
+            return lane >= d ? a : b;
+        };
+        const float at = am + from_left(a0, pa0, 1) + from_left(a1, pa1, 2) + from_left(a2, pa2, 3);
+        pa0 = a0;
+        pa1 = a1;
+        pa2 = a2;
+        const float at1 = at * x1;
+
+        // ---- a2/a5: D[o][k] += At * (M0 + x1 M1)[rb_o + k][node]
+        if constexpr (NOB > NA) {
+            float2 rawb[NOB - NA][4];
 #pragma unroll
-    for (int o = 0; o < NOB; ++o) acc[o] = sb::warp_sum(acc[o]);
-    if (lane == 0) {
+            for (int o = NA; o < NOB; ++o) {
+                const char *p = colp + rowoff[o];
 #pragma unroll
-        for (int o = 0; o < NOB; ++o) res[W.slot[o]] = acc[o];
+                for (int k = 0; k < 4; ++k) rawb[o - NA][k] = __ldg(reinterpret_cast<const float2 *>(p + k * ROWB));
+            }
+#pragma unroll
+            for (int o = 0; o < NA; ++o) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) D[o * 4 + k] = __fmaf_rn(at, rawa[o][k].x, __fmaf_rn(at1, rawa[o][k].y, D[o * 4 + k]));
+            }
+#pragma unroll
+            for (int o = NA; o < NOB; ++o) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    D[o * 4 + k] = __fmaf_rn(at, rawb[o - NA][k].x, __fmaf_rn(at1, rawb[o - NA][k].y, D[o * 4 + k]));
+            }
+        } else {
+#pragma unroll
+            for (int o = 0; o < NA; ++o) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) D[o * 4 + k] = __fmaf_rn(at, rawa[o][k].x, __fmaf_rn(at1, rawa[o][k].y, D[o * 4 + k]));
+            }
+        }
+        colp += 32 * sizeof(float2);
+        gq += 32;
     }
+    // ---- a5: warp reduction (lane (o, k) ends with D[o][k]), phase weights, sum over the 4 rows
+    float v = warp_reduce_transpose<NV>(D, lane) * my_w;
+    v += __shfl_xor_sync(FULL, v, 1 << SH);
+    v += __shfl_xor_sync(FULL, v, 2 << SH);
+    if (my_slot >= 0 && my_k == 0 && (lane & ((1 << SH) - 1)) == 0) res[my_slot] = v;
     __syncwarp();
 }
 
@@ -318,16 +362,10 @@ template <int NCL, int LDN>
 __device__ __forceinline__ void run_chunk_n(int n, const SbHParams &P, const HSeg &S, const HGeo &G,
                                             const HColour<NCL> &col, WScratch &W, const float *s_w, float *res, int lane)
 {
-    switch (n) {
-    case 1: run_chunk<1, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
-    case 2: run_chunk<2, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
-    case 3: run_chunk<3, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
-    case 4: run_chunk<4, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
-    case 5: run_chunk<5, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
-    case 6: run_chunk<6, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
-    case 7: run_chunk<7, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
-    default: run_chunk<8, NCL, LDN>(P, S, G, col, W, s_w, res, lane); break;
-    }
+    if (n > 4) run_chunk<8, NCL, LDN>(n, P, S, G, col, W, s_w, res, lane);
+    else if (n > 2) run_chunk<4, NCL, LDN>(n, P, S, G, col, W, s_w, res, lane);
+    else if (n > 1) run_chunk<2, NCL, LDN>(n, P, S, G, col, W, s_w, res, lane);
+    else run_chunk<1, NCL, LDN>(n, P, S, G, col, W, s_w, res, lane);
 }
 
 // One item: the observations of segment S in band b.
@@ -416,7 +454,7 @@ __device__ __forceinline__ void run_item(const SbHParams &P, const HSeg &S, int 
         qn += __popc(m);
         __syncwarp();
         while (qn >= kOB) {
-            run_chunk<kOB, NCL, LDN>(P, S, G, col, W, s_w, res, lane);
+            run_chunk<kOB, NCL, LDN>(kOB, P, S, G, col, W, s_w, res, lane);
             const int rest = qn - kOB; // <= 31
             int v = 0;
             if (lane < rest) v = W.queue[kOB + lane];

@@ -32,7 +32,7 @@ struct SbModelParams {
 // Interleaved {M0, M1} fp32 table of the band-grouped kernel (sb_hoist.cuh): [n_phase][SBH_LDN]
 // float2, node l at column l + SBH_PAD_L, zero padded.  The row stride is a compile-time constant so
 // that the four phase rows of a cell are reached with immediate offsets from one pointer.
-#define SBH_PAD_L 2
+#define SBH_PAD_L 16
 #define SBH_LDN 1856
 
 struct sb_model {
