@@ -43,6 +43,11 @@ FLOPS_PER_EVAL_FWD = 60    # phase weights, zero point, chi^2 term, butterfly
 FLOPS_PER_SAMPLE_GRAD = 46  # + unscaled arg 1, 2 extra poly3 12, f 1, 3 extra accumulators 6 (-1: no pre-scale)
 FLOPS_PER_CELL_GRAD = 82    # collapse 16 FFMA + x1 combine = 34, three coefficient sets 48
 FLOPS_PER_EVAL_GRAD = 120
+# Grouped (node-weight / adjoint) formulation, csrc/sb_hoist.cuh: per band sample of a CHUNK (up to 8
+# observations of one (unit, band) share it): colour Horner 8, ex2 1, x W 1, moments 9, steps 2;
+# per model cell of a chunk: sample range 9, moments -> node weights 20, x1 1; per node per
+# observation: 8 FFMA; per eval: phase weights, zero point, chi^2 term, reduction.
+FLOPS_G_SAMPLE, FLOPS_G_CELL, FLOPS_G_NODE_OBS, FLOPS_G_EVAL = 21, 30, 16, 60
 # SURVEY.md section 8(d) "direct (G = 1)" model, reported beside ours for reference.
 SURVEY_SAMPLE, SURVEY_NODE, SURVEY_EVAL = 55, 18, 40
 SURVEY_SAMPLE_GRAD, SURVEY_NODE_GRAD, SURVEY_EVAL_GRAD = 77, 36, 100
@@ -78,10 +83,28 @@ def geometry_counts(wl):
     return np.where(inside, n_in, 0), np.where(inside, n_cell, 0)
 
 
-def flops_per_call(wl, grad: bool):
+def chunk_share(wl, chunk: int = 8):
+    """Per observation: chunks of its (unit, band) item / observations of the item (the fraction of
+    the item's shared per-sample and per-cell work that one observation carries)."""
+    n_obs = np.diff(wl.obs_offset)
+    unit = np.repeat(np.arange(wl.n_sn, dtype=np.int64), n_obs)
+    key = unit * wl.n_bands + wl.band.astype(np.int64)
+    cnt = np.bincount(key, minlength=wl.n_sn * wl.n_bands)
+    c = cnt[key]
+    return np.ceil(c / chunk) / c
+
+
+def flops_per_call(wl, grad: bool, form: str = "direct"):
     n_in, n_cell = geometry_counts(wl)
     ns = wl.n_samples
     s_in, s_cell, n_ev = float(n_in.sum()) * ns, float(n_cell.sum()) * ns, float(wl.n_evals)
+    if form == "grouped" and not grad:
+        share = chunk_share(wl)
+        g_in, g_cell = float((n_in * share).sum()) * ns, float((n_cell * share).sum()) * ns
+        s_node = float((n_cell + 3 * (n_cell > 0)).sum()) * ns
+        ours = g_in * FLOPS_G_SAMPLE + g_cell * FLOPS_G_CELL + s_node * FLOPS_G_NODE_OBS + n_ev * FLOPS_G_EVAL
+        surv = s_in * SURVEY_SAMPLE + (s_cell + 3 * n_ev) * SURVEY_NODE + n_ev * SURVEY_EVAL
+        return ours, surv, s_in / max(n_ev, 1.0), s_cell / max(n_ev, 1.0)
     if grad:
         ours = s_in * FLOPS_PER_SAMPLE_GRAD + s_cell * FLOPS_PER_CELL_GRAD + n_ev * FLOPS_PER_EVAL_GRAD
         surv = s_in * SURVEY_SAMPLE_GRAD + (s_cell + 3 * n_ev) * SURVEY_NODE_GRAD + n_ev * SURVEY_EVAL_GRAD
@@ -241,6 +264,8 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--mode", default="chi2", choices=["chi2", "grad"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--form", default="auto", choices=["auto", "direct", "grouped"],
+                    help="formulation (include/saltband.h SB_FORM_*): auto = the library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-evals", type=int, default=400000, help="evals in the cpu_baseline sample")
     args = ap.parse_args()
@@ -284,7 +309,8 @@ def main():
     for k in ("x0", "x1", "c", "t0"):
         h[k] = pin(wl.theta[k], ft)
     d = {k: v.to(dev, non_blocking=True) for k, v in h.items()}
-    common = dict(dtype=sb.SB_F32, n_sn=wl.n_sn, n_samples=ns, n_obs_total=n_tot)
+    form_bits = {"auto": 0, "direct": sb.SB_FORM_DIRECT, "grouped": sb.SB_FORM_GROUPED}[args.form]
+    common = dict(dtype=sb.SB_F32 | form_bits, n_sn=wl.n_sn, n_samples=ns, n_obs_total=n_tot)
 
     # photometry: the CUDA path's own flux at theta_true + seeded noise (inputs of the timed call only)
     tt = {k: torch.as_tensor(wl.theta_true[k]).to(dev) for k in ("x0", "x1", "c", "t0")}
@@ -390,8 +416,12 @@ def main():
         return 0
 
     # ---- roofline of the (single) kernel: ALU-bound, against the FP32 FMA peak measured here
-    flops_ours, flops_survey, mean_in, mean_cell = flops_per_call(wl, grad)
-    kernel_ms = float(np.mean(per_step_ms))  # one kernel per step; events bracket exactly that launch
+    # which formulation ran: the grouped kernel launches a one-CTA z-order kernel before the main one
+    form_run = "grouped" if launches_per_step[0] == 2 else "direct"
+    flops_ours, flops_survey, mean_in, mean_cell = flops_per_call(wl, grad, form_run)
+    # events bracket the step's launches: the main kernel plus, in the grouped form, the one-CTA
+    # z-order kernel (< 1 % of the step, profiles/)
+    kernel_ms = float(np.mean(per_step_ms))
     try:
         peak_tf, _ = fp32_peak_tflops(torch.cuda.current_stream().cuda_stream)
         peak_src = "measured: FFMA-chain microbenchmark (csrc/sb_probe.cu) in this run"
@@ -401,9 +431,13 @@ def main():
     algo_bytes = in_bytes + out_bytes
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
-        "traffic": None, "kernel": "sb_fused_kernel<float,%s>" % ("grad" if grad else "fwd"),
+        "traffic": None,
+        "kernel": ("sb_hoist_kernel<fwd>" if form_run == "grouped" else "sb_fused_kernel<float,%s>" % ("grad" if grad else "fwd")),
+        "form": form_run,
         "kernel_ms": kernel_ms, "flops_per_eval": flops_ours / n_ev, "peak_source": peak_src,
-        "flop_model": "executed formulation (DESIGN.md): G_geom = G_col = 1",
+        "flop_model": ("executed formulation (DESIGN.md): node-weight re-association, G_geom = G_col = observations "
+                       "per (unit, band) chunk (<= 8)" if form_run == "grouped"
+                       else "executed formulation (DESIGN.md): G_geom = G_col = 1"),
         "survey_direct_model": {"flops_per_eval": flops_survey / n_ev,
                                 "achieved": flops_survey / (kernel_ms * 1e-3) * 1e-12,
                                 "frac": flops_survey / (kernel_ms * 1e-3) * 1e-12 / peak_tf},
@@ -421,7 +455,7 @@ def main():
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": wl.name, "n_sn": wl.n_sn, "n_samples": ns, "n_obs_total": n_tot, "n_evals": n_ev,
-                   "mode": args.mode, "chi2_evals_per_sec": n_units * world * steps / (total_ms * 1e-3),
+                   "mode": args.mode, "form": form_run, "chi2_evals_per_sec": n_units * world * steps / (total_ms * 1e-3),
                    "l2": "inputs+outputs %.0f MB > 126 MB L2, no flush" % ((in_bytes + out_bytes) / 1e6) if not need_flush
                    else "L2 flushed (256 MB write) between timed steps", "parallelism": f"dp{world} (independent shards)"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": d2h,
