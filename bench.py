@@ -48,6 +48,11 @@ FLOPS_PER_EVAL_GRAD = 120
 # per model cell of a chunk: sample range 9, moments -> node weights 20, x1 1; per node per
 # observation: 8 FFMA; per eval: phase weights, zero point, chi^2 term, reduction.
 FLOPS_G_SAMPLE, FLOPS_G_CELL, FLOPS_G_NODE_OBS, FLOPS_G_EVAL = 21, 30, 16, 60
+# Tiled formulation, csrc/sb_tiled.cuh: the same per-sample and per-cell work once per (unit, band)
+# ITEM (all its observations share it); per node per observation 8 FFMA (phase collapse of M0, M1
+# with x1 folded into the weights) + 1 FFMA (node weight) = 18.  Only nodes of the item's window count;
+# the zero-padded remainder of the 128-node half windows the kernel also multiplies is not counted.
+FLOPS_T_NODE_OBS = 18
 # SURVEY.md section 8(d) "direct (G = 1)" model, reported beside ours for reference.
 SURVEY_SAMPLE, SURVEY_NODE, SURVEY_EVAL = 55, 18, 40
 SURVEY_SAMPLE_GRAD, SURVEY_NODE_GRAD, SURVEY_EVAL_GRAD = 77, 36, 100
@@ -83,7 +88,7 @@ def geometry_counts(wl):
     return np.where(inside, n_in, 0), np.where(inside, n_cell, 0)
 
 
-def chunk_share(wl, chunk: int = 8):
+def chunk_share(wl, chunk: int = 8):  # chunk = 0: the whole item is one chunk
     """Per observation: chunks of its (unit, band) item / observations of the item (the fraction of
     the item's shared per-sample and per-cell work that one observation carries)."""
     n_obs = np.diff(wl.obs_offset)
@@ -91,18 +96,19 @@ def chunk_share(wl, chunk: int = 8):
     key = unit * wl.n_bands + wl.band.astype(np.int64)
     cnt = np.bincount(key, minlength=wl.n_sn * wl.n_bands)
     c = cnt[key]
-    return np.ceil(c / chunk) / c
+    return (np.ceil(c / chunk) if chunk > 0 else 1.0) / c
 
 
 def flops_per_call(wl, grad: bool, form: str = "direct"):
     n_in, n_cell = geometry_counts(wl)
     ns = wl.n_samples
     s_in, s_cell, n_ev = float(n_in.sum()) * ns, float(n_cell.sum()) * ns, float(wl.n_evals)
-    if form == "grouped" and not grad:
-        share = chunk_share(wl)
+    if form in ("grouped", "tiled") and not grad:
+        share = chunk_share(wl, 8 if form == "grouped" else 0)
+        node_obs = FLOPS_G_NODE_OBS if form == "grouped" else FLOPS_T_NODE_OBS
         g_in, g_cell = float((n_in * share).sum()) * ns, float((n_cell * share).sum()) * ns
         s_node = float((n_cell + 3 * (n_cell > 0)).sum()) * ns
-        ours = g_in * FLOPS_G_SAMPLE + g_cell * FLOPS_G_CELL + s_node * FLOPS_G_NODE_OBS + n_ev * FLOPS_G_EVAL
+        ours = g_in * FLOPS_G_SAMPLE + g_cell * FLOPS_G_CELL + s_node * node_obs + n_ev * FLOPS_G_EVAL
         surv = s_in * SURVEY_SAMPLE + (s_cell + 3 * n_ev) * SURVEY_NODE + n_ev * SURVEY_EVAL
         return ours, surv, s_in / max(n_ev, 1.0), s_cell / max(n_ev, 1.0)
     if grad:
@@ -264,7 +270,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--mode", default="chi2", choices=["chi2", "grad"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--form", default="auto", choices=["auto", "direct", "grouped"],
+    ap.add_argument("--form", default="auto", choices=["auto", "direct", "grouped", "tiled"],
                     help="formulation (include/saltband.h SB_FORM_*): auto = the library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-evals", type=int, default=400000, help="evals in the cpu_baseline sample")
@@ -309,7 +315,7 @@ def main():
     for k in ("x0", "x1", "c", "t0"):
         h[k] = pin(wl.theta[k], ft)
     d = {k: v.to(dev, non_blocking=True) for k, v in h.items()}
-    form_bits = {"auto": 0, "direct": sb.SB_FORM_DIRECT, "grouped": sb.SB_FORM_GROUPED}[args.form]
+    form_bits = {"auto": 0, "direct": sb.SB_FORM_DIRECT, "grouped": sb.SB_FORM_GROUPED, "tiled": sb.SB_FORM_TILED}[args.form]
     common = dict(dtype=sb.SB_F32 | form_bits, n_sn=wl.n_sn, n_samples=ns, n_obs_total=n_tot)
 
     # photometry: the CUDA path's own flux at theta_true + seeded noise (inputs of the timed call only)
@@ -327,6 +333,7 @@ def main():
     o_dflux = torch.empty(n_ev * 4, dtype=ft, device=dev) if grad else None
     o_dchi = torch.empty(n_units * 4, dtype=ft, device=dev) if grad else None
     launches_per_step = [0]
+    form_ran = [""]
 
     def step(t):
         if grad:
@@ -339,6 +346,7 @@ def main():
                        x0=t["x0"], x1=t["x1"], c=t["c"], t0=t["t0"], flux=t["flux"], fluxerr=t["fluxerr"],
                        out_chi2=o_chi, out_flux=o_flux, **common)
         launches_per_step[0] = sb.last_launch_count()
+        form_ran[0] = sb.last_form()
 
     in_bytes = sum(v.numel() * v.element_size() for v in h.values())
     out_bytes = o_flux.numel() * 4 + o_chi.numel() * 4 + (o_dflux.numel() * 4 + o_dchi.numel() * 4 if grad else 0)
@@ -417,7 +425,7 @@ def main():
 
     # ---- roofline of the (single) kernel: ALU-bound, against the FP32 FMA peak measured here
     # which formulation ran: the grouped kernel launches a one-CTA z-order kernel before the main one
-    form_run = "grouped" if launches_per_step[0] == 2 else "direct"
+    form_run = form_ran[0]
     flops_ours, flops_survey, mean_in, mean_cell = flops_per_call(wl, grad, form_run)
     # events bracket the step's launches: the main kernel plus, in the grouped form, the one-CTA
     # z-order kernel (< 1 % of the step, profiles/)
@@ -432,12 +440,15 @@ def main():
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
         "traffic": None,
-        "kernel": ("sb_hoist_kernel<fwd>" if form_run == "grouped" else "sb_fused_kernel<float,%s>" % ("grad" if grad else "fwd")),
+        "kernel": {"grouped": "sb_hoist_kernel<fwd>", "tiled": "sb_tiled_kernel<fwd>"}.get(
+            form_run, "sb_fused_kernel<float,%s>" % ("grad" if grad else "fwd")),
         "form": form_run,
         "kernel_ms": kernel_ms, "flops_per_eval": flops_ours / n_ev, "peak_source": peak_src,
-        "flop_model": ("executed formulation (DESIGN.md): node-weight re-association, G_geom = G_col = observations "
-                       "per (unit, band) chunk (<= 8)" if form_run == "grouped"
-                       else "executed formulation (DESIGN.md): G_geom = G_col = 1"),
+        "flop_model": {"grouped": "executed formulation (DESIGN.md): node-weight re-association, G_geom = G_col = "
+                                  "observations per (unit, band) chunk (<= 8)",
+                       "tiled": "executed formulation (DESIGN.md): node-weight re-association, G_geom = G_col = "
+                                "observations per (unit, band)"}.get(
+            form_run, "executed formulation (DESIGN.md): G_geom = G_col = 1"),
         "survey_direct_model": {"flops_per_eval": flops_survey / n_ev,
                                 "achieved": flops_survey / (kernel_ms * 1e-3) * 1e-12,
                                 "frac": flops_survey / (kernel_ms * 1e-3) * 1e-12 / peak_tf},

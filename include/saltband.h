@@ -60,8 +60,11 @@ typedef enum { SB_F32 = 0, SB_F64 = 1 } sb_dtype;
  *   SB_FORM_GROUPED  the observations of a unit that share a band are integrated together, sharing
  *                    the rest-frame geometry and the colour factor; fp32 forward calls with uniform
  *                    band grids only -- a call that demands it where it does not apply returns
- *                    SB_ELIMIT. */
-enum { SB_FORM_DIRECT = 0x100, SB_FORM_GROUPED = 0x200 };
+ *                    SB_ELIMIT.
+ *   SB_FORM_TILED    as SB_FORM_GROUPED, and the observations of a group of units that are neighbours
+ *                    in redshift are ordered by phase so that the model rows they read stay in
+ *                    registers; same applicability and error behaviour. */
+enum { SB_FORM_DIRECT = 0x100, SB_FORM_GROUPED = 0x200, SB_FORM_TILED = 0x400 };
 
 typedef enum {
     SB_OK = 0,
@@ -145,6 +148,9 @@ int32_t sb_bands_count(const sb_bands *b);
 double sb_bands_zpab(const sb_bands *b, int32_t band);
 /* Number of kernels launched by the calling thread's most recent compute call (0 if it failed). */
 int32_t sb_last_launch_count(void);
+/* SB_FORM_* bit of the formulation that the calling thread's most recent compute call ran (0 if it
+ * failed or launched nothing). */
+int32_t sb_last_form(void);
 /* cudaError_t of the calling thread's most recent failing CUDA call (0 if none). */
 int32_t sb_last_cuda_error(void);
 const char *sb_strerror(int status);

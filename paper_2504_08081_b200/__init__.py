@@ -10,9 +10,11 @@ from .api import (  # noqa: F401
     SB_F64,
     SB_FORM_DIRECT,
     SB_FORM_GROUPED,
+    SB_FORM_TILED,
     Bands,
     Model,
     SaltbandError,
+    last_form,
     last_launch_count,
     lib_path,
     sb_bandflux,

@@ -12,7 +12,7 @@ from typing import Optional
 import numpy as np
 
 SB_F32, SB_F64 = 0, 1
-SB_FORM_DIRECT, SB_FORM_GROUPED = 0x100, 0x200  # optional formulation bits OR-ed into dtype
+SB_FORM_DIRECT, SB_FORM_GROUPED, SB_FORM_TILED = 0x100, 0x200, 0x400  # optional formulation bits OR-ed into dtype
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "libsaltband.so")
@@ -68,6 +68,7 @@ def _load():
     L.sb_bands_zpab.argtypes = [vp, C.c_int32]
     L.sb_last_launch_count.restype = C.c_int32
     L.sb_last_cuda_error.restype = C.c_int32
+    L.sb_last_form.restype = C.c_int32
     L.sb_strerror.restype = C.c_char_p
     L.sb_strerror.argtypes = [C.c_int]
     L.sb_version.restype = C.c_char_p
@@ -88,6 +89,11 @@ def version() -> str:
 
 def last_launch_count() -> int:
     return int(_load().sb_last_launch_count())
+
+
+def last_form() -> str:
+    """Formulation the most recent compute call ran: 'direct', 'grouped', 'tiled' or ''."""
+    return {SB_FORM_DIRECT: "direct", SB_FORM_GROUPED: "grouped", SB_FORM_TILED: "tiled"}.get(int(_load().sb_last_form()), "")
 
 
 def _f64(a) -> np.ndarray:

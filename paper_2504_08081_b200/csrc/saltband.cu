@@ -10,11 +10,13 @@
 #include "sb_internal.h"
 #include "sb_kernels.cuh"
 #include "sb_hoist.cuh"
+#include "sb_tiled.cuh"
 
 namespace {
 
 thread_local int32_t tl_launches = 0;
 thread_local int32_t tl_cuda_err = 0;
+thread_local int32_t tl_form = 0;
 
 bool cuda_ok(cudaError_t e)
 {
@@ -96,6 +98,7 @@ const char *sb_strerror(int status)
 
 int32_t sb_last_launch_count(void) { return tl_launches; }
 int32_t sb_last_cuda_error(void) { return tl_cuda_err; }
+int32_t sb_last_form(void) { return tl_form; }
 
 int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int32_t n_wave, const double *m0,
                   const double *m1, const double *cl_coef, int32_t n_cl, double cl_wave_b, double cl_wave_v,
@@ -288,6 +291,7 @@ int launch_inst(const SbKParams &kp, size_t smem, int grid, cudaStream_t st)
     kern<<<grid, NWARPS * 32, smem, st>>>(kp);
     if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
     tl_launches += 1;
+    tl_form = SB_FORM_DIRECT;
     return SB_OK;
 }
 
@@ -337,26 +341,36 @@ int launch_typed(SbKParams &kp, const sb_bands *b, int n_obs_total, cudaStream_t
     return launch_inst<T, GRAD, SB_MAX_CL, false, NWARPS>(kp, smem, grid, st);
 }
 
-// Band-grouped kernel (sb_hoist.cuh): fp32 forward, uniform band grids.  Returns 1 when it is not
-// applicable (the caller then runs the per-evaluation kernel), SB_OK or an error otherwise.
-int launch_hoisted(const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux, const void *fluxerr,
-                   void *out_flux, void *out_chi2, cudaStream_t st)
+// Band-grouped kernels: fp32 forward, uniform band grids.  tiled = true: sb_tiled.cuh (register-tiled
+// node contraction), false: sb_hoist.cuh.  Returns 1 when the kernel is not applicable (the caller
+// then tries the next formulation), SB_OK or an error otherwise.
+int launch_grouped(bool tiled, const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux,
+                   const void *fluxerr, void *out_flux, void *out_chi2, cudaStream_t st)
 {
     constexpr int NCL = 5;
-    if (!m->m01_f32 || !b->all_uniform || m->prm.n_cl > NCL || b->n_bands > 64) return 1;
+    if (!b->all_uniform || m->prm.n_cl > NCL || b->n_bands > 64) return 1;
+    if (tiled && (m->prm.n_phase < 4 || m->prm.n_phase > 4096)) return 1;
+    if (!tiled && !m->m01_f32) return 1;
     const int smem_max = device_smem_optin();
     const int n_sm = device_sm_count();
     if (smem_max <= 0 || n_sm <= 0) return SB_ECUDA;
     const long long n_units = (long long)bt->n_sn * bt->n_samples;
     const double mean_obs = bt->n_sn > 0 ? (double)bt->n_obs_total / (double)bt->n_sn : 1.0;
     // units per group: enough groups for every SM (>= 4 per CTA), at most kMaxSeg, about <= cap observations
-    const int cap = 4096;
+    int cap = tiled ? 3072 : 4096;
+    size_t smem = 0;
+    if (tiled) {
+        while (cap >= 512 && sbt::TSmem(b->n_total, cap).total > (size_t)smem_max) cap -= 512;
+        if (cap < 512) return 1;
+        smem = sbt::TSmem(b->n_total, cap).total;
+    } else {
+        smem = sbh::HSmem(b->n_total, cap).total;
+        if (smem > (size_t)smem_max || smem > 100 * 1024) return 1;
+    }
     long long g = n_units / ((long long)n_sm * 4);
     if (g > sbh::kMaxSeg) g = sbh::kMaxSeg;
     if ((double)g * mean_obs > (double)cap) g = (long long)((double)cap / mean_obs);
     if (g < 1) g = 1;
-    const sbh::HSmem L(b->n_total, cap);
-    if (L.total > (size_t)smem_max || L.total > 100 * 1024) return 1;
 
     unsigned char *ws = nullptr; // workspace: group counter + z-order permutation (stream-ordered)
     const size_t ws_bytes = 256 + sizeof(int32_t) * (size_t)bt->n_sn;
@@ -365,6 +379,8 @@ int launch_hoisted(const sb_model *m, const sb_bands *b, const sb_batch *bt, con
     memset(&hp, 0, sizeof(hp));
     hp.mp = m->prm;
     hp.m01 = m->m01_f32;
+    hp.m0 = m->m0_f32;
+    hp.m1 = m->m1_f32;
     hp.n_bands = b->n_bands;
     hp.n_band_total = b->n_total;
     hp.band_off = b->d_off;
@@ -397,14 +413,20 @@ int launch_hoisted(const sb_model *m, const sb_bands *b, const sb_batch *bt, con
     if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
     if (rc == SB_OK) {
         tl_launches += 1;
-        auto kern = sbh::sb_hoist_kernel<NCL, SBH_LDN>;
         const long long n_groups = (n_units + g - 1) / g;
         const int grid = (int)(n_groups < (long long)n_sm ? n_groups : (long long)n_sm);
-        if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total))) rc = SB_ECUDA;
+        if (tiled) {
+            auto kern = sbt::sb_tiled_kernel<NCL>;
+            if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) rc = SB_ECUDA;
+            if (rc == SB_OK) kern<<<grid, sbt::kThreads, smem, st>>>(hp);
+        } else {
+            auto kern = sbh::sb_hoist_kernel<NCL, SBH_LDN>;
+            if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) rc = SB_ECUDA;
+            if (rc == SB_OK) kern<<<grid, sbh::kThreads, smem, st>>>(hp);
+        }
         if (rc == SB_OK) {
-            kern<<<grid, sbh::kThreads, L.total, st>>>(hp);
             if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
-            else tl_launches += 1;
+            else { tl_launches += 1; tl_form = tiled ? SB_FORM_TILED : SB_FORM_GROUPED; }
         }
     }
     if (!cuda_ok(cudaFreeAsync(ws, st)) && rc == SB_OK) rc = SB_ECUDA;
@@ -415,12 +437,14 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void 
         void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2, void *stream, bool grad)
 {
     tl_launches = 0;
+    tl_form = 0;
     if (!m || !b || !bt_in) return SB_EINVAL;
     sb_batch batch = *bt_in; // split the formulation bits off the dtype
-    const int32_t form = batch.dtype & (SB_FORM_DIRECT | SB_FORM_GROUPED);
-    batch.dtype &= ~(SB_FORM_DIRECT | SB_FORM_GROUPED);
+    constexpr int32_t kForms = SB_FORM_DIRECT | SB_FORM_GROUPED | SB_FORM_TILED;
+    const int32_t form = batch.dtype & kForms;
+    batch.dtype &= ~kForms;
     const sb_batch *bt = &batch;
-    if (form == (SB_FORM_DIRECT | SB_FORM_GROUPED)) return SB_EINVAL;
+    if (form & (form - 1)) return SB_EINVAL; // at most one formulation bit
     if (bt->dtype != SB_F32 && bt->dtype != SB_F64) return SB_EINVAL;
     if (bt->n_sn < 0 || bt->n_samples < 1 || bt->n_obs_total < 0) return SB_EINVAL;
     if ((out_chi2 || out_dchi2) && (!flux || !fluxerr)) return SB_EINVAL;
@@ -461,10 +485,16 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void 
     kp.out_dchi2 = out_dchi2;
     cudaStream_t st = (cudaStream_t)stream;
     if (f32 && !grad && form != SB_FORM_DIRECT && bt->n_obs_total > 0) {
-        const int rc = launch_hoisted(m, b, bt, flux, fluxerr, out_flux, out_chi2, st);
-        if (rc != 1) return rc;
+        if (form != SB_FORM_GROUPED) {
+            const int rc = launch_grouped(true, m, b, bt, flux, fluxerr, out_flux, out_chi2, st);
+            if (rc != 1) return rc;
+        }
+        if (form != SB_FORM_TILED) {
+            const int rc = launch_grouped(false, m, b, bt, flux, fluxerr, out_flux, out_chi2, st);
+            if (rc != 1) return rc;
+        }
     }
-    if (form == SB_FORM_GROUPED) return SB_ELIMIT; // the grouped formulation was demanded but does not apply
+    if (form == SB_FORM_GROUPED || form == SB_FORM_TILED) return SB_ELIMIT; // demanded but does not apply
     if (f32) {
         if (grad) return launch_typed<float, true, 8>(kp, b, bt->n_obs_total, st);
         return launch_typed<float, false, 16>(kp, b, bt->n_obs_total, st);

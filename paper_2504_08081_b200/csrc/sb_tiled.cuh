@@ -1,0 +1,656 @@
+// sb_tiled.cuh -- the register-tiled node-weight kernel (sm_100a), fp32 forward.
+//
+// Same sums per evaluation as sb_kernels.cuh / sb_hoist.cuh, with
+// the band integral re-associated as in sb_hoist.cuh (an exact exchange of two finite sums):
+//     raw_o = sum_l At[l] * R_o[l],   At[l] = sum_j ew_j w_{l-i_j}(tau_j)   (NODE WEIGHTS of (unit, band)),
+//     R_o[l] = sum_k wp_k(o) (M0 + x1 M1)[rb_o + k][l]                      (phase-collapsed row of o),
+// ew_j = exp(c CL(lambda_j/(1+z))) W_j, w = Keys a = -1/2 weights (reading G1).
+//
+// What differs from sb_hoist.cuh is WHO holds WHAT.  There a lane reloaded the four phase rows of
+// {M0, M1} for every observation (four LDG.64 per eight FFMA: bound by the L1 data pipe).  Here a CTA
+// works on a GROUP of up to 32 units that are neighbours in redshift, one STAGE (a set of bands) at a
+// time, in two phases separated by a CTA barrier:
+//   phase A  one warp per ITEM (unit, band): lanes own model cells, walk the band samples of their
+//            cell (colour factor x folded weight, moments sum ew tau^p), turn the moments into node
+//            weights and store At[item][node] in SHARED MEMORY (<= 512 nodes per item and pass);
+//   phase B  the observations of the stage, sorted by (band, first phase row rb), are cut into equal
+//            contiguous chunks, one per warp.  A lane owns 8 nodes of a 256-node window and keeps the
+//            four phase rows of M0 and of M1 at those nodes in REGISTERS (64 values, row r in slot
+//            r mod 4); moving to the next observation only reloads the rows that changed.  Per
+//            observation a lane reads its 8 node weights (two LDS.128) and issues 72 FFMA; four
+//            observations share one transposed warp reduction.
+// HBM sees only the per-observation records; the model window is read from L2/L1 about once per
+// (warp, stage) instead of once per observation.
+// Requirements (checked by the host, otherwise sb_hoist.cuh / sb_kernels.cuh run): fp32, forward
+// only, uniform band grids, n_phase in [4, 4096], n_cl <= NCL, n_bands <= 64.
+#pragma once
+#include "sb_internal.h"
+#include "sb_kernels.cuh"
+#include "sb_hoist.cuh"
+
+namespace sbt {
+
+using sbh::HColour;
+using sbh::HSeg;
+using sbh::HUnitTmp;
+using sbh::kMaxSeg;
+
+constexpr int kWarps = 16;
+constexpr int kThreads = kWarps * 32;
+constexpr int kSlots = 32;        // items (unit, band) per stage
+constexpr int kW = 512;           // node weights per item slot (one window segment)
+constexpr int kPassSeg = kW / 32; // phase-A passes per window segment
+constexpr int kNPL = 8;           // nodes per lane in phase B
+constexpr int kWinB = 32 * kNPL;  // nodes per phase-B window
+constexpr int kBins = 2048;       // bins of the (band, phase row) counting sort
+constexpr int kMaxBands = 64;
+
+// One item (segment, band) of the current stage.
+struct TItem {
+    int32_t n_in;    // in-range band samples (0: nothing to do)
+    int32_t ncell;   // model cells spanned
+    int32_t g_first; // first cell
+    int32_t wbase;   // index of the first in-range sample in the staged weight table
+    int32_t cmode;
+    int32_t nb0;     // first node of the item's window (multiple of 4, >= -4)
+    int32_t n_pass;  // 32-node passes of the whole window
+    int32_t nbw;     // first node held in the slot for the current window segment
+    int32_t lenw;    // nodes held in the slot (multiple of 32; 0: none)
+    float c0, ha_hi, ha_lo, inv_ha, hal, r_first, lin_a, lin_b;
+};
+
+struct TSmem {
+    size_t w, at, res, ws, info, key, hist, bstart, segs, utmp, items, win, misc, total;
+    __host__ __device__ TSmem(int n_band_total, int cap)
+    {
+        size_t o = 0;
+        at = o; o += (size_t)kSlots * kW * sizeof(float);
+        ws = o; o += (size_t)cap * sizeof(float4);
+        w = o; o += (size_t)((n_band_total + 3) & ~3) * sizeof(float);
+        res = o; o += (size_t)cap * sizeof(float);
+        info = o; o += (size_t)cap * sizeof(uint32_t);
+        hist = o; o += (size_t)kBins * sizeof(int32_t);
+        bstart = o; o += (size_t)(kMaxBands + 4) * sizeof(int32_t);
+        key = o; o += (size_t)((cap + 7) & ~7) * sizeof(uint16_t);
+        o = (o + 15) & ~(size_t)15;
+        segs = o; o += (size_t)kMaxSeg * sizeof(HSeg);
+        utmp = o; o += (size_t)kMaxSeg * sizeof(HUnitTmp);
+        items = o; o += (size_t)kSlots * sizeof(TItem);
+        win = o; o += (size_t)2 * kSlots * sizeof(int32_t);
+        misc = o; o += 64;
+        total = o;
+    }
+};
+
+__device__ __forceinline__ float4 lds128(const float *p) { return *reinterpret_cast<const float4 *>(p); }
+
+// ---- geometry of one item (segment S, band b): one thread.  Same decisions as sbh::run_item: the
+// in-range sample range [j_lo, j_hi) in fp64 (reading G9), the window of model cells, the colour mode.
+__device__ __forceinline__ void item_geometry(const SbHParams &P, const HSeg &S, int b, TItem &I)
+{
+    const SbModelParams &mp = P.mp;
+    const int nW = mp.n_wave;
+    I.n_in = 0;
+    I.n_pass = 0;
+    I.lenw = 0;
+    I.nbw = 0;
+    const int boff = __ldg(P.band_off + b);
+    const int nb = __ldg(P.band_off + b + 1) - boff;
+    const double lam_first = __ldg(P.band_lam_first + b);
+    const double h = __ldg(P.band_h + b);
+    const double opz = S.opz, inv_opz = S.inv_opz;
+    const double dl_lo = mp.l0 * opz - lam_first;
+    const double dl_hi = (mp.l0 + (double)(nW - 1) * mp.dl) * opz - lam_first;
+    const double *__restrict__ dlam = P.band_dlam + boff;
+    int j_lo = (int)fmin(fmax(ceil(dl_lo / h), 0.0), (double)nb);
+    while (j_lo > 0 && __ldg(dlam + j_lo - 1) >= dl_lo) --j_lo;
+    while (j_lo < nb && __ldg(dlam + j_lo) < dl_lo) ++j_lo;
+    int j_hi = (int)fmin(fmax(floor(dl_hi / h) + 1.0, 0.0), (double)nb);
+    while (j_hi < nb && __ldg(dlam + j_hi) <= dl_hi) ++j_hi;
+    while (j_hi > 0 && __ldg(dlam + j_hi - 1) > dl_hi) --j_hi;
+    if (j_lo >= j_hi) return; // band entirely outside the model grid: results stay 0 (G3)
+
+    const double a_d = inv_opz / mp.dl;                      // cells per observer-frame Angstrom
+    const double ub = (lam_first * inv_opz - mp.l0) / mp.dl; // u of dlam = 0
+    const double ha = h * a_d;                               // cells per band sample
+    const double u_lo = (double)j_lo * ha + ub;
+    const double u_hi = (double)(j_hi - 1) * ha + ub;
+    const int g_first = min(max((int)floor(u_lo), 0), nW - 2);
+    const int g_last = min(max((int)floor(u_hi), 0), nW - 2);
+    I.n_in = j_hi - j_lo;
+    I.g_first = g_first;
+    I.ncell = g_last - g_first + 1;
+    I.wbase = boff + j_lo;
+    I.c0 = (float)(u_lo - (double)g_first);
+    I.ha_hi = (float)ha;
+    I.ha_lo = (float)(ha - (double)I.ha_hi);
+    I.inv_ha = (float)(1.0 / ha);
+    const double al_d = inv_opz * mp.cl_inv_span;
+    const double be_d = (lam_first * inv_opz - mp.cl_b) * mp.cl_inv_span;
+    const double hal = h * al_d;
+    const double r_a = (double)j_lo * hal + be_d, r_b = (double)(j_hi - 1) * hal + be_d;
+    I.hal = (float)hal;
+    I.r_first = (float)r_a;
+    I.lin_a = 0.f;
+    I.lin_b = 0.f;
+    const double r_min = fmin(r_a, r_b), r_max = fmax(r_a, r_b);
+    const double margin = 1e-4;
+    int cmode = sb::CM_GENERIC;
+    if (r_min >= mp.r_lo + margin && r_max <= mp.r_hi - margin) {
+        cmode = sb::CM_INSIDE;
+    } else if (r_min >= mp.r_hi + margin) { // arg = p_hi + s_hi (r - r_hi)
+        cmode = sb::CM_LINEAR;
+        I.lin_b = S.s_hi;
+        I.lin_a = (float)((double)S.p_hi - (double)S.s_hi * mp.r_hi);
+    } else if (r_max <= mp.r_lo - margin) {
+        cmode = sb::CM_LINEAR;
+        I.lin_b = S.s_lo;
+        I.lin_a = (float)((double)S.p_lo - (double)S.s_lo * mp.r_lo);
+    }
+    I.cmode = cmode;
+    // window of nodes g_first-1 .. g_last+2, first node aligned down to a multiple of 4
+    I.nb0 = (g_first - 1) & ~3;
+    I.n_pass = (g_last + 2 - I.nb0) / 32 + 1;
+}
+
+// ---- phase A: node weights of one item for window segment wseg -> At slot (one warp) -------------
+// Pass q: lane l <-> NODE nb0 + 32 q + l and <-> CELL node + 1.  Node n takes w_{-1} of cell n+1 (this
+// lane), w_0 of cell n (lane - 1), w_1 of cell n-1 (lane - 2) and w_2 of cell n-2 (lane - 3); lanes
+// 0..2 take them from the previous pass (carried in registers; for wseg > 0 the pass before the
+// segment is recomputed for its carries only).
+template <int NCL>
+__device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg &S, TItem &I, int wseg,
+                                             const float *__restrict__ s_w, float *__restrict__ at_slot, int lane)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    const int q_lo = wseg * kPassSeg;
+    const int q_hi = min(q_lo + kPassSeg, I.n_pass);
+    if (I.n_in == 0 || q_lo >= q_hi) {
+        if (lane == 0) I.lenw = 0;
+        return;
+    }
+    HColour<NCL> col;
+#pragma unroll
+    for (int q = 0; q < NCL; ++q) col.a[q] = S.cl[q];
+    col.r_lo = (float)mp.r_lo;
+    col.r_hi = (float)mp.r_hi;
+    col.s_lo = S.s_lo;
+    col.s_hi = S.s_hi;
+    col.lin_a = I.lin_a;
+    col.lin_b = I.lin_b;
+    const int nW = mp.n_wave;
+    const float c0 = I.c0, inv_ha = I.inv_ha, ha_hi = I.ha_hi, ha_lo = I.ha_lo, hal = I.hal, r_first = I.r_first;
+    const int n_in = I.n_in, ncell = I.ncell, cmode = I.cmode;
+    auto jstart = [&](int x) { // first band sample (relative to the first in-range one) of cell x
+        int j = (int)ceilf(((float)x - c0) * inv_ha);
+        j = min(max(j, 0), n_in);
+        if (x <= 0) j = 0;
+        if (x >= ncell) j = n_in;
+        return j;
+    };
+    const int q_start = q_lo > 0 ? q_lo - 1 : 0;
+    float pa0 = 0.f, pa1 = 0.f, pa2 = 0.f;
+    int gq = I.nb0 + 32 * q_start + lane + 1 - I.g_first; // this lane's cell relative to g_first
+    for (int q = q_start; q < q_hi; ++q) {
+        const int js = jstart(gq), je = jstart(gq + 1);
+        const int cnt = je - js;
+        const float jsf = (float)js;
+        float tau = __fmaf_rn(jsf, ha_lo, __fmaf_rn(jsf, ha_hi, -(float)gq)) + c0; // u_js - cell
+        float r = __fmaf_rn(jsf, hal, r_first);
+        const float *wp = s_w + (I.wbase + js);
+        const int km = __reduce_max_sync(FULL, cnt);
+        float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+        auto samples = [&](auto cm_tag) {
+            constexpr int CM = decltype(cm_tag)::value;
+            for (int k = 0; k < km; ++k) {
+                float w = 0.f;
+                if (k < cnt) w = wp[k];
+                const float ew = sb::exp_scaled(col.template arg<CM>(r)) * w;
+                const float t2 = tau * tau;
+                s0 += ew;
+                s1 = __fmaf_rn(ew, tau, s1);
+                s2 = __fmaf_rn(ew, t2, s2);
+                s3 = __fmaf_rn(ew, t2 * tau, s3);
+                tau += ha_hi;
+                r += hal;
+            }
+        };
+        if (cmode == sb::CM_INSIDE) samples(std::integral_constant<int, sb::CM_INSIDE>{});
+        else if (cmode == sb::CM_LINEAR) samples(std::integral_constant<int, sb::CM_LINEAR>{});
+        else samples(std::integral_constant<int, sb::CM_GENERIC>{});
+        // moments -> weights on the cell's four nodes (Keys a = -1/2; linear in border cells, G2)
+        const int g = I.g_first + gq;
+        float am = 0.5f * (__fmaf_rn(2.0f, s2, -s3) - s1);
+        float a0 = __fmaf_rn(1.5f, s3, __fmaf_rn(-2.5f, s2, s0));
+        float a1 = 0.5f * (__fmaf_rn(4.0f, s2, s1) - 3.0f * s3);
+        float a2 = 0.5f * (s3 - s2);
+        if (g <= 0 || g >= nW - 2) {
+            am = 0.f;
+            a0 = s0 - s1;
+            a1 = s1;
+            a2 = 0.f;
+        }
+        auto from_left = [&](float cur, float prev, int d) {
+            const float a = __shfl_up_sync(FULL, cur, d);
+            const float b = __shfl_sync(FULL, prev, (lane - d) & 31);
+            return lane >= d ? a : b;
+        };
+        const float at = am + from_left(a0, pa0, 1) + from_left(a1, pa1, 2) + from_left(a2, pa2, 3);
+        pa0 = a0;
+        pa1 = a1;
+        pa2 = a2;
+        if (q >= q_lo) at_slot[(q - q_lo) * 32 + lane] = at;
+        gq += 32;
+    }
+    if (lane == 0) {
+        I.nbw = I.nb0 + 32 * q_lo;
+        I.lenw = 32 * (q_hi - q_lo);
+    }
+}
+
+// ---- phase B: the observations [i_lo, i_hi) of the sorted list (all of one band) on one warp ------
+// Node window [S, S + 256): lane l owns nodes S + 4 l .. + 3 and S + 128 + 4 l .. + 3.
+struct RowRegs {
+    float m0[4][kNPL], m1[4][kNPL]; // [slot = row mod 4][node]
+};
+
+__device__ __forceinline__ void load_row(RowRegs &R, int s, const float *__restrict__ p0, const float *__restrict__ p1,
+                                         ptrdiff_t rowoff, bool ok_lo, bool ok_hi)
+{
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
+    if (ok_lo) {
+        a = __ldg(reinterpret_cast<const float4 *>(p0 + rowoff));
+        c = __ldg(reinterpret_cast<const float4 *>(p1 + rowoff));
+    }
+    if (ok_hi) {
+        b = __ldg(reinterpret_cast<const float4 *>(p0 + rowoff + 128));
+        d = __ldg(reinterpret_cast<const float4 *>(p1 + rowoff + 128));
+    }
+    R.m0[s][0] = a.x; R.m0[s][1] = a.y; R.m0[s][2] = a.z; R.m0[s][3] = a.w;
+    R.m0[s][4] = b.x; R.m0[s][5] = b.y; R.m0[s][6] = b.z; R.m0[s][7] = b.w;
+    R.m1[s][0] = c.x; R.m1[s][1] = c.y; R.m1[s][2] = c.z; R.m1[s][3] = c.w;
+    R.m1[s][4] = d.x; R.m1[s][5] = d.y; R.m1[s][6] = d.z; R.m1[s][7] = d.w;
+}
+
+__device__ __forceinline__ void phase_b_chunk(const SbHParams &P, const HSeg *__restrict__ segs,
+                                              const TItem *__restrict__ items_band, const float *__restrict__ s_at,
+                                              int slot0, const float4 *__restrict__ s_ws,
+                                              const uint32_t *__restrict__ s_info, float *__restrict__ res, int i_lo,
+                                              int i_hi, int w_lo, int w_hi, int lane)
+{
+    const int ld = P.mp.ld;
+    for (int S = w_lo; S < w_hi; S += kWinB) {
+        RowRegs R;
+        int held[4] = {-1, -1, -1, -1};
+        const int col = S + SB_PAD_L + 4 * lane; // column of this lane's first node (multiple of 4)
+        const bool ok_lo = col >= 0 && col + 4 <= ld;
+        const bool ok_hi = col + 128 >= 0 && col + 132 <= ld;
+        const float *p0 = P.m0 + col, *p1 = P.m1 + col;
+#pragma unroll
+        for (int s = 0; s < 4; ++s)
+#pragma unroll
+            for (int q = 0; q < kNPL; ++q) { R.m0[s][q] = 0.f; R.m1[s][q] = 0.f; }
+
+        for (int i = i_lo; i < i_hi; i += 4) {
+            float acc[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                acc[j] = 0.f;
+                if (i + j >= i_hi) continue;
+                const uint32_t info = s_info[i + j];
+                const int sg = (int)(info & 31u), rb = (int)((info >> 5) & 4095u);
+                const TItem &I = items_band[sg];
+                const int off = S - I.nbw; // multiple of 4
+                const int len = I.lenw;
+                if (len == 0 || off + kWinB <= 0 || off >= len) continue; // the item's nodes do not reach this window
+                // rows rb .. rb+3, row r in slot r mod 4: reload only what changed
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    const int row = rb + ((s - rb) & 3);
+                    if (held[s] != row) {
+                        load_row(R, s, p0, p1, (ptrdiff_t)row * ld, ok_lo, ok_hi);
+                        held[s] = row;
+                    }
+                }
+                const float4 w4 = s_ws[i + j];
+                const float x1 = segs[sg].x1;
+                const float ws[4] = {w4.x, w4.y, w4.z, w4.w};
+                const float vs[4] = {w4.x * x1, w4.y * x1, w4.z * x1, w4.w * x1};
+                const float *ap = s_at + (size_t)(slot0 + sg) * kW;
+                const int o = off + 4 * lane;
+                float a = 0.f;
+                {
+                    float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (o >= 0 && o < len) t = lds128(ap + o);
+                    const float av[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        float r = ws[0] * R.m0[0][q];
+#pragma unroll
+                        for (int s = 1; s < 4; ++s) r = __fmaf_rn(ws[s], R.m0[s][q], r);
+#pragma unroll
+                        for (int s = 0; s < 4; ++s) r = __fmaf_rn(vs[s], R.m1[s][q], r);
+                        a = __fmaf_rn(av[q], r, a);
+                    }
+                }
+                if (off + 128 < len) { // warp-uniform: the upper half of the window holds nodes of the item
+                    const int o2 = o + 128;
+                    float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (o2 >= 0 && o2 < len) t = lds128(ap + o2);
+                    const float av[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        float r = ws[0] * R.m0[0][4 + q];
+#pragma unroll
+                        for (int s = 1; s < 4; ++s) r = __fmaf_rn(ws[s], R.m0[s][4 + q], r);
+#pragma unroll
+                        for (int s = 0; s < 4; ++s) r = __fmaf_rn(vs[s], R.m1[s][4 + q], r);
+                        a = __fmaf_rn(av[q], r, a);
+                    }
+                }
+                acc[j] = a;
+            }
+            // lane L ends with the total of observation i + (L >> 3)
+            const float v = sbh::warp_reduce_transpose<4>(acc, lane);
+            const int jj = lane >> 3;
+            if ((lane & 7) == 0 && i + jj < i_hi) {
+                const int e = (int)(s_info[i + jj] >> 17);
+                res[e] += v;
+            }
+        }
+        __syncwarp();
+    }
+}
+
+// Phase of observation o of segment S: first loaded phase row rb (rows rb .. rb+3) and the weights of
+// those rows (Keys a = -1/2, linear in the border cells -- readings G1, G2), scalar work in fp64.
+// Returns false when the phase is outside the grid (zero flux, reading G3).
+__device__ __forceinline__ bool obs_phase(const SbModelParams &mp, const HSeg &S, float t, int &rb, double (&wrow)[4])
+{
+    const int nP = mp.n_phase;
+    const double p = ((double)t - S.t0) * S.inv_opz;
+    const double up = (p - mp.p0) / mp.dp;
+    if (!((up >= 0.0) && (up <= (double)(nP - 1)))) return false;
+    const int kp = min((int)floor(up), nP - 2);
+    double wv[4], wd[4];
+    sb::phase_weights(up - (double)kp, (kp == 0) || (kp == nP - 2), 1.0, wv, wd);
+    rb = min(max(kp - 1, 0), nP - 4);
+    const int shift = (kp - 1) - rb; // row rb + k carries Keys weight index k - shift
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int src = k - shift;
+        double w = 0.0;
+        if (src == 0) w = wv[0];
+        if (src == 1) w = wv[1];
+        if (src == 2) w = wv[2];
+        if (src == 3) w = wv[3];
+        wrow[k] = w;
+    }
+    return true;
+}
+
+// ---- the kernel ---------------------------------------------------------------------------------
+template <int NCL>
+__global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_constant__ SbHParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr unsigned FULL = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const SbModelParams &mp = P.mp;
+    const TSmem L(P.n_band_total, P.cap);
+    float *s_at = reinterpret_cast<float *>(smem_raw + L.at);
+    float4 *s_ws = reinterpret_cast<float4 *>(smem_raw + L.ws);
+    float *s_w = reinterpret_cast<float *>(smem_raw + L.w);
+    float *res = reinterpret_cast<float *>(smem_raw + L.res);
+    uint32_t *s_info = reinterpret_cast<uint32_t *>(smem_raw + L.info);
+    uint16_t *s_key = reinterpret_cast<uint16_t *>(smem_raw + L.key);
+    int *hist = reinterpret_cast<int *>(smem_raw + L.hist);
+    int *bstart = reinterpret_cast<int *>(smem_raw + L.bstart);
+    HSeg *segs = reinterpret_cast<HSeg *>(smem_raw + L.segs);
+    HUnitTmp *utmp = reinterpret_cast<HUnitTmp *>(smem_raw + L.utmp);
+    TItem *items = reinterpret_cast<TItem *>(smem_raw + L.items);
+    int *win = reinterpret_cast<int *>(smem_raw + L.win);               // [0..kSlots) lowest node, [kSlots..) end node per band of the stage
+    int *misc = reinterpret_cast<int *>(smem_raw + L.misc);             // [0] group, [1] n_seg, [2] n_ev, [3] next unit, [4] next offset, [5] window segments
+    double *carry = reinterpret_cast<double *>(smem_raw + L.misc + 32); // chi^2 of a unit split over rounds
+
+    for (int i = tid; i < P.n_band_total; i += kThreads) s_w[i] = __ldg(P.band_w + i);
+    const long long n_units = (long long)P.n_sn * P.n_samples;
+    const int G = P.group_units, CAP = P.cap;
+    const long long n_groups = (n_units + G - 1) / G;
+    const bool want_chi = P.out_chi2 != nullptr;
+    const int nP = mp.n_phase, n_bands = P.n_bands;
+    const int nq = max(1, min(nP - 3, kBins / n_bands)); // phase-row bins per band
+    constexpr uint16_t kNoKey = 0xffffu;
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) misc[0] = (int)atomicAdd(P.counter, 1u);
+        __syncthreads();
+        const long long group = (long long)(unsigned)misc[0];
+        if (group >= n_groups) break;
+        const long long pos0 = group * G;
+        const int npos = (int)min((long long)G, n_units - pos0);
+        if (tid < npos) { // unit -> supernova (z-ordered), observation range
+            const long long pos = pos0 + tid;
+            const int si = (int)(pos / P.n_samples);
+            const int ks = (int)(pos - (long long)si * P.n_samples);
+            const int sn = P.perm ? __ldg(P.perm + si) : si;
+            HUnitTmp t;
+            t.sn = sn;
+            t.unit = sn * P.n_samples + ks;
+            t.o_lo = __ldg(P.obs_offset + sn);
+            t.n = __ldg(P.obs_offset + sn + 1) - t.o_lo;
+            utmp[tid] = t;
+        }
+        if (tid == 0) { misc[3] = 0; misc[4] = 0; }
+        __syncthreads();
+
+        for (;;) {
+            const int cur_u = misc[3];
+            __syncthreads();
+            if (cur_u >= npos) break;
+            // ---- round: consecutive units whose observations fit the result array (a unit larger
+            // than the array is processed alone, CAP observations at a time)
+            if (tid == 0) {
+                int u = misc[3], off = misc[4], n_ev = 0, n_seg = 0;
+                while (u < npos && n_seg < kMaxSeg) {
+                    const int rem = utmp[u].n - off;
+                    HSeg &S = segs[n_seg];
+                    if (rem <= CAP - n_ev) {
+                        S.unit = u; S.o_lo = off; S.n = rem; S.e_begin = n_ev; S.first = (off == 0); S.last = 1;
+                        n_ev += rem; ++n_seg; ++u; off = 0;
+                    } else if (n_ev == 0) {
+                        S.unit = u; S.o_lo = off; S.n = CAP; S.e_begin = 0; S.first = (off == 0); S.last = 0;
+                        n_ev = CAP; ++n_seg; off += CAP;
+                        break;
+                    } else {
+                        break;
+                    }
+                }
+                misc[1] = n_seg; misc[2] = n_ev; misc[3] = u; misc[4] = off;
+            }
+            for (int i = tid; i < kBins; i += kThreads) hist[i] = 0;
+            __syncthreads();
+            const int n_seg = misc[1], n_ev = misc[2];
+            if (tid < n_seg) { // segment parameters (S.unit / S.o_lo hold group-local values until here)
+                HSeg &S = segs[tid];
+                const HUnitTmp t = utmp[S.unit];
+                const int off = S.o_lo;
+                const int ks = t.unit - t.sn * P.n_samples;
+                S.unit = t.unit;
+                S.sn = t.sn;
+                S.o_lo = t.o_lo + off;
+                S.out_base = (long long)t.o_lo * P.n_samples + (long long)ks * t.n + off;
+                const double z = (double)__ldg(P.z + t.sn);
+                const double cc = (double)__ldg(P.c + t.unit);
+                S.opz = 1.0 + z;
+                S.inv_opz = 1.0 / S.opz;
+                S.x0 = (double)__ldg(P.x0 + t.unit);
+                S.x1 = __ldg(P.x1 + t.unit);
+                S.t0 = (double)__ldg(P.t0 + t.unit);
+                S.cc = cc;
+                const double cscale = cc * 1.4426950408889634; // exponent in log2 units (ex2)
+#pragma unroll
+                for (int q = 0; q < SB_MAX_CL; ++q) S.cl[q] = (float)(mp.cl[q] * cscale);
+                S.s_lo = (float)(mp.s_lo * cscale);
+                S.s_hi = (float)(mp.s_hi * cscale);
+                S.p_lo = (float)(mp.p_lo * cscale);
+                S.p_hi = (float)(mp.p_hi * cscale);
+            }
+            for (int e = tid; e < n_ev; e += kThreads) res[e] = 0.f;
+            __syncthreads();
+
+            // ---- a1: counting sort of the round's observations by (band, phase row) ----------------
+            auto seg_of = [&](int e) {
+                int lo = 0, hi = n_seg - 1;
+                while (lo < hi) {
+                    const int mid = (lo + hi + 1) >> 1;
+                    if (segs[mid].e_begin <= e) lo = mid;
+                    else hi = mid - 1;
+                }
+                return lo;
+            };
+            for (int e = tid; e < n_ev; e += kThreads) {
+                const int sg = seg_of(e);
+                const HSeg &S = segs[sg];
+                const int o = S.o_lo + (e - S.e_begin);
+                const int b = __ldg(P.band + o);
+                uint16_t key = kNoKey;
+                if ((unsigned)b < (unsigned)n_bands) {
+                    int rb;
+                    double wrow[4];
+                    if (obs_phase(mp, S, __ldg(P.time + o), rb, wrow)) {
+                        key = (uint16_t)(b * nq + (rb * nq) / (nP - 3));
+                        atomicAdd(&hist[key], 1);
+                    }
+                }
+                s_key[e] = key;
+            }
+            __syncthreads();
+            if (tid < 32) { // exclusive scan of the bins, start of every band's run
+                constexpr int PER = kBins / 32;
+                int s = 0;
+                for (int k = 0; k < PER; ++k) s += hist[tid * PER + k];
+                int incl = s;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int v = __shfl_up_sync(FULL, incl, o);
+                    if (tid >= o) incl += v;
+                }
+                int run = incl - s;
+                for (int k = 0; k < PER; ++k) {
+                    const int c = hist[tid * PER + k];
+                    hist[tid * PER + k] = run;
+                    run += c;
+                }
+                if (tid == 31) bstart[n_bands] = run;
+                __syncwarp();
+                for (int b = tid; b < n_bands; b += 32) bstart[b] = hist[b * nq];
+            }
+            __syncthreads();
+            for (int e = tid; e < n_ev; e += kThreads) {
+                const uint16_t key = s_key[e];
+                if (key == kNoKey) continue;
+                const int sg = seg_of(e);
+                const HSeg &S = segs[sg];
+                const int o = S.o_lo + (e - S.e_begin);
+                int rb = 0;
+                double wrow[4] = {0.0, 0.0, 0.0, 0.0};
+                obs_phase(mp, S, __ldg(P.time + o), rb, wrow);
+                float wsl[4]; // slot s holds the row congruent to s mod 4
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    const int k = (s - rb) & 3;
+                    wsl[s] = (float)(k == 0 ? wrow[0] : k == 1 ? wrow[1] : k == 2 ? wrow[2] : wrow[3]);
+                }
+                const int pos = atomicAdd(&hist[key], 1);
+                s_ws[pos] = make_float4(wsl[0], wsl[1], wsl[2], wsl[3]);
+                s_info[pos] = (uint32_t)sg | ((uint32_t)rb << 5) | ((uint32_t)e << 17);
+            }
+            __syncthreads();
+
+            // ---- stages: as many whole bands as fit the item slots -----------------------------------
+            const int bps = max(1, kSlots / n_seg); // bands per stage
+            for (int b0 = 0; b0 < n_bands; b0 += bps) {
+                const int nbs = min(bps, n_bands - b0);
+                const int n_items = nbs * n_seg;
+                if (bstart[b0 + nbs] == bstart[b0]) continue; // no observation in these bands (CTA-uniform)
+                if (tid == 0) misc[5] = 0;
+                __syncthreads();
+                if (tid < n_items) { // geometry of item (band b0 + tid / n_seg, segment tid % n_seg)
+                    const int bl = tid / n_seg, sg = tid - bl * n_seg;
+                    TItem &I = items[tid];
+                    I.n_in = 0; I.n_pass = 0; I.lenw = 0; I.nbw = 0;
+                    if (bstart[b0 + bl + 1] > bstart[b0 + bl] && segs[sg].n > 0) item_geometry(P, segs[sg], b0 + bl, I);
+                    if (I.n_pass > 0) atomicMax(&misc[5], (I.n_pass + kPassSeg - 1) / kPassSeg);
+                }
+                __syncthreads();
+                const int n_wseg = misc[5];
+                for (int wseg = 0; wseg < n_wseg; ++wseg) {
+                    if (tid < nbs) { win[tid] = 0x7fffffff; win[kSlots + tid] = -0x7fffffff; }
+                    __syncthreads();
+                    // phase A: node weights of every item
+                    for (int it = warp; it < n_items; it += kWarps) {
+                        TItem &I = items[it];
+                        const int bl = it / n_seg, sg = it - bl * n_seg;
+                        phase_a_item<NCL>(mp, segs[sg], I, wseg, s_w, s_at + (size_t)it * kW, lane);
+                        __syncwarp();
+                        if (lane == 0 && I.lenw > 0) {
+                            atomicMin(&win[bl], I.nbw);
+                            atomicMax(&win[kSlots + bl], I.nbw + I.lenw);
+                        }
+                    }
+                    __syncthreads();
+                    // phase B: contraction with the model rows, observations in (band, phase row) order
+                    for (int bl = 0; bl < nbs; ++bl) {
+                        const int w_lo = win[bl], w_hi = win[kSlots + bl];
+                        if (w_lo >= w_hi) continue;
+                        const int lo = bstart[b0 + bl], n = bstart[b0 + bl + 1] - lo;
+                        const int per = (((n + kWarps - 1) / kWarps) + 3) & ~3;
+                        const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
+                        if (i_lo < i_hi)
+                            phase_b_chunk(P, segs, items + bl * n_seg, s_at, bl * n_seg, s_ws, s_info, res, i_lo, i_hi,
+                                          w_lo, w_hi, lane);
+                    }
+                    __syncthreads();
+                }
+            }
+            __syncthreads();
+
+            // ---- epilogue: one warp per segment; a6 zero point (fp64), flux out (coalesced), a7 chi^2
+            for (int sg = warp; sg < n_seg; sg += kWarps) {
+                const HSeg &S = segs[sg];
+                double sum = 0.0;
+                for (int i = lane; i < S.n; i += 32) {
+                    const int o = S.o_lo + i;
+                    const int b = __ldg(P.band + o);
+                    double m;
+                    if ((unsigned)b >= (unsigned)P.n_bands) {
+                        m = __longlong_as_double(0x7ff8000000000000LL);
+                    } else {
+                        double sc = 1.0;
+                        if (P.zp != nullptr) sc = exp10(0.4 * (double)__ldg(P.zp + o)) * __ldg(P.band_zpab_inv + b);
+                        m = sc * S.x0 * (double)res[S.e_begin + i];
+                    }
+                    if (P.out_flux) P.out_flux[S.out_base + i] = (float)m;
+                    if (want_chi) {
+                        const double f = (double)__ldg(P.flux + o), e = (double)__ldg(P.fluxerr + o);
+                        const double qv = (f - m) / e;
+                        sum += qv * qv;
+                    }
+                }
+                if (want_chi) {
+                    sum = sb::warp_sum(sum);
+                    if (lane == 0) {
+                        const double total = (S.first ? 0.0 : *carry) + sum;
+                        if (S.last) P.out_chi2[S.unit] = (float)total;
+                        else *carry = total;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+} // namespace sbt

@@ -29,7 +29,7 @@ def run_gpu(wl, *, mode: str = "chi2", fp64: bool = False, theta: Optional[Dict[
     dev = torch.device("cuda:0")
     ft = torch.float64 if fp64 else torch.float32
     dt = sb.SB_F64 if fp64 else sb.SB_F32
-    dt |= {None: 0, "direct": sb.SB_FORM_DIRECT, "grouped": sb.SB_FORM_GROUPED}[form]
+    dt |= {None: 0, "direct": sb.SB_FORM_DIRECT, "grouped": sb.SB_FORM_GROUPED, "tiled": sb.SB_FORM_TILED}[form]
     model, bands = handles if handles is not None else load_handles(wl)
     th = wl.theta if theta is None else theta
     n_units = len(th["x0"])
@@ -72,6 +72,7 @@ def run_gpu(wl, *, mode: str = "chi2", fp64: bool = False, theta: Optional[Dict[
         raise ValueError(mode)
     torch.cuda.synchronize()
     out["launches"] = sb.last_launch_count()
+    out["form"] = sb.last_form()
     if o_flux is not None:
         out["flux"] = o_flux.double().cpu().numpy()
     return out

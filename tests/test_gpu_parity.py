@@ -145,7 +145,7 @@ def test_no_zero_point_is_raw_photon_flux(cuda_device):
     assert np.all(np.abs(got["flux"] - want) <= 1e-5 * np.abs(want) + 1e-9 * np.max(np.abs(want)))
 
 
-@pytest.mark.parametrize("form", ["direct", "grouped"])
+@pytest.mark.parametrize("form", ["direct", "grouped", "tiled"])
 @pytest.mark.parametrize("config,kw", [(2, {"n_sn": 257, "ragged": True}), (3, {"n_samples": 200}), (5, {"n_sn": 200})])
 def test_each_formulation_against_oracle(cuda_device, form, config, kw):
     """include/saltband.h SB_FORM_*: the per-evaluation kernel and the band-grouped kernel are both
@@ -153,5 +153,5 @@ def test_each_formulation_against_oracle(cuda_device, form, config, kw):
     wl = prepare(config, **kw)
     ref = oracle_all(wl)
     got = sbgpu.run_gpu(wl, mode="chi2", form=form)
-    assert got["launches"] == (2 if form == "grouped" else 1)
+    assert got["launches"] == (1 if form == "direct" else 2) and got["form"] == form
     check_flux_chi2(wl, got, ref, False)
