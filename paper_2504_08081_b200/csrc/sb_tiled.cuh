@@ -52,15 +52,13 @@ struct TItem {
     int32_t g_first; // first cell
     int32_t wbase;   // index of the first in-range sample in the staged weight table
     int32_t cmode;
-    int32_t nb0;     // first node of the item's window (multiple of 4, >= -4)
-    int32_t n_pass;  // 32-node passes of the whole window
-    int32_t nbw;     // first node held in the slot for the current window segment
-    int32_t lenw;    // nodes held in the slot (multiple of 32; 0: none)
+    int32_t n_lo;    // first node that carries a weight (g_first - 1, >= -1)
+    int32_t n_end;   // one past the last node that carries a weight (g_last + 3)
     float c0, ha_hi, ha_lo, inv_ha, hal, r_first, lin_a, lin_b;
 };
 
 struct TSmem {
-    size_t w, at, res, ws, info, key, hist, bstart, segs, utmp, items, win, misc, total;
+    size_t w, at, res, ws, info, key, hist, bstart, segs, utmp, items, win, x1, misc, total;
     __host__ __device__ TSmem(int n_band_total, int cap)
     {
         size_t o = 0;
@@ -75,8 +73,9 @@ struct TSmem {
         o = (o + 15) & ~(size_t)15;
         segs = o; o += (size_t)kMaxSeg * sizeof(HSeg);
         utmp = o; o += (size_t)kMaxSeg * sizeof(HUnitTmp);
-        items = o; o += (size_t)kSlots * sizeof(TItem);
-        win = o; o += (size_t)2 * kSlots * sizeof(int32_t);
+        items = o; o += (size_t)2 * kSlots * sizeof(TItem);       // double buffered over stages
+        win = o; o += (size_t)2 * 2 * kSlots * sizeof(int32_t);    // [buffer][lo | end][band of the stage]
+        x1 = o; o += (size_t)2 * kSlots * sizeof(float);          // [buffer][item slot]
         misc = o; o += 64;
         total = o;
     }
@@ -91,9 +90,8 @@ __device__ __forceinline__ void item_geometry(const SbHParams &P, const HSeg &S,
     const SbModelParams &mp = P.mp;
     const int nW = mp.n_wave;
     I.n_in = 0;
-    I.n_pass = 0;
-    I.lenw = 0;
-    I.nbw = 0;
+    I.n_lo = 0;
+    I.n_end = 0;
     const int boff = __ldg(P.band_off + b);
     const int nb = __ldg(P.band_off + b + 1) - boff;
     const double lam_first = __ldg(P.band_lam_first + b);
@@ -148,27 +146,23 @@ __device__ __forceinline__ void item_geometry(const SbHParams &P, const HSeg &S,
         I.lin_a = (float)((double)S.p_lo - (double)S.s_lo * mp.r_lo);
     }
     I.cmode = cmode;
-    // window of nodes g_first-1 .. g_last+2, first node aligned down to a multiple of 4
-    I.nb0 = (g_first - 1) & ~3;
-    I.n_pass = (g_last + 2 - I.nb0) / 32 + 1;
+    I.n_lo = g_first - 1; // nodes g_first-1 .. g_last+2 carry weights
+    I.n_end = g_last + 3;
 }
 
-// ---- phase A: node weights of one item for window segment wseg -> At slot (one warp) -------------
-// Pass q: lane l <-> NODE nb0 + 32 q + l and <-> CELL node + 1.  Node n takes w_{-1} of cell n+1 (this
-// lane), w_0 of cell n (lane - 1), w_1 of cell n-1 (lane - 2) and w_2 of cell n-2 (lane - 3); lanes
-// 0..2 take them from the previous pass (carried in registers; for wseg > 0 the pass before the
-// segment is recomputed for its carries only).
-template <int NCL>
-__device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg &S, TItem &I, int wseg,
-                                             const float *__restrict__ s_w, float *__restrict__ at_slot, int lane)
+// ---- phase A: node weights of one item -> At slot (one warp) --------------------------------------
+// All items of a band use the BAND's node grid: node w_lo + 32 q + l belongs to lane l of pass q, and
+// the slot holds passes [q_lo, q_hi) of it (one window segment).  Lane l also owns CELL node + 1.
+// Node n takes w_{-1} of cell n+1 (this lane), w_0 of cell n (lane - 1), w_1 of cell n-1 (lane - 2)
+// and w_2 of cell n-2 (lane - 3); lanes 0..2 take them from the previous pass (carried in registers;
+// when the segment starts inside the item's window the pass before it is recomputed for its carries).
+// Passes outside the item's own nodes [n_lo, n_end) are zero filled.
+template <int NCL, int CM>
+__device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HSeg &S, const TItem &I, int w_lo,
+                                               int q_start, int q_a, int q_b, int q_lo,
+                                               const float *__restrict__ s_w, float *__restrict__ at_slot, int lane)
 {
     constexpr unsigned FULL = 0xffffffffu;
-    const int q_lo = wseg * kPassSeg;
-    const int q_hi = min(q_lo + kPassSeg, I.n_pass);
-    if (I.n_in == 0 || q_lo >= q_hi) {
-        if (lane == 0) I.lenw = 0;
-        return;
-    }
     HColour<NCL> col;
 #pragma unroll
     for (int q = 0; q < NCL; ++q) col.a[q] = S.cl[q];
@@ -180,44 +174,54 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg
     col.lin_b = I.lin_b;
     const int nW = mp.n_wave;
     const float c0 = I.c0, inv_ha = I.inv_ha, ha_hi = I.ha_hi, ha_lo = I.ha_lo, hal = I.hal, r_first = I.r_first;
-    const int n_in = I.n_in, ncell = I.ncell, cmode = I.cmode;
+    const float ha2 = 2.0f * ha_hi, hal2 = 2.0f * hal;
+    const int n_in = I.n_in, ncell = I.ncell;
     auto jstart = [&](int x) { // first band sample (relative to the first in-range one) of cell x
         int j = (int)ceilf(((float)x - c0) * inv_ha);
-        j = min(max(j, 0), n_in);
-        if (x <= 0) j = 0;
+        j = min(max(j, 0), n_in); // x <= 0 gives j <= 0 because c0 >= 0
         if (x >= ncell) j = n_in;
         return j;
     };
-    const int q_start = q_lo > 0 ? q_lo - 1 : 0;
     float pa0 = 0.f, pa1 = 0.f, pa2 = 0.f;
-    int gq = I.nb0 + 32 * q_start + lane + 1 - I.g_first; // this lane's cell relative to g_first
-    for (int q = q_start; q < q_hi; ++q) {
-        const int js = jstart(gq), je = jstart(gq + 1);
+    int gq = w_lo + 32 * q_start + lane + 1 - I.g_first; // this lane's cell relative to g_first
+    int carry = jstart(gq);                                // lane 0: start of its cell
+    const float *wbase = s_w + I.wbase;
+    float *outp = at_slot + (q_start - q_lo) * 32 + lane;
+#pragma unroll 1
+    for (int q = q_start; q < q_b; ++q) {
+        const int je = jstart(gq + 1);
+        int js = __shfl_up_sync(FULL, je, 1);
+        if (lane == 0) js = carry;
+        carry = __shfl_sync(FULL, je, 31);
         const int cnt = je - js;
         const float jsf = (float)js;
         float tau = __fmaf_rn(jsf, ha_lo, __fmaf_rn(jsf, ha_hi, -(float)gq)) + c0; // u_js - cell
         float r = __fmaf_rn(jsf, hal, r_first);
-        const float *wp = s_w + (I.wbase + js);
+        const float *wp = wbase + js;
         const int km = __reduce_max_sync(FULL, cnt);
         float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-        auto samples = [&](auto cm_tag) {
-            constexpr int CM = decltype(cm_tag)::value;
-            for (int k = 0; k < km; ++k) {
-                float w = 0.f;
-                if (k < cnt) w = wp[k];
-                const float ew = sb::exp_scaled(col.template arg<CM>(r)) * w;
-                const float t2 = tau * tau;
-                s0 += ew;
-                s1 = __fmaf_rn(ew, tau, s1);
-                s2 = __fmaf_rn(ew, t2, s2);
-                s3 = __fmaf_rn(ew, t2 * tau, s3);
-                tau += ha_hi;
-                r += hal;
-            }
-        };
-        if (cmode == sb::CM_INSIDE) samples(std::integral_constant<int, sb::CM_INSIDE>{});
-        else if (cmode == sb::CM_LINEAR) samples(std::integral_constant<int, sb::CM_LINEAR>{});
-        else samples(std::integral_constant<int, sb::CM_GENERIC>{});
+#pragma unroll 1
+        for (int k = 0; k < km; k += 2) { // two samples per trip: independent colour-law chains
+            float w0 = 0.f, w1 = 0.f;
+            if (k < cnt) w0 = wp[0];
+            if (k + 1 < cnt) w1 = wp[1];
+            const float ra = r, rb = r + hal;
+            const float ta = tau, tb = tau + ha_hi;
+            const float ea = sb::exp_scaled(col.template arg<CM>(ra)) * w0;
+            const float eb = sb::exp_scaled(col.template arg<CM>(rb)) * w1;
+            const float ta2 = ta * ta, tb2 = tb * tb;
+            s0 += ea;
+            s1 = __fmaf_rn(ea, ta, s1);
+            s2 = __fmaf_rn(ea, ta2, s2);
+            s3 = __fmaf_rn(ea, ta2 * ta, s3);
+            s0 += eb;
+            s1 = __fmaf_rn(eb, tb, s1);
+            s2 = __fmaf_rn(eb, tb2, s2);
+            s3 = __fmaf_rn(eb, tb2 * tb, s3);
+            tau += ha2;
+            r += hal2;
+            wp += 2;
+        }
         // moments -> weights on the cell's four nodes (Keys a = -1/2; linear in border cells, G2)
         const int g = I.g_first + gq;
         float am = 0.5f * (__fmaf_rn(2.0f, s2, -s3) - s1);
@@ -239,127 +243,151 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg
         pa0 = a0;
         pa1 = a1;
         pa2 = a2;
-        if (q >= q_lo) at_slot[(q - q_lo) * 32 + lane] = at;
+        if (q >= q_a) *outp = at;
+        outp += 32;
         gq += 32;
-    }
-    if (lane == 0) {
-        I.nbw = I.nb0 + 32 * q_lo;
-        I.lenw = 32 * (q_hi - q_lo);
     }
 }
 
-// ---- phase B: the observations [i_lo, i_hi) of the sorted list (all of one band) on one warp ------
-// Node window [S, S + 256): lane l owns nodes S + 4 l .. + 3 and S + 128 + 4 l .. + 3.
+template <int NCL>
+__device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg &S, const TItem &I, int w_lo,
+                                             int q_lo, int q_hi, const float *__restrict__ s_w,
+                                             float *__restrict__ at_slot, int lane)
+{
+    // passes of the band grid that hold nodes of this item
+    int q_a = q_hi, q_b = q_hi, qa = 0;
+    if (I.n_in > 0) {
+        qa = (I.n_lo - w_lo) >> 5;
+        const int qb = (I.n_end - 1 - w_lo) >> 5;
+        q_a = min(max(qa, q_lo), q_hi);
+        q_b = max(min(qb + 1, q_hi), q_a);
+    }
+    for (int q = q_lo; q < q_a; ++q) at_slot[(q - q_lo) * 32 + lane] = 0.f;
+    for (int q = q_b; q < q_hi; ++q) at_slot[(q - q_lo) * 32 + lane] = 0.f;
+    if (q_a >= q_b) return;
+    const int q_start = q_a > qa ? q_a - 1 : q_a;
+    if (I.cmode == sb::CM_INSIDE)
+        phase_a_passes<NCL, sb::CM_INSIDE>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+    else if (I.cmode == sb::CM_LINEAR)
+        phase_a_passes<NCL, sb::CM_LINEAR>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+    else
+        phase_a_passes<NCL, sb::CM_GENERIC>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+}
+
+// ---- phase B: observations [i_lo, i_hi) of the sorted list (all of one band) on one warp ----------
+// Node window of 256 (TWO = true) or 128 nodes starting at node n0, whose weights start at float
+// a_off of every item slot: lane l owns nodes n0 + 4 l .. + 3 and n0 + 128 + 4 l .. + 3.
 struct RowRegs {
     float m0[4][kNPL], m1[4][kNPL]; // [slot = row mod 4][node]
 };
 
+template <bool TWO>
 __device__ __forceinline__ void load_row(RowRegs &R, int s, const float *__restrict__ p0, const float *__restrict__ p1,
-                                         ptrdiff_t rowoff, bool ok_lo, bool ok_hi)
+                                         bool ok_lo, bool ok_hi)
 {
     float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
     if (ok_lo) {
-        a = __ldg(reinterpret_cast<const float4 *>(p0 + rowoff));
-        c = __ldg(reinterpret_cast<const float4 *>(p1 + rowoff));
+        a = __ldg(reinterpret_cast<const float4 *>(p0));
+        c = __ldg(reinterpret_cast<const float4 *>(p1));
     }
-    if (ok_hi) {
-        b = __ldg(reinterpret_cast<const float4 *>(p0 + rowoff + 128));
-        d = __ldg(reinterpret_cast<const float4 *>(p1 + rowoff + 128));
+    if (TWO && ok_hi) {
+        b = __ldg(reinterpret_cast<const float4 *>(p0 + 128));
+        d = __ldg(reinterpret_cast<const float4 *>(p1 + 128));
     }
     R.m0[s][0] = a.x; R.m0[s][1] = a.y; R.m0[s][2] = a.z; R.m0[s][3] = a.w;
-    R.m0[s][4] = b.x; R.m0[s][5] = b.y; R.m0[s][6] = b.z; R.m0[s][7] = b.w;
     R.m1[s][0] = c.x; R.m1[s][1] = c.y; R.m1[s][2] = c.z; R.m1[s][3] = c.w;
-    R.m1[s][4] = d.x; R.m1[s][5] = d.y; R.m1[s][6] = d.z; R.m1[s][7] = d.w;
+    if (TWO) {
+        R.m0[s][4] = b.x; R.m0[s][5] = b.y; R.m0[s][6] = b.z; R.m0[s][7] = b.w;
+        R.m1[s][4] = d.x; R.m1[s][5] = d.y; R.m1[s][6] = d.z; R.m1[s][7] = d.w;
+    }
 }
 
-__device__ __forceinline__ void phase_b_chunk(const SbHParams &P, const HSeg *__restrict__ segs,
-                                              const TItem *__restrict__ items_band, const float *__restrict__ s_at,
-                                              int slot0, const float4 *__restrict__ s_ws,
-                                              const uint32_t *__restrict__ s_info, float *__restrict__ res, int i_lo,
-                                              int i_hi, int w_lo, int w_hi, int lane)
+template <bool TWO>
+__device__ __forceinline__ void phase_b_window(const SbHParams &P, int n0, const float *__restrict__ s_at_l,
+                                               const float *__restrict__ s_x1, const float4 *__restrict__ s_ws,
+                                               const uint32_t *__restrict__ s_info, float *__restrict__ res, int i_lo,
+                                               int i_hi, int lane)
 {
     const int ld = P.mp.ld;
-    for (int S = w_lo; S < w_hi; S += kWinB) {
-        RowRegs R;
-        int held[4] = {-1, -1, -1, -1};
-        const int col = S + SB_PAD_L + 4 * lane; // column of this lane's first node (multiple of 4)
-        const bool ok_lo = col >= 0 && col + 4 <= ld;
-        const bool ok_hi = col + 128 >= 0 && col + 132 <= ld;
-        const float *p0 = P.m0 + col, *p1 = P.m1 + col;
+    RowRegs R;
+    int held[4] = {-1, -1, -1, -1};
+    int rb_held = -1;
+    const int col = n0 + SB_PAD_L + 4 * lane; // column of this lane's first node (multiple of 4)
+    const bool ok_lo = col >= 0 && col + 4 <= ld;
+    const bool ok_hi = col + 128 >= 0 && col + 132 <= ld;
+    const float *p0 = P.m0 + col, *p1 = P.m1 + col;
 #pragma unroll
-        for (int s = 0; s < 4; ++s)
+    for (int s = 0; s < 4; ++s)
 #pragma unroll
-            for (int q = 0; q < kNPL; ++q) { R.m0[s][q] = 0.f; R.m1[s][q] = 0.f; }
+        for (int q = 0; q < kNPL; ++q) { R.m0[s][q] = 0.f; R.m1[s][q] = 0.f; }
 
-        for (int i = i_lo; i < i_hi; i += 4) {
-            float acc[4];
+    auto one = [&](int i) -> float { // the window's share of observation i of the sorted list
+        const uint32_t info = s_info[i];
+        const int slot = (int)(info & 31u), rb = (int)((info >> 5) & 4095u);
+        if (rb != rb_held) { // rows rb .. rb+3, row r in register slot r mod 4: reload only what changed
+            rb_held = rb;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                acc[j] = 0.f;
-                if (i + j >= i_hi) continue;
-                const uint32_t info = s_info[i + j];
-                const int sg = (int)(info & 31u), rb = (int)((info >> 5) & 4095u);
-                const TItem &I = items_band[sg];
-                const int off = S - I.nbw; // multiple of 4
-                const int len = I.lenw;
-                if (len == 0 || off + kWinB <= 0 || off >= len) continue; // the item's nodes do not reach this window
-                // rows rb .. rb+3, row r in slot r mod 4: reload only what changed
-#pragma unroll
-                for (int s = 0; s < 4; ++s) {
-                    const int row = rb + ((s - rb) & 3);
-                    if (held[s] != row) {
-                        load_row(R, s, p0, p1, (ptrdiff_t)row * ld, ok_lo, ok_hi);
-                        held[s] = row;
-                    }
+            for (int s = 0; s < 4; ++s) {
+                const int row = rb + ((s - rb) & 3);
+                if (held[s] != row) {
+                    const ptrdiff_t ro = (ptrdiff_t)row * ld;
+                    load_row<TWO>(R, s, p0 + ro, p1 + ro, ok_lo, ok_hi);
+                    held[s] = row;
                 }
-                const float4 w4 = s_ws[i + j];
-                const float x1 = segs[sg].x1;
-                const float ws[4] = {w4.x, w4.y, w4.z, w4.w};
-                const float vs[4] = {w4.x * x1, w4.y * x1, w4.z * x1, w4.w * x1};
-                const float *ap = s_at + (size_t)(slot0 + sg) * kW;
-                const int o = off + 4 * lane;
-                float a = 0.f;
-                {
-                    float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (o >= 0 && o < len) t = lds128(ap + o);
-                    const float av[4] = {t.x, t.y, t.z, t.w};
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        float r = ws[0] * R.m0[0][q];
-#pragma unroll
-                        for (int s = 1; s < 4; ++s) r = __fmaf_rn(ws[s], R.m0[s][q], r);
-#pragma unroll
-                        for (int s = 0; s < 4; ++s) r = __fmaf_rn(vs[s], R.m1[s][q], r);
-                        a = __fmaf_rn(av[q], r, a);
-                    }
-                }
-                if (off + 128 < len) { // warp-uniform: the upper half of the window holds nodes of the item
-                    const int o2 = o + 128;
-                    float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (o2 >= 0 && o2 < len) t = lds128(ap + o2);
-                    const float av[4] = {t.x, t.y, t.z, t.w};
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        float r = ws[0] * R.m0[0][4 + q];
-#pragma unroll
-                        for (int s = 1; s < 4; ++s) r = __fmaf_rn(ws[s], R.m0[s][4 + q], r);
-#pragma unroll
-                        for (int s = 0; s < 4; ++s) r = __fmaf_rn(vs[s], R.m1[s][4 + q], r);
-                        a = __fmaf_rn(av[q], r, a);
-                    }
-                }
-                acc[j] = a;
-            }
-            // lane L ends with the total of observation i + (L >> 3)
-            const float v = sbh::warp_reduce_transpose<4>(acc, lane);
-            const int jj = lane >> 3;
-            if ((lane & 7) == 0 && i + jj < i_hi) {
-                const int e = (int)(s_info[i + jj] >> 17);
-                res[e] += v;
             }
         }
-        __syncwarp();
+        const float4 w4 = s_ws[i];
+        const float x1 = s_x1[slot];
+        const float ws[4] = {w4.x, w4.y, w4.z, w4.w};
+        const float vs[4] = {w4.x * x1, w4.y * x1, w4.z * x1, w4.w * x1};
+        const float *ap = s_at_l + slot * kW;
+        float a = 0.f;
+        {
+            const float4 t = lds128(ap);
+            const float av[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                float r = ws[0] * R.m0[0][q];
+#pragma unroll
+                for (int s = 1; s < 4; ++s) r = __fmaf_rn(ws[s], R.m0[s][q], r);
+#pragma unroll
+                for (int s = 0; s < 4; ++s) r = __fmaf_rn(vs[s], R.m1[s][q], r);
+                a = __fmaf_rn(av[q], r, a);
+            }
+        }
+        if (TWO) {
+            const float4 t = lds128(ap + 128);
+            const float av[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                float r = ws[0] * R.m0[0][4 + q];
+#pragma unroll
+                for (int s = 1; s < 4; ++s) r = __fmaf_rn(ws[s], R.m0[s][4 + q], r);
+#pragma unroll
+                for (int s = 0; s < 4; ++s) r = __fmaf_rn(vs[s], R.m1[s][4 + q], r);
+                a = __fmaf_rn(av[q], r, a);
+            }
+        }
+        return a;
+    };
+
+    int i = i_lo;
+    for (; i + 4 <= i_hi; i += 4) {
+        float acc[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[j] = one(i + j);
+        const float v = sbh::warp_reduce_transpose<4>(acc, lane); // lane L: total of observation i + (L >> 3)
+        if ((lane & 7) == 0) res[s_info[i + (lane >> 3)] >> 17] += v;
     }
+    if (i < i_hi) {
+        float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+            if (i + j < i_hi) acc[j] = one(i + j);
+        const float v = sbh::warp_reduce_transpose<4>(acc, lane);
+        if ((lane & 7) == 0 && i + (lane >> 3) < i_hi) res[s_info[i + (lane >> 3)] >> 17] += v;
+    }
+    __syncwarp();
 }
 
 // Phase of observation o of segment S: first loaded phase row rb (rows rb .. rb+3) and the weights of
@@ -408,9 +436,10 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
     int *bstart = reinterpret_cast<int *>(smem_raw + L.bstart);
     HSeg *segs = reinterpret_cast<HSeg *>(smem_raw + L.segs);
     HUnitTmp *utmp = reinterpret_cast<HUnitTmp *>(smem_raw + L.utmp);
-    TItem *items = reinterpret_cast<TItem *>(smem_raw + L.items);
-    int *win = reinterpret_cast<int *>(smem_raw + L.win);               // [0..kSlots) lowest node, [kSlots..) end node per band of the stage
-    int *misc = reinterpret_cast<int *>(smem_raw + L.misc);             // [0] group, [1] n_seg, [2] n_ev, [3] next unit, [4] next offset, [5] window segments
+    TItem *items_all = reinterpret_cast<TItem *>(smem_raw + L.items);   // [2][kSlots]
+    int *win_all = reinterpret_cast<int *>(smem_raw + L.win);           // [2][lo: kSlots | end: kSlots]
+    float *x1_all = reinterpret_cast<float *>(smem_raw + L.x1);         // [2][kSlots]
+    int *misc = reinterpret_cast<int *>(smem_raw + L.misc);             // [0] group, [1] n_seg, [2] n_ev, [3] next unit, [4] next offset
     double *carry = reinterpret_cast<double *>(smem_raw + L.misc + 32); // chi^2 of a unit split over rounds
 
     for (int i = tid; i < P.n_band_total; i += kThreads) s_w[i] = __ldg(P.band_w + i);
@@ -548,6 +577,7 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                 for (int b = tid; b < n_bands; b += 32) bstart[b] = hist[b * nq];
             }
             __syncthreads();
+            const int bps = max(1, kSlots / n_seg); // bands per stage
             for (int e = tid; e < n_ev; e += kThreads) {
                 const uint16_t key = s_key[e];
                 if (key == kNoKey) continue;
@@ -557,65 +587,98 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                 int rb = 0;
                 double wrow[4] = {0.0, 0.0, 0.0, 0.0};
                 obs_phase(mp, S, __ldg(P.time + o), rb, wrow);
-                float wsl[4]; // slot s holds the row congruent to s mod 4
+                float wsl[4]; // register slot s holds the row congruent to s mod 4
 #pragma unroll
                 for (int s = 0; s < 4; ++s) {
                     const int k = (s - rb) & 3;
                     wsl[s] = (float)(k == 0 ? wrow[0] : k == 1 ? wrow[1] : k == 2 ? wrow[2] : wrow[3]);
                 }
+                const int b = (int)key / nq;
+                const int slot = (b % bps) * n_seg + sg; // item slot inside the band's stage
                 const int pos = atomicAdd(&hist[key], 1);
                 s_ws[pos] = make_float4(wsl[0], wsl[1], wsl[2], wsl[3]);
-                s_info[pos] = (uint32_t)sg | ((uint32_t)rb << 5) | ((uint32_t)e << 17);
+                s_info[pos] = (uint32_t)slot | ((uint32_t)rb << 5) | ((uint32_t)e << 17);
             }
-            __syncthreads();
 
-            // ---- stages: as many whole bands as fit the item slots -----------------------------------
-            const int bps = max(1, kSlots / n_seg); // bands per stage
-            for (int b0 = 0; b0 < n_bands; b0 += bps) {
-                const int nbs = min(bps, n_bands - b0);
-                const int n_items = nbs * n_seg;
-                if (bstart[b0 + nbs] == bstart[b0]) continue; // no observation in these bands (CTA-uniform)
-                if (tid == 0) misc[5] = 0;
-                __syncthreads();
-                if (tid < n_items) { // geometry of item (band b0 + tid / n_seg, segment tid % n_seg)
+            // ---- stages: as many whole bands as fit the item slots; the small per-stage state (items,
+            // band windows, x1) is double buffered so that the geometry of stage s+1 is computed behind
+            // phase B of stage s: two CTA barriers per stage and window segment.
+            const int n_stage = (n_bands + bps - 1) / bps;
+            auto stage_reset = [&](int buf) { // band windows of a buffer: empty
+                int *win = win_all + buf * 2 * kSlots;
+                if (tid < kSlots) { win[tid] = 0x7fffffff; win[kSlots + tid] = -0x7fffffff; }
+            };
+            auto stage_geometry = [&](int buf, int st) { // items of stage st, union window of every band
+                if (st >= n_stage) return;
+                const int b0 = st * bps, nbs = min(bps, n_bands - b0), n_items = nbs * n_seg;
+                if (tid < n_items) {
                     const int bl = tid / n_seg, sg = tid - bl * n_seg;
-                    TItem &I = items[tid];
-                    I.n_in = 0; I.n_pass = 0; I.lenw = 0; I.nbw = 0;
+                    TItem &I = items_all[buf * kSlots + tid];
+                    int *win = win_all + buf * 2 * kSlots;
+                    I.n_in = 0; I.n_lo = 0; I.n_end = 0;
                     if (bstart[b0 + bl + 1] > bstart[b0 + bl] && segs[sg].n > 0) item_geometry(P, segs[sg], b0 + bl, I);
-                    if (I.n_pass > 0) atomicMax(&misc[5], (I.n_pass + kPassSeg - 1) / kPassSeg);
+                    if (I.n_in > 0) {
+                        atomicMin(&win[bl], I.n_lo & ~3); // multiple of 4: 16-byte aligned row loads
+                        atomicMax(&win[kSlots + bl], I.n_end);
+                    }
+                    x1_all[buf * kSlots + tid] = segs[sg].x1;
                 }
-                __syncthreads();
-                const int n_wseg = misc[5];
-                for (int wseg = 0; wseg < n_wseg; ++wseg) {
-                    if (tid < nbs) { win[tid] = 0x7fffffff; win[kSlots + tid] = -0x7fffffff; }
-                    __syncthreads();
-                    // phase A: node weights of every item
-                    for (int it = warp; it < n_items; it += kWarps) {
-                        TItem &I = items[it];
-                        const int bl = it / n_seg, sg = it - bl * n_seg;
-                        phase_a_item<NCL>(mp, segs[sg], I, wseg, s_w, s_at + (size_t)it * kW, lane);
-                        __syncwarp();
-                        if (lane == 0 && I.lenw > 0) {
-                            atomicMin(&win[bl], I.nbw);
-                            atomicMax(&win[kSlots + bl], I.nbw + I.lenw);
+            };
+            stage_reset(0);
+            __syncthreads(); // sorted records, bstart and the reset are visible
+            stage_geometry(0, 0);
+            __syncthreads();
+            for (int st = 0; st < n_stage; ++st) {
+                const int buf = st & 1;
+                const int b0 = st * bps, nbs = min(bps, n_bands - b0), n_items = nbs * n_seg;
+                const TItem *items = items_all + buf * kSlots;
+                const int *win = win_all + buf * 2 * kSlots;
+                const float *s_x1 = x1_all + buf * kSlots;
+                int n_wseg = 0; // window segments of kW nodes: the widest band of the stage decides
+                for (int bl = 0; bl < nbs; ++bl) {
+                    const int len = win[kSlots + bl] - win[bl];
+                    if (len > 0) n_wseg = max(n_wseg, (len + kW - 1) / kW);
+                }
+                const int n_step = max(n_wseg, 1);
+                for (int wseg = 0; wseg < n_step; ++wseg) {
+                    if (wseg == 0) stage_reset(buf ^ 1);
+                    // phase A: node weights of every item on its band's node grid
+                    if (wseg < n_wseg) {
+                        for (int it = warp; it < n_items; it += kWarps) {
+                            const int bl = it / n_seg, sg = it - bl * n_seg;
+                            const int w_lo = win[bl], len = win[kSlots + bl] - w_lo;
+                            if (len <= 0) continue;
+                            const int np_b = (len + 31) >> 5;
+                            const int q_lo = wseg * kPassSeg, q_hi = min(q_lo + kPassSeg, np_b);
+                            if (q_lo >= q_hi) continue;
+                            phase_a_item<NCL>(mp, segs[sg], items[it], w_lo, q_lo, q_hi, s_w, s_at + (size_t)it * kW, lane);
                         }
                     }
                     __syncthreads();
                     // phase B: contraction with the model rows, observations in (band, phase row) order
-                    for (int bl = 0; bl < nbs; ++bl) {
-                        const int w_lo = win[bl], w_hi = win[kSlots + bl];
-                        if (w_lo >= w_hi) continue;
-                        const int lo = bstart[b0 + bl], n = bstart[b0 + bl + 1] - lo;
-                        const int per = (((n + kWarps - 1) / kWarps) + 3) & ~3;
-                        const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
-                        if (i_lo < i_hi)
-                            phase_b_chunk(P, segs, items + bl * n_seg, s_at, bl * n_seg, s_ws, s_info, res, i_lo, i_hi,
-                                          w_lo, w_hi, lane);
+                    if (wseg < n_wseg) {
+                        for (int bl = 0; bl < nbs; ++bl) {
+                            const int w_lo = win[bl], len = win[kSlots + bl] - w_lo;
+                            if (len <= 0) continue;
+                            const int np_w = min(kPassSeg, ((len + 31) >> 5) - wseg * kPassSeg);
+                            if (np_w <= 0) continue;
+                            const int lo = bstart[b0 + bl], n = bstart[b0 + bl + 1] - lo;
+                            const int per = (((n + kWarps - 1) / kWarps) + 3) & ~3;
+                            const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
+                            if (i_lo >= i_hi) continue;
+                            const int n_half = (np_w * 32 + 127) >> 7; // 128-node halves of this segment
+                            for (int h0 = 0; h0 < n_half; h0 += 2) {
+                                const int n0 = w_lo + wseg * kW + 128 * h0;
+                                const float *at_l = s_at + 128 * h0 + 4 * lane;
+                                if (h0 + 1 < n_half) phase_b_window<true>(P, n0, at_l, s_x1, s_ws, s_info, res, i_lo, i_hi, lane);
+                                else phase_b_window<false>(P, n0, at_l, s_x1, s_ws, s_info, res, i_lo, i_hi, lane);
+                            }
+                        }
                     }
+                    if (wseg == n_step - 1) stage_geometry(buf ^ 1, st + 1);
                     __syncthreads();
                 }
             }
-            __syncthreads();
 
             // ---- epilogue: one warp per segment; a6 zero point (fp64), flux out (coalesced), a7 chi^2
             for (int sg = warp; sg < n_seg; sg += kWarps) {

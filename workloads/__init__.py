@@ -14,4 +14,6 @@ from .generators import (  # noqa: F401
     make_colour_law,
     make_model,
     make_workload,
+    shard_bounds,
+    subset,
 )

@@ -333,3 +333,42 @@ def attach_data(wl: Workload, model_flux_true: np.ndarray) -> Workload:
     wl.flux = _f32(m + sigma * wl.noise)
     wl.fluxerr = _f32(sigma)
     return wl
+
+
+def subset(wl: Workload, sn_index) -> Workload:
+    """The supernovae `sn_index` (any order) of `wl` as their own Workload: same tables, the
+    selected observation and parameter slices copied in that order.  Index bookkeeping only."""
+    idx = np.asarray(sn_index, dtype=np.int64)
+    ns = wl.n_samples
+    n_obs = np.diff(wl.obs_offset).astype(np.int64)
+    off = np.zeros(len(idx) + 1, dtype=np.int64)
+    off[1:] = np.cumsum(n_obs[idx])
+    if len(idx):
+        sel = np.concatenate([np.arange(wl.obs_offset[s], wl.obs_offset[s + 1], dtype=np.int64) for s in idx])
+    else:
+        sel = np.zeros(0, dtype=np.int64)
+    usel = (idx[:, None] * ns + np.arange(ns, dtype=np.int64)[None, :]).ravel()
+    sub = Workload(
+        config=wl.config, name=f"{wl.name}[subset {len(idx)}]", model=wl.model, bands=wl.bands, n_sn=len(idx),
+        n_samples=ns, obs_offset=off.astype(np.int32), time=wl.time[sel].copy(), band=wl.band[sel].copy(),
+        zp=wl.zp[sel].copy(), z=wl.z[idx].copy(), theta_true={k: v[idx].copy() for k, v in wl.theta_true.items()},
+        theta={k: v[usel].copy() for k, v in wl.theta.items()}, noise=wl.noise[sel].copy(), meta=dict(wl.meta))
+    if wl.flux is not None:
+        sub.flux, sub.fluxerr = wl.flux[sel].copy(), wl.fluxerr[sel].copy()
+    return sub
+
+
+def shard_bounds(n_sn: int, weight: np.ndarray, world: int):
+    """Contiguous partition of supernovae 0..n_sn over `world` ranks balanced by `weight` (e.g. the
+    observations per supernova): bounds[r] .. bounds[r+1] is rank r's range."""
+    w = np.asarray(weight, dtype=np.float64)
+    if w.shape != (n_sn,):
+        raise ValueError("weight must be [n_sn]")
+    cum = np.concatenate([[0.0], np.cumsum(w)])
+    total = cum[-1]
+    bounds = [0]
+    for r in range(1, world):
+        target = total * r / world
+        bounds.append(int(np.clip(np.searchsorted(cum, target, side="left"), bounds[-1], n_sn)))
+    bounds.append(n_sn)
+    return bounds
