@@ -53,6 +53,9 @@ FLOPS_G_SAMPLE, FLOPS_G_CELL, FLOPS_G_NODE_OBS, FLOPS_G_EVAL = 21, 30, 16, 60
 # with x1 folded into the weights) + 1 FFMA (node weight) = 18.  Only nodes of the item's window count;
 # the zero-padded remainder of the 128-node half windows the kernel also multiplies is not counted.
 FLOPS_T_NODE_OBS = 18
+# Tiled gradient: per sample + CL scaling 1, CL weighting 1, four CL-weighted moments 8 = 31; per cell two
+# weight sets 50; per node per observation 21 FFMA = 42 (value, M1-only, d/dt0 rows, four sums).
+FLOPS_TG_SAMPLE, FLOPS_TG_CELL, FLOPS_TG_NODE_OBS, FLOPS_TG_EVAL = 31, 50, 42, 120
 # SURVEY.md section 8(d) "direct (G = 1)" model, reported beside ours for reference.
 SURVEY_SAMPLE, SURVEY_NODE, SURVEY_EVAL = 55, 18, 40
 SURVEY_SAMPLE_GRAD, SURVEY_NODE_GRAD, SURVEY_EVAL_GRAD = 77, 36, 100
@@ -103,6 +106,13 @@ def flops_per_call(wl, grad: bool, form: str = "direct"):
     n_in, n_cell = geometry_counts(wl)
     ns = wl.n_samples
     s_in, s_cell, n_ev = float(n_in.sum()) * ns, float(n_cell.sum()) * ns, float(wl.n_evals)
+    if form == "tiled" and grad:
+        share = chunk_share(wl, 0)
+        g_in, g_cell = float((n_in * share).sum()) * ns, float((n_cell * share).sum()) * ns
+        s_node = float((n_cell + 3 * (n_cell > 0)).sum()) * ns
+        ours = g_in * FLOPS_TG_SAMPLE + g_cell * FLOPS_TG_CELL + s_node * FLOPS_TG_NODE_OBS + n_ev * FLOPS_TG_EVAL
+        surv = s_in * SURVEY_SAMPLE_GRAD + (s_cell + 3 * n_ev) * SURVEY_NODE_GRAD + n_ev * SURVEY_EVAL_GRAD
+        return ours, surv, s_in / max(n_ev, 1.0), s_cell / max(n_ev, 1.0)
     if form in ("grouped", "tiled") and not grad:
         share = chunk_share(wl, 8 if form == "grouped" else 0)
         node_obs = FLOPS_G_NODE_OBS if form == "grouped" else FLOPS_T_NODE_OBS
@@ -440,7 +450,7 @@ def main():
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
         "traffic": None,
-        "kernel": {"grouped": "sb_hoist_kernel<fwd>", "tiled": "sb_tiled_kernel<fwd>"}.get(
+        "kernel": {"grouped": "sb_hoist_kernel<fwd>", "tiled": "sb_tiled_kernel<%s>" % ("grad" if grad else "fwd")}.get(
             form_run, "sb_fused_kernel<float,%s>" % ("grad" if grad else "fwd")),
         "form": form_run,
         "kernel_ms": kernel_ms, "flops_per_eval": flops_ours / n_ev, "peak_source": peak_src,

@@ -344,9 +344,11 @@ int launch_typed(SbKParams &kp, const sb_bands *b, int n_obs_total, cudaStream_t
 // Band-grouped kernels: fp32 forward, uniform band grids.  tiled = true: sb_tiled.cuh (register-tiled
 // node contraction), false: sb_hoist.cuh.  Returns 1 when the kernel is not applicable (the caller
 // then tries the next formulation), SB_OK or an error otherwise.
-int launch_grouped(bool tiled, const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux,
-                   const void *fluxerr, void *out_flux, void *out_chi2, cudaStream_t st)
+int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux,
+                   const void *fluxerr, void *out_flux, void *out_chi2, void *out_dflux, void *out_dchi2,
+                   cudaStream_t st)
 {
+    if (grad && !tiled) return 1;
     constexpr int NCL = 5;
     if (!b->all_uniform || m->prm.n_cl > NCL || b->n_bands > 64) return 1;
     if (tiled && (m->prm.n_phase < 4 || m->prm.n_phase > 4096)) return 1;
@@ -357,18 +359,19 @@ int launch_grouped(bool tiled, const sb_model *m, const sb_bands *b, const sb_ba
     const long long n_units = (long long)bt->n_sn * bt->n_samples;
     const double mean_obs = bt->n_sn > 0 ? (double)bt->n_obs_total / (double)bt->n_sn : 1.0;
     // units per group: enough groups for every SM (>= 4 per CTA), at most kMaxSeg, about <= cap observations
-    int cap = tiled ? 3072 : 4096;
+    int cap = tiled ? (grad ? 1536 : 3072) : 4096;
     size_t smem = 0;
     if (tiled) {
-        while (cap >= 512 && sbt::TSmem(b->n_total, cap).total > (size_t)smem_max) cap -= 512;
+        while (cap >= 512 && sbt::TSmem(b->n_total, cap, grad).total > (size_t)smem_max) cap -= 256;
         if (cap < 512) return 1;
-        smem = sbt::TSmem(b->n_total, cap).total;
+        smem = sbt::TSmem(b->n_total, cap, grad).total;
     } else {
         smem = sbh::HSmem(b->n_total, cap).total;
         if (smem > (size_t)smem_max || smem > 100 * 1024) return 1;
     }
     long long g = n_units / ((long long)n_sm * 4);
     if (g > sbh::kMaxSeg) g = sbh::kMaxSeg;
+    if (grad && g > sbt::kSlots / 2) g = sbt::kSlots / 2;
     if ((double)g * mean_obs > (double)cap) g = (long long)((double)cap / mean_obs);
     if (g < 1) g = 1;
 
@@ -404,6 +407,8 @@ int launch_grouped(bool tiled, const sb_model *m, const sb_bands *b, const sb_ba
     hp.fluxerr = (const float *)fluxerr;
     hp.out_flux = (float *)out_flux;
     hp.out_chi2 = (float *)out_chi2;
+    hp.out_dflux = (float *)out_dflux;
+    hp.out_dchi2 = (float *)out_dchi2;
     hp.counter = reinterpret_cast<unsigned int *>(ws);
     hp.perm = reinterpret_cast<const int32_t *>(ws + 256);
     hp.group_units = (int)g;
@@ -415,8 +420,12 @@ int launch_grouped(bool tiled, const sb_model *m, const sb_bands *b, const sb_ba
         tl_launches += 1;
         const long long n_groups = (n_units + g - 1) / g;
         const int grid = (int)(n_groups < (long long)n_sm ? n_groups : (long long)n_sm);
-        if (tiled) {
-            auto kern = sbt::sb_tiled_kernel<NCL>;
+        if (tiled && grad) {
+            auto kern = sbt::sb_tiled_kernel<NCL, true>;
+            if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) rc = SB_ECUDA;
+            if (rc == SB_OK) kern<<<grid, sbt::kThreads, smem, st>>>(hp);
+        } else if (tiled) {
+            auto kern = sbt::sb_tiled_kernel<NCL, false>;
             if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) rc = SB_ECUDA;
             if (rc == SB_OK) kern<<<grid, sbt::kThreads, smem, st>>>(hp);
         } else {
@@ -484,13 +493,13 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void 
     kp.out_chi2 = out_chi2;
     kp.out_dchi2 = out_dchi2;
     cudaStream_t st = (cudaStream_t)stream;
-    if (f32 && !grad && form != SB_FORM_DIRECT && bt->n_obs_total > 0) {
+    if (f32 && form != SB_FORM_DIRECT && bt->n_obs_total > 0) {
         if (form != SB_FORM_GROUPED) {
-            const int rc = launch_grouped(true, m, b, bt, flux, fluxerr, out_flux, out_chi2, st);
+            const int rc = launch_grouped(true, grad, m, b, bt, flux, fluxerr, out_flux, out_chi2, out_dflux, out_dchi2, st);
             if (rc != 1) return rc;
         }
-        if (form != SB_FORM_TILED) {
-            const int rc = launch_grouped(false, m, b, bt, flux, fluxerr, out_flux, out_chi2, st);
+        if (form != SB_FORM_TILED && !grad) {
+            const int rc = launch_grouped(false, false, m, b, bt, flux, fluxerr, out_flux, out_chi2, nullptr, nullptr, st);
             if (rc != 1) return rc;
         }
     }

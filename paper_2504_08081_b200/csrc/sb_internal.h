@@ -94,6 +94,7 @@ struct SbHParams {
     const int32_t *band;
     const float *flux, *fluxerr;      // may be NULL
     float *out_flux, *out_chi2;       // may be NULL
+    float *out_dflux, *out_dchi2;     // gradient kernel only; may be NULL
     const int32_t *perm;              // z-ordered supernova indices (workspace) or NULL
     unsigned int *counter;            // group counter (workspace, zeroed by sb_zorder_kernel)
     int32_t group_units;              // units per group (<= 32)

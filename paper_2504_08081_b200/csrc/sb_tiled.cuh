@@ -59,13 +59,15 @@ struct TItem {
 
 struct TSmem {
     size_t w, at, res, ws, info, key, hist, bstart, segs, utmp, items, win, x1, misc, total;
-    __host__ __device__ TSmem(int n_band_total, int cap)
+    // grad: two weight sets per item (value, d/dc) in the same At array (half as many item slots), two
+    // float4 of phase weights (value, d/dt0) and four results per observation
+    __host__ __device__ TSmem(int n_band_total, int cap, bool grad)
     {
         size_t o = 0;
         at = o; o += (size_t)kSlots * kW * sizeof(float);
-        ws = o; o += (size_t)cap * sizeof(float4);
+        ws = o; o += (size_t)cap * sizeof(float4) * (grad ? 2 : 1);
         w = o; o += (size_t)((n_band_total + 3) & ~3) * sizeof(float);
-        res = o; o += (size_t)cap * sizeof(float);
+        res = o; o += (size_t)cap * sizeof(float) * (grad ? 4 : 1);
         info = o; o += (size_t)cap * sizeof(uint32_t);
         hist = o; o += (size_t)kBins * sizeof(int32_t);
         bstart = o; o += (size_t)(kMaxBands + 4) * sizeof(int32_t);
@@ -85,7 +87,8 @@ __device__ __forceinline__ float4 lds128(const float *p) { return *reinterpret_c
 
 // ---- geometry of one item (segment S, band b): one thread.  Same decisions as sbh::run_item: the
 // in-range sample range [j_lo, j_hi) in fp64 (reading G9), the window of model cells, the colour mode.
-__device__ __forceinline__ void item_geometry(const SbHParams &P, const HSeg &S, int b, TItem &I)
+// unscaled = true (gradient kernel): lin_a / lin_b describe CL itself, not CL times c log2(e).
+__device__ __forceinline__ void item_geometry(const SbHParams &P, const HSeg &S, int b, TItem &I, bool unscaled)
 {
     const SbModelParams &mp = P.mp;
     const int nW = mp.n_wave;
@@ -138,12 +141,14 @@ __device__ __forceinline__ void item_geometry(const SbHParams &P, const HSeg &S,
         cmode = sb::CM_INSIDE;
     } else if (r_min >= mp.r_hi + margin) { // arg = p_hi + s_hi (r - r_hi)
         cmode = sb::CM_LINEAR;
-        I.lin_b = S.s_hi;
-        I.lin_a = (float)((double)S.p_hi - (double)S.s_hi * mp.r_hi);
+        const double sl = unscaled ? mp.s_hi : (double)S.s_hi, pv = unscaled ? mp.p_hi : (double)S.p_hi;
+        I.lin_b = (float)sl;
+        I.lin_a = (float)(pv - sl * mp.r_hi);
     } else if (r_max <= mp.r_lo - margin) {
         cmode = sb::CM_LINEAR;
-        I.lin_b = S.s_lo;
-        I.lin_a = (float)((double)S.p_lo - (double)S.s_lo * mp.r_lo);
+        const double sl = unscaled ? mp.s_lo : (double)S.s_lo, pv = unscaled ? mp.p_lo : (double)S.p_lo;
+        I.lin_b = (float)sl;
+        I.lin_a = (float)(pv - sl * mp.r_lo);
     }
     I.cmode = cmode;
     I.n_lo = g_first - 1; // nodes g_first-1 .. g_last+2 carry weights
@@ -157,7 +162,9 @@ __device__ __forceinline__ void item_geometry(const SbHParams &P, const HSeg &S,
 // and w_2 of cell n-2 (lane - 3); lanes 0..2 take them from the previous pass (carried in registers;
 // when the segment starts inside the item's window the pass before it is recomputed for its carries).
 // Passes outside the item's own nodes [n_lo, n_end) are zero filled.
-template <int NCL, int CM>
+// GRAD: the colour law is evaluated unscaled (CL itself; exponent = CL * c log2(e)) and a second set
+// of moments, weighted by CL, gives the node weights of d/dc (at_slot + kW).
+template <int NCL, int CM, bool GRAD>
 __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HSeg &S, const TItem &I, int w_lo,
                                                int q_start, int q_a, int q_b, int q_lo,
                                                const float *__restrict__ s_w, float *__restrict__ at_slot, int lane)
@@ -165,13 +172,14 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
     constexpr unsigned FULL = 0xffffffffu;
     HColour<NCL> col;
 #pragma unroll
-    for (int q = 0; q < NCL; ++q) col.a[q] = S.cl[q];
+    for (int q = 0; q < NCL; ++q) col.a[q] = GRAD ? (float)mp.cl[q] : S.cl[q];
     col.r_lo = (float)mp.r_lo;
     col.r_hi = (float)mp.r_hi;
-    col.s_lo = S.s_lo;
-    col.s_hi = S.s_hi;
+    col.s_lo = GRAD ? (float)mp.s_lo : S.s_lo;
+    col.s_hi = GRAD ? (float)mp.s_hi : S.s_hi;
     col.lin_a = I.lin_a;
     col.lin_b = I.lin_b;
+    const float cs = (float)(S.cc * 1.4426950408889634); // GRAD: exponent in log2 units = CL * cs
     const int nW = mp.n_wave;
     const float c0 = I.c0, inv_ha = I.inv_ha, ha_hi = I.ha_hi, ha_lo = I.ha_lo, hal = I.hal, r_first = I.r_first;
     const float ha2 = 2.0f * ha_hi, hal2 = 2.0f * hal;
@@ -183,6 +191,7 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
         return j;
     };
     float pa0 = 0.f, pa1 = 0.f, pa2 = 0.f;
+    float pc0 = 0.f, pc1 = 0.f, pc2 = 0.f; // GRAD: carries of the d/dc weights
     int gq = w_lo + 32 * q_start + lane + 1 - I.g_first; // this lane's cell relative to g_first
     int carry = jstart(gq);                                // lane 0: start of its cell
     const float *wbase = s_w + I.wbase;
@@ -200,6 +209,7 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
         const float *wp = wbase + js;
         const int km = __reduce_max_sync(FULL, cnt);
         float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+        float d0 = 0.f, d1 = 0.f, d2 = 0.f, d3 = 0.f; // GRAD: moments weighted by CL
 #pragma unroll 1
         for (int k = 0; k < km; k += 2) { // two samples per trip: independent colour-law chains
             float w0 = 0.f, w1 = 0.f;
@@ -207,49 +217,71 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
             if (k + 1 < cnt) w1 = wp[1];
             const float ra = r, rb = r + hal;
             const float ta = tau, tb = tau + ha_hi;
-            const float ea = sb::exp_scaled(col.template arg<CM>(ra)) * w0;
-            const float eb = sb::exp_scaled(col.template arg<CM>(rb)) * w1;
+            const float cla = col.template arg<CM>(ra), clb = col.template arg<CM>(rb);
+            const float ea = sb::exp_scaled(GRAD ? cla * cs : cla) * w0;
+            const float eb = sb::exp_scaled(GRAD ? clb * cs : clb) * w1;
             const float ta2 = ta * ta, tb2 = tb * tb;
+            const float ta3 = ta2 * ta, tb3 = tb2 * tb;
             s0 += ea;
             s1 = __fmaf_rn(ea, ta, s1);
             s2 = __fmaf_rn(ea, ta2, s2);
-            s3 = __fmaf_rn(ea, ta2 * ta, s3);
+            s3 = __fmaf_rn(ea, ta3, s3);
             s0 += eb;
             s1 = __fmaf_rn(eb, tb, s1);
             s2 = __fmaf_rn(eb, tb2, s2);
-            s3 = __fmaf_rn(eb, tb2 * tb, s3);
+            s3 = __fmaf_rn(eb, tb3, s3);
+            if (GRAD) {
+                const float ca = ea * cla, cb = eb * clb;
+                d0 += ca;
+                d1 = __fmaf_rn(ca, ta, d1);
+                d2 = __fmaf_rn(ca, ta2, d2);
+                d3 = __fmaf_rn(ca, ta3, d3);
+                d0 += cb;
+                d1 = __fmaf_rn(cb, tb, d1);
+                d2 = __fmaf_rn(cb, tb2, d2);
+                d3 = __fmaf_rn(cb, tb3, d3);
+            }
             tau += ha2;
             r += hal2;
             wp += 2;
         }
         // moments -> weights on the cell's four nodes (Keys a = -1/2; linear in border cells, G2)
         const int g = I.g_first + gq;
-        float am = 0.5f * (__fmaf_rn(2.0f, s2, -s3) - s1);
-        float a0 = __fmaf_rn(1.5f, s3, __fmaf_rn(-2.5f, s2, s0));
-        float a1 = 0.5f * (__fmaf_rn(4.0f, s2, s1) - 3.0f * s3);
-        float a2 = 0.5f * (s3 - s2);
-        if (g <= 0 || g >= nW - 2) {
-            am = 0.f;
-            a0 = s0 - s1;
-            a1 = s1;
-            a2 = 0.f;
-        }
+        const bool border = g <= 0 || g >= nW - 2;
         auto from_left = [&](float cur, float prev, int d) {
             const float a = __shfl_up_sync(FULL, cur, d);
             const float b = __shfl_sync(FULL, prev, (lane - d) & 31);
             return lane >= d ? a : b;
         };
-        const float at = am + from_left(a0, pa0, 1) + from_left(a1, pa1, 2) + from_left(a2, pa2, 3);
-        pa0 = a0;
-        pa1 = a1;
-        pa2 = a2;
+        auto node_weight = [&](float m0, float m1, float m2, float m3, float &p0, float &p1, float &p2) {
+            float am = 0.5f * (__fmaf_rn(2.0f, m2, -m3) - m1);
+            float a0 = __fmaf_rn(1.5f, m3, __fmaf_rn(-2.5f, m2, m0));
+            float a1 = 0.5f * (__fmaf_rn(4.0f, m2, m1) - 3.0f * m3);
+            float a2 = 0.5f * (m3 - m2);
+            if (border) {
+                am = 0.f;
+                a0 = m0 - m1;
+                a1 = m1;
+                a2 = 0.f;
+            }
+            const float at = am + from_left(a0, p0, 1) + from_left(a1, p1, 2) + from_left(a2, p2, 3);
+            p0 = a0;
+            p1 = a1;
+            p2 = a2;
+            return at;
+        };
+        const float at = node_weight(s0, s1, s2, s3, pa0, pa1, pa2);
         if (q >= q_a) *outp = at;
+        if (GRAD) {
+            const float atc = node_weight(d0, d1, d2, d3, pc0, pc1, pc2);
+            if (q >= q_a) outp[kW] = atc;
+        }
         outp += 32;
         gq += 32;
     }
 }
 
-template <int NCL>
+template <int NCL, bool GRAD>
 __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg &S, const TItem &I, int w_lo,
                                              int q_lo, int q_hi, const float *__restrict__ s_w,
                                              float *__restrict__ at_slot, int lane)
@@ -262,16 +294,24 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg
         q_a = min(max(qa, q_lo), q_hi);
         q_b = max(min(qb + 1, q_hi), q_a);
     }
-    for (int q = q_lo; q < q_a; ++q) at_slot[(q - q_lo) * 32 + lane] = 0.f;
-    for (int q = q_b; q < q_hi; ++q) at_slot[(q - q_lo) * 32 + lane] = 0.f;
+    // zero fill up to a whole 128-node half window: phase B reads the slot in halves
+    const int q_fill = q_lo + (((q_hi - q_lo) + 3) & ~3);
+    for (int q = q_lo; q < q_a; ++q) {
+        at_slot[(q - q_lo) * 32 + lane] = 0.f;
+        if (GRAD) at_slot[kW + (q - q_lo) * 32 + lane] = 0.f;
+    }
+    for (int q = q_b; q < q_fill; ++q) {
+        at_slot[(q - q_lo) * 32 + lane] = 0.f;
+        if (GRAD) at_slot[kW + (q - q_lo) * 32 + lane] = 0.f;
+    }
     if (q_a >= q_b) return;
     const int q_start = q_a > qa ? q_a - 1 : q_a;
     if (I.cmode == sb::CM_INSIDE)
-        phase_a_passes<NCL, sb::CM_INSIDE>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+        phase_a_passes<NCL, sb::CM_INSIDE, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
     else if (I.cmode == sb::CM_LINEAR)
-        phase_a_passes<NCL, sb::CM_LINEAR>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+        phase_a_passes<NCL, sb::CM_LINEAR, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
     else
-        phase_a_passes<NCL, sb::CM_GENERIC>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+        phase_a_passes<NCL, sb::CM_GENERIC, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
 }
 
 // ---- phase B: observations [i_lo, i_hi) of the sorted list (all of one band) on one warp ----------
@@ -390,10 +430,98 @@ __device__ __forceinline__ void phase_b_window(const SbHParams &P, int n0, const
     __syncwarp();
 }
 
+// Gradient variant of phase B: 128-node window (4 nodes per lane), four sums per observation --
+// value, M1-only (d/dx1), CL-weighted node weights (d/dc), phase-derivative weights (d/dt0; the factor
+// -1/((1+z) dP) is folded into the weights) -- PAPER.md:45, 49; BASELINE.json north_star (a8).
+__device__ __forceinline__ void phase_b_window_grad(const SbHParams &P, int n0, const float *__restrict__ s_at_l,
+                                                    const float *__restrict__ s_x1, const float4 *__restrict__ s_ws,
+                                                    const float4 *__restrict__ s_wd,
+                                                    const uint32_t *__restrict__ s_info, float *__restrict__ res,
+                                                    int cap, int i_lo, int i_hi, int lane)
+{
+    const int ld = P.mp.ld;
+    float m0[4][4], m1[4][4]; // [slot = row mod 4][node]
+    int held[4] = {-1, -1, -1, -1};
+    int rb_held = -1;
+    const int col = n0 + SB_PAD_L + 4 * lane;
+    const bool ok = col >= 0 && col + 4 <= ld;
+    const float *p0 = P.m0 + col, *p1 = P.m1 + col;
+#pragma unroll
+    for (int s = 0; s < 4; ++s)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { m0[s][q] = 0.f; m1[s][q] = 0.f; }
+
+    auto one = [&](int i, float *acc) { // acc[0..3] = value, M1-only, d/dc, d/dt0 shares of observation i
+        const uint32_t info = s_info[i];
+        const int slot = (int)(info & 31u), rb = (int)((info >> 5) & 4095u);
+        if (rb != rb_held) {
+            rb_held = rb;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const int row = rb + ((s - rb) & 3);
+                if (held[s] != row) {
+                    const ptrdiff_t ro = (ptrdiff_t)row * ld;
+                    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), c = a;
+                    if (ok) {
+                        a = __ldg(reinterpret_cast<const float4 *>(p0 + ro));
+                        c = __ldg(reinterpret_cast<const float4 *>(p1 + ro));
+                    }
+                    m0[s][0] = a.x; m0[s][1] = a.y; m0[s][2] = a.z; m0[s][3] = a.w;
+                    m1[s][0] = c.x; m1[s][1] = c.y; m1[s][2] = c.z; m1[s][3] = c.w;
+                    held[s] = row;
+                }
+            }
+        }
+        const float4 w4 = s_ws[i], d4 = s_wd[i];
+        const float x1 = s_x1[slot];
+        const float ws[4] = {w4.x, w4.y, w4.z, w4.w};
+        const float wd[4] = {d4.x, d4.y, d4.z, d4.w};
+        const float vd[4] = {d4.x * x1, d4.y * x1, d4.z * x1, d4.w * x1};
+        const float *ap = s_at_l + slot * (2 * kW);
+        const float4 t = lds128(ap), tc = lds128(ap + kW);
+        const float av[4] = {t.x, t.y, t.z, t.w};
+        const float ac[4] = {tc.x, tc.y, tc.z, tc.w};
+        float a = 0.f, a1 = 0.f, a_c = 0.f, a_d = 0.f;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            float r0 = ws[0] * m0[0][q], r1 = ws[0] * m1[0][q], rd = wd[0] * m0[0][q];
+#pragma unroll
+            for (int s = 1; s < 4; ++s) {
+                r0 = __fmaf_rn(ws[s], m0[s][q], r0);
+                r1 = __fmaf_rn(ws[s], m1[s][q], r1);
+                rd = __fmaf_rn(wd[s], m0[s][q], rd);
+            }
+#pragma unroll
+            for (int s = 0; s < 4; ++s) rd = __fmaf_rn(vd[s], m1[s][q], rd);
+            const float r = __fmaf_rn(x1, r1, r0);
+            a = __fmaf_rn(av[q], r, a);
+            a1 = __fmaf_rn(av[q], r1, a1);
+            a_c = __fmaf_rn(ac[q], r, a_c);
+            a_d = __fmaf_rn(av[q], rd, a_d);
+        }
+        acc[0] = a; acc[1] = a1; acc[2] = a_c; acc[3] = a_d;
+    };
+
+    for (int i = i_lo; i < i_hi; i += 4) {
+        float acc[16];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (i + j < i_hi) one(i + j, acc + 4 * j);
+            else { acc[4 * j] = 0.f; acc[4 * j + 1] = 0.f; acc[4 * j + 2] = 0.f; acc[4 * j + 3] = 0.f; }
+        }
+        // lane L ends with value (L >> 1) = 4 * observation + component
+        const float v = sbh::warp_reduce_transpose<16>(acc, lane);
+        const int vi = lane >> 1, j = vi >> 2, comp = vi & 3;
+        if ((lane & 1) == 0 && i + j < i_hi) res[comp * cap + (int)(s_info[i + j] >> 17)] += v;
+    }
+    __syncwarp();
+}
+
 // Phase of observation o of segment S: first loaded phase row rb (rows rb .. rb+3) and the weights of
 // those rows (Keys a = -1/2, linear in the border cells -- readings G1, G2), scalar work in fp64.
 // Returns false when the phase is outside the grid (zero flux, reading G3).
-__device__ __forceinline__ bool obs_phase(const SbModelParams &mp, const HSeg &S, float t, int &rb, double (&wrow)[4])
+__device__ __forceinline__ bool obs_phase(const SbModelParams &mp, const HSeg &S, float t, int &rb, double (&wrow)[4],
+                                          double (&drow)[4])
 {
     const int nP = mp.n_phase;
     const double p = ((double)t - S.t0) * S.inv_opz;
@@ -401,31 +529,37 @@ __device__ __forceinline__ bool obs_phase(const SbModelParams &mp, const HSeg &S
     if (!((up >= 0.0) && (up <= (double)(nP - 1)))) return false;
     const int kp = min((int)floor(up), nP - 2);
     double wv[4], wd[4];
-    sb::phase_weights(up - (double)kp, (kp == 0) || (kp == nP - 2), 1.0, wv, wd);
+    // d/dt0 of the weights: d tau/d t0 = -1/((1+z) dP)
+    sb::phase_weights(up - (double)kp, (kp == 0) || (kp == nP - 2), -S.inv_opz / mp.dp, wv, wd);
     rb = min(max(kp - 1, 0), nP - 4);
     const int shift = (kp - 1) - rb; // row rb + k carries Keys weight index k - shift
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const int src = k - shift;
-        double w = 0.0;
-        if (src == 0) w = wv[0];
-        if (src == 1) w = wv[1];
-        if (src == 2) w = wv[2];
-        if (src == 3) w = wv[3];
+        double w = 0.0, d = 0.0;
+        if (src == 0) { w = wv[0]; d = wd[0]; }
+        if (src == 1) { w = wv[1]; d = wd[1]; }
+        if (src == 2) { w = wv[2]; d = wd[2]; }
+        if (src == 3) { w = wv[3]; d = wd[3]; }
         wrow[k] = w;
+        drow[k] = d;
     }
     return true;
 }
 
 // ---- the kernel ---------------------------------------------------------------------------------
-template <int NCL>
+// GRAD = true: also d m/d(x0, x1, c, t0) and d chi^2/d theta (row a8); half as many item slots (two
+// weight sets per item), 128-node windows in phase B.
+template <int NCL, bool GRAD>
 __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_constant__ SbHParams P)
 {
+    constexpr int NSL = GRAD ? kSlots / 2 : kSlots; // item slots per stage
+    constexpr int ATS = GRAD ? 2 * kW : kW;         // floats per item slot
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr unsigned FULL = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const SbModelParams &mp = P.mp;
-    const TSmem L(P.n_band_total, P.cap);
+    const TSmem L(P.n_band_total, P.cap, GRAD);
     float *s_at = reinterpret_cast<float *>(smem_raw + L.at);
     float4 *s_ws = reinterpret_cast<float4 *>(smem_raw + L.ws);
     float *s_w = reinterpret_cast<float *>(smem_raw + L.w);
@@ -440,13 +574,14 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
     int *win_all = reinterpret_cast<int *>(smem_raw + L.win);           // [2][lo: kSlots | end: kSlots]
     float *x1_all = reinterpret_cast<float *>(smem_raw + L.x1);         // [2][kSlots]
     int *misc = reinterpret_cast<int *>(smem_raw + L.misc);             // [0] group, [1] n_seg, [2] n_ev, [3] next unit, [4] next offset
-    double *carry = reinterpret_cast<double *>(smem_raw + L.misc + 32); // chi^2 of a unit split over rounds
+    double *carry = reinterpret_cast<double *>(smem_raw + L.misc + 24); // chi^2 [, d chi^2] of a unit split over rounds
+    const float4 *s_wd = s_ws + P.cap;                                  // GRAD: d/dt0 phase weights
 
     for (int i = tid; i < P.n_band_total; i += kThreads) s_w[i] = __ldg(P.band_w + i);
     const long long n_units = (long long)P.n_sn * P.n_samples;
     const int G = P.group_units, CAP = P.cap;
     const long long n_groups = (n_units + G - 1) / G;
-    const bool want_chi = P.out_chi2 != nullptr;
+    const bool want_chi = P.out_chi2 != nullptr || (GRAD && P.out_dchi2 != nullptr);
     const int nP = mp.n_phase, n_bands = P.n_bands;
     const int nq = max(1, min(nP - 3, kBins / n_bands)); // phase-row bins per band
     constexpr uint16_t kNoKey = 0xffffu;
@@ -482,7 +617,7 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
             // than the array is processed alone, CAP observations at a time)
             if (tid == 0) {
                 int u = misc[3], off = misc[4], n_ev = 0, n_seg = 0;
-                while (u < npos && n_seg < kMaxSeg) {
+                while (u < npos && n_seg < NSL) {
                     const int rem = utmp[u].n - off;
                     HSeg &S = segs[n_seg];
                     if (rem <= CAP - n_ev) {
@@ -526,7 +661,10 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                 S.p_lo = (float)(mp.p_lo * cscale);
                 S.p_hi = (float)(mp.p_hi * cscale);
             }
-            for (int e = tid; e < n_ev; e += kThreads) res[e] = 0.f;
+            for (int e = tid; e < n_ev; e += kThreads) {
+                res[e] = 0.f;
+                if (GRAD) { res[CAP + e] = 0.f; res[2 * CAP + e] = 0.f; res[3 * CAP + e] = 0.f; }
+            }
             __syncthreads();
 
             // ---- a1: counting sort of the round's observations by (band, phase row) ----------------
@@ -547,8 +685,8 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                 uint16_t key = kNoKey;
                 if ((unsigned)b < (unsigned)n_bands) {
                     int rb;
-                    double wrow[4];
-                    if (obs_phase(mp, S, __ldg(P.time + o), rb, wrow)) {
+                    double wrow[4], drow[4];
+                    if (obs_phase(mp, S, __ldg(P.time + o), rb, wrow, drow)) {
                         key = (uint16_t)(b * nq + (rb * nq) / (nP - 3));
                         atomicAdd(&hist[key], 1);
                     }
@@ -577,7 +715,7 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                 for (int b = tid; b < n_bands; b += 32) bstart[b] = hist[b * nq];
             }
             __syncthreads();
-            const int bps = max(1, kSlots / n_seg); // bands per stage
+            const int bps = max(1, NSL / n_seg); // bands per stage
             for (int e = tid; e < n_ev; e += kThreads) {
                 const uint16_t key = s_key[e];
                 if (key == kNoKey) continue;
@@ -585,18 +723,20 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                 const HSeg &S = segs[sg];
                 const int o = S.o_lo + (e - S.e_begin);
                 int rb = 0;
-                double wrow[4] = {0.0, 0.0, 0.0, 0.0};
-                obs_phase(mp, S, __ldg(P.time + o), rb, wrow);
-                float wsl[4]; // register slot s holds the row congruent to s mod 4
+                double wrow[4] = {0.0, 0.0, 0.0, 0.0}, drow[4] = {0.0, 0.0, 0.0, 0.0};
+                obs_phase(mp, S, __ldg(P.time + o), rb, wrow, drow);
+                float wsl[4], wdl[4]; // register slot s holds the row congruent to s mod 4
 #pragma unroll
                 for (int s = 0; s < 4; ++s) {
                     const int k = (s - rb) & 3;
                     wsl[s] = (float)(k == 0 ? wrow[0] : k == 1 ? wrow[1] : k == 2 ? wrow[2] : wrow[3]);
+                    wdl[s] = (float)(k == 0 ? drow[0] : k == 1 ? drow[1] : k == 2 ? drow[2] : drow[3]);
                 }
                 const int b = (int)key / nq;
                 const int slot = (b % bps) * n_seg + sg; // item slot inside the band's stage
                 const int pos = atomicAdd(&hist[key], 1);
                 s_ws[pos] = make_float4(wsl[0], wsl[1], wsl[2], wsl[3]);
+                if (GRAD) s_ws[CAP + pos] = make_float4(wdl[0], wdl[1], wdl[2], wdl[3]);
                 s_info[pos] = (uint32_t)slot | ((uint32_t)rb << 5) | ((uint32_t)e << 17);
             }
 
@@ -616,7 +756,7 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                     TItem &I = items_all[buf * kSlots + tid];
                     int *win = win_all + buf * 2 * kSlots;
                     I.n_in = 0; I.n_lo = 0; I.n_end = 0;
-                    if (bstart[b0 + bl + 1] > bstart[b0 + bl] && segs[sg].n > 0) item_geometry(P, segs[sg], b0 + bl, I);
+                    if (bstart[b0 + bl + 1] > bstart[b0 + bl] && segs[sg].n > 0) item_geometry(P, segs[sg], b0 + bl, I, GRAD);
                     if (I.n_in > 0) {
                         atomicMin(&win[bl], I.n_lo & ~3); // multiple of 4: 16-byte aligned row loads
                         atomicMax(&win[kSlots + bl], I.n_end);
@@ -651,7 +791,7 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                             const int np_b = (len + 31) >> 5;
                             const int q_lo = wseg * kPassSeg, q_hi = min(q_lo + kPassSeg, np_b);
                             if (q_lo >= q_hi) continue;
-                            phase_a_item<NCL>(mp, segs[sg], items[it], w_lo, q_lo, q_hi, s_w, s_at + (size_t)it * kW, lane);
+                            phase_a_item<NCL, GRAD>(mp, segs[sg], items[it], w_lo, q_lo, q_hi, s_w, s_at + (size_t)it * ATS, lane);
                         }
                     }
                     __syncthreads();
@@ -667,6 +807,11 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                             const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
                             if (i_lo >= i_hi) continue;
                             const int n_half = (np_w * 32 + 127) >> 7; // 128-node halves of this segment
+                            if constexpr (GRAD) {
+                                for (int h0 = 0; h0 < n_half; ++h0)
+                                    phase_b_window_grad(P, w_lo + wseg * kW + 128 * h0, s_at + 128 * h0 + 4 * lane, s_x1, s_ws,
+                                                        s_wd, s_info, res, CAP, i_lo, i_hi, lane);
+                            } else
                             for (int h0 = 0; h0 < n_half; h0 += 2) {
                                 const int n0 = w_lo + wseg * kW + 128 * h0;
                                 const float *at_l = s_at + 128 * h0 + 4 * lane;
@@ -680,34 +825,62 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                 }
             }
 
-            // ---- epilogue: one warp per segment; a6 zero point (fp64), flux out (coalesced), a7 chi^2
+            // ---- epilogue: one warp per segment; a6 zero point (fp64), flux [, gradient] out (coalesced),
+            // a7 chi^2 [, a8 d chi^2/d theta = -2 sum (f - m)/sigma^2 dm/dtheta] in a fixed order
             for (int sg = warp; sg < n_seg; sg += kWarps) {
                 const HSeg &S = segs[sg];
-                double sum = 0.0;
+                constexpr int NS = GRAD ? 5 : 1;
+                double sum[NS];
+#pragma unroll
+                for (int k = 0; k < NS; ++k) sum[k] = 0.0;
                 for (int i = lane; i < S.n; i += 32) {
                     const int o = S.o_lo + i;
                     const int b = __ldg(P.band + o);
-                    double m;
-                    if ((unsigned)b >= (unsigned)P.n_bands) {
-                        m = __longlong_as_double(0x7ff8000000000000LL);
-                    } else {
+                    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+                    double m = qnan, dm[4] = {qnan, qnan, qnan, qnan};
+                    if ((unsigned)b < (unsigned)P.n_bands) {
                         double sc = 1.0;
                         if (P.zp != nullptr) sc = exp10(0.4 * (double)__ldg(P.zp + o)) * __ldg(P.band_zpab_inv + b);
-                        m = sc * S.x0 * (double)res[S.e_begin + i];
+                        const double raw = (double)res[S.e_begin + i];
+                        m = sc * S.x0 * raw;
+                        if (GRAD) {
+                            dm[0] = sc * raw;
+                            dm[1] = sc * S.x0 * (double)res[CAP + S.e_begin + i];
+                            dm[2] = sc * S.x0 * (double)res[2 * CAP + S.e_begin + i];
+                            dm[3] = sc * S.x0 * (double)res[3 * CAP + S.e_begin + i];
+                        }
                     }
                     if (P.out_flux) P.out_flux[S.out_base + i] = (float)m;
+                    if (GRAD && P.out_dflux)
+                        reinterpret_cast<float4 *>(P.out_dflux)[S.out_base + i] =
+                            make_float4((float)dm[0], (float)dm[1], (float)dm[2], (float)dm[3]);
                     if (want_chi) {
                         const double f = (double)__ldg(P.flux + o), e = (double)__ldg(P.fluxerr + o);
                         const double qv = (f - m) / e;
-                        sum += qv * qv;
+                        sum[0] += qv * qv;
+                        if (GRAD) {
+                            const double g = -2.0 * (f - m) / (e * e);
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) sum[1 + k] += g * dm[k];
+                        }
                     }
                 }
                 if (want_chi) {
-                    sum = sb::warp_sum(sum);
+#pragma unroll
+                    for (int k = 0; k < NS; ++k) sum[k] = sb::warp_sum(sum[k]);
                     if (lane == 0) {
-                        const double total = (S.first ? 0.0 : *carry) + sum;
-                        if (S.last) P.out_chi2[S.unit] = (float)total;
-                        else *carry = total;
+                        double total[NS];
+#pragma unroll
+                        for (int k = 0; k < NS; ++k) total[k] = (S.first ? 0.0 : carry[k]) + sum[k];
+                        if (S.last) {
+                            if (P.out_chi2) P.out_chi2[S.unit] = (float)total[0];
+                            if (GRAD && P.out_dchi2)
+                                reinterpret_cast<float4 *>(P.out_dchi2)[S.unit] =
+                                    make_float4((float)total[1], (float)total[2], (float)total[3], (float)total[4]);
+                        } else {
+#pragma unroll
+                            for (int k = 0; k < NS; ++k) carry[k] = total[k];
+                        }
                     }
                 }
             }

@@ -74,11 +74,13 @@ def test_config3_samples_axis(cuda_device, fp64):
     assert np.array_equal(got2["chi2"], got["chi2"])
 
 
-@pytest.mark.parametrize("fp64", [False, True])
-def test_config4_forward_and_gradient(cuda_device, fp64):
+@pytest.mark.parametrize("fp64,form", [(False, None), (False, "direct"), (False, "tiled"), (True, None)])
+def test_config4_forward_and_gradient(cuda_device, fp64, form):
     wl = prepare(4, n_sn=160)
     ref = oracle_all(wl, grad=True)
-    got = sbgpu.run_gpu(wl, mode="grad", fp64=fp64)
+    got = sbgpu.run_gpu(wl, mode="grad", fp64=fp64, form=form)
+    if form is not None:
+        assert got["form"] == form
     ns = wl.n_samples
     check_flux_chi2(wl, got, ref, fp64)
     tol_f = sbgpu.flux_tolerance(wl, ref["flux"], ns, fp64)
@@ -155,3 +157,23 @@ def test_each_formulation_against_oracle(cuda_device, form, config, kw):
     got = sbgpu.run_gpu(wl, mode="chi2", form=form)
     assert got["launches"] == (1 if form == "direct" else 2) and got["form"] == form
     check_flux_chi2(wl, got, ref, False)
+
+
+def test_gradient_formulations_on_samples_axis_and_ragged_units(cuda_device):
+    """sb_bandflux_grad in the tiled formulation where units share a supernova (config 3 shape: the
+    group of a CTA is 16 parameter samples of one object) and where units are ragged (config 2 shape)."""
+    for config, kw in ((3, {"n_samples": 150}), (2, {"n_sn": 133, "ragged": True}), (5, {"n_sn": 150})):
+        wl = prepare(config, **kw)
+        ref = oracle_all(wl, grad=True)
+        ns = wl.n_samples
+        for form in ("tiled", "direct"):
+            got = sbgpu.run_gpu(wl, mode="grad", form=form)
+            assert got["form"] == form
+            check_flux_chi2(wl, got, ref, False)
+            tol_f = sbgpu.flux_tolerance(wl, ref["flux"], ns, False)
+            tol_d = sbgpu.grad_tolerance(wl, ref, wl.theta, ns, False)
+            err = np.abs(got["dflux"] - ref["dflux"])
+            assert np.all(err <= tol_d), (config, form, np.max(err / np.maximum(tol_d, 1e-300), axis=0))
+            tol_g = sbgpu.dchi2_tolerance(wl, ref, tol_f, tol_d, ns, False)
+            errg = np.abs(got["dchi2"] - ref["dchi2"])
+            assert np.all(errg <= tol_g), (config, form, np.max(errg / np.maximum(tol_g, 1e-300), axis=0))
