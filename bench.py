@@ -131,7 +131,7 @@ def flops_per_call(wl, grad: bool, form: str = "direct"):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
 
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
@@ -143,7 +143,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200"],
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -275,15 +275,16 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--mode", default="chi2", choices=["chi2", "grad"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--form", default="auto", choices=["auto", "direct", "grouped", "tiled"],
                     help="formulation (include/saltband.h SB_FORM_*): auto = the library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-evals", type=int, default=400000, help="evals in the cpu_baseline sample")
+    ap.add_argument("--cpu-evals", type=int, default=2400000,
+                    help="evals in the cpu_baseline sample (about 15 s of the fp64 oracle on 16 host threads)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -449,7 +450,7 @@ def main():
     algo_bytes = in_bytes + out_bytes
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
-        "traffic": None,
+        "traffic": _ncu_traffic(form_run, grad, wl.name),
         "kernel": {"grouped": "sb_hoist_kernel<fwd>", "tiled": "sb_tiled_kernel<%s>" % ("grad" if grad else "fwd")}.get(
             form_run, "sb_fused_kernel<float,%s>" % ("grad" if grad else "fwd")),
         "form": form_run,
@@ -488,6 +489,19 @@ def main():
     if dist is not None:
         dist.destroy_process_group()
     return 0
+
+
+def _ncu_traffic(form: str, grad: bool, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the step's main kernel, copied from
+    the `ncu --set full` capture summarised under profiles/ (profiles/traffic.json); None if this
+    (formulation, mode, workload) has not been captured."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            tab = json.load(fh)
+    except (OSError, ValueError):
+        return None
+    ent = tab.get(f"{form}:{'grad' if grad else 'fwd'}:{workload}")
+    return ent.get("dram_bytes") if isinstance(ent, dict) else None
 
 
 def _measured_peaks():
