@@ -369,11 +369,18 @@ int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, 
         smem = sbh::HSmem(b->n_total, cap).total;
         if (smem > (size_t)smem_max || smem > 100 * 1024) return 1;
     }
-    long long g = n_units / ((long long)n_sm * 4);
-    if (g > sbh::kMaxSeg) g = sbh::kMaxSeg;
-    if (grad && g > sbt::kSlots / 2) g = sbt::kSlots / 2;
-    if ((double)g * mean_obs > (double)cap) g = (long long)((double)cap / mean_obs);
-    if (g < 1) g = 1;
+    // units per group g: the busiest CTA gets ceil(n_groups / n_sm) groups and a group costs about
+    // g + 4 unit-times (per-group work that does not shrink with g: sort, barriers, short chunks --
+    // measured on configs 2, 4, 5), so minimise that product; at most gmax units and cap observations
+    const int gmax = tiled ? (grad ? sbt::kSlots / 2 : sbt::kSlots) : sbh::kMaxSeg;
+    long long g = 1;
+    double best = 0.0;
+    for (long long c = 1; c <= gmax; ++c) {
+        if (c > 1 && (double)c * mean_obs > (double)cap) break;
+        const long long ng = (n_units + c - 1) / c;
+        const double load = (double)((ng + n_sm - 1) / n_sm) * (double)(c + 4);
+        if (c == 1 || load <= best) { best = load; g = c; }
+    }
 
     unsigned char *ws = nullptr; // workspace: group counter + z-order permutation (stream-ordered)
     const size_t ws_bytes = 256 + sizeof(int32_t) * (size_t)bt->n_sn;
@@ -493,7 +500,9 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void 
     kp.out_chi2 = out_chi2;
     kp.out_dchi2 = out_dchi2;
     cudaStream_t st = (cudaStream_t)stream;
-    if (f32 && form != SB_FORM_DIRECT && bt->n_obs_total > 0) {
+    // automatic choice: calls too small to fill the warps of one CTA per SM go to the direct kernel
+    const bool tiny = form == 0 && (long long)bt->n_obs_total * bt->n_samples < 4096;
+    if (f32 && form != SB_FORM_DIRECT && !tiny && bt->n_obs_total > 0) {
         if (form != SB_FORM_GROUPED) {
             const int rc = launch_grouped(true, grad, m, b, bt, flux, fluxerr, out_flux, out_chi2, out_dflux, out_dchi2, st);
             if (rc != 1) return rc;
