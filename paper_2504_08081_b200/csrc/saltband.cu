@@ -359,12 +359,12 @@ int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, 
     const long long n_units = (long long)bt->n_sn * bt->n_samples;
     const double mean_obs = bt->n_sn > 0 ? (double)bt->n_obs_total / (double)bt->n_sn : 1.0;
     // units per group: enough groups for every SM (>= 4 per CTA), at most kMaxSeg, about <= cap observations
+    const int gmax = tiled ? (grad ? sbt::kSlots / 2 : sbt::kSlots) : sbh::kMaxSeg;
     int cap = tiled ? (grad ? 1536 : 3072) : 4096;
     size_t smem = 0;
     if (tiled) {
-        while (cap >= 512 && sbt::TSmem(b->n_total, cap, grad).total > (size_t)smem_max) cap -= 256;
+        while (cap >= 512 && sbt::TSmem(b->n_total, cap, grad, b->n_bands * gmax).total > (size_t)smem_max) cap -= 256;
         if (cap < 512) return 1;
-        smem = sbt::TSmem(b->n_total, cap, grad).total;
     } else {
         smem = sbh::HSmem(b->n_total, cap).total;
         if (smem > (size_t)smem_max || smem > 100 * 1024) return 1;
@@ -372,7 +372,6 @@ int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, 
     // units per group g: the busiest CTA gets ceil(n_groups / n_sm) groups and a group costs about
     // g + 4 unit-times (per-group work that does not shrink with g: sort, barriers, short chunks --
     // measured on configs 2, 4, 5), so minimise that product; at most gmax units and cap observations
-    const int gmax = tiled ? (grad ? sbt::kSlots / 2 : sbt::kSlots) : sbh::kMaxSeg;
     long long g = 1;
     double best = 0.0;
     for (long long c = 1; c <= gmax; ++c) {
@@ -381,6 +380,7 @@ int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, 
         const double load = (double)((ng + n_sm - 1) / n_sm) * (double)(c + 4);
         if (c == 1 || load <= best) { best = load; g = c; }
     }
+    if (tiled) smem = sbt::TSmem(b->n_total, cap, grad, b->n_bands * (int)g).total;
 
     unsigned char *ws = nullptr; // workspace: group counter + z-order permutation (stream-ordered)
     const size_t ws_bytes = 256 + sizeof(int32_t) * (size_t)bt->n_sn;

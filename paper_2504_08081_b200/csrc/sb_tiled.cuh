@@ -61,7 +61,7 @@ struct TSmem {
     size_t w, at, res, ws, info, key, hist, bstart, segs, utmp, items, win, x1, misc, total;
     // grad: two weight sets per item (value, d/dc) in the same At array (half as many item slots), two
     // float4 of phase weights (value, d/dt0) and four results per observation
-    __host__ __device__ TSmem(int n_band_total, int cap, bool grad)
+    __host__ __device__ TSmem(int n_band_total, int cap, bool grad, int n_items)
     {
         size_t o = 0;
         at = o; o += (size_t)kSlots * kW * sizeof(float);
@@ -75,9 +75,9 @@ struct TSmem {
         o = (o + 15) & ~(size_t)15;
         segs = o; o += (size_t)kMaxSeg * sizeof(HSeg);
         utmp = o; o += (size_t)kMaxSeg * sizeof(HUnitTmp);
-        items = o; o += (size_t)2 * kSlots * sizeof(TItem);       // double buffered over stages
-        win = o; o += (size_t)2 * 2 * kSlots * sizeof(int32_t);    // [buffer][lo | end][band of the stage]
-        x1 = o; o += (size_t)2 * kSlots * sizeof(float);          // [buffer][item slot]
+        items = o; o += (size_t)n_items * sizeof(TItem);          // every (band, segment) of a round
+        win = o; o += (size_t)2 * kMaxBands * sizeof(int32_t);     // [lo | end][band]: union node window
+        x1 = o; o += (size_t)kSlots * sizeof(float);              // [item slot of a stage]
         misc = o; o += 64;
         total = o;
     }
@@ -559,7 +559,7 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
     constexpr unsigned FULL = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const SbModelParams &mp = P.mp;
-    const TSmem L(P.n_band_total, P.cap, GRAD);
+    const TSmem L(P.n_band_total, P.cap, GRAD, P.n_bands * P.group_units);
     float *s_at = reinterpret_cast<float *>(smem_raw + L.at);
     float4 *s_ws = reinterpret_cast<float4 *>(smem_raw + L.ws);
     float *s_w = reinterpret_cast<float *>(smem_raw + L.w);
@@ -570,9 +570,9 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
     int *bstart = reinterpret_cast<int *>(smem_raw + L.bstart);
     HSeg *segs = reinterpret_cast<HSeg *>(smem_raw + L.segs);
     HUnitTmp *utmp = reinterpret_cast<HUnitTmp *>(smem_raw + L.utmp);
-    TItem *items_all = reinterpret_cast<TItem *>(smem_raw + L.items);   // [2][kSlots]
-    int *win_all = reinterpret_cast<int *>(smem_raw + L.win);           // [2][lo: kSlots | end: kSlots]
-    float *x1_all = reinterpret_cast<float *>(smem_raw + L.x1);         // [2][kSlots]
+    TItem *items_all = reinterpret_cast<TItem *>(smem_raw + L.items);   // [band][segment]
+    int *win_all = reinterpret_cast<int *>(smem_raw + L.win);           // [lo: kMaxBands | end: kMaxBands]
+    float *x1_all = reinterpret_cast<float *>(smem_raw + L.x1);         // [kSlots]
     int *misc = reinterpret_cast<int *>(smem_raw + L.misc);             // [0] group, [1] n_seg, [2] n_ev, [3] next unit, [4] next offset
     double *carry = reinterpret_cast<double *>(smem_raw + L.misc + 24); // chi^2 [, d chi^2] of a unit split over rounds
     const float4 *s_wd = s_ws + P.cap;                                  // GRAD: d/dt0 phase weights
@@ -634,6 +634,7 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                 misc[1] = n_seg; misc[2] = n_ev; misc[3] = u; misc[4] = off;
             }
             for (int i = tid; i < kBins; i += kThreads) hist[i] = 0;
+            if (tid < kMaxBands) { win_all[tid] = 0x7fffffff; win_all[kMaxBands + tid] = -0x7fffffff; }
             __syncthreads();
             const int n_seg = misc[1], n_ev = misc[2];
             if (tid < n_seg) { // segment parameters (S.unit / S.o_lo hold group-local values until here)
@@ -740,78 +741,62 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                 s_info[pos] = (uint32_t)slot | ((uint32_t)rb << 5) | ((uint32_t)e << 17);
             }
 
-            // ---- stages: as many whole bands as fit the item slots; the small per-stage state (items,
-            // band windows, x1) is double buffered so that the geometry of stage s+1 is computed behind
-            // phase B of stage s: two CTA barriers per stage and window segment.
-            const int n_stage = (n_bands + bps - 1) / bps;
-            auto stage_reset = [&](int buf) { // band windows of a buffer: empty
-                int *win = win_all + buf * 2 * kSlots;
-                if (tid < kSlots) { win[tid] = 0x7fffffff; win[kSlots + tid] = -0x7fffffff; }
-            };
-            auto stage_geometry = [&](int buf, int st) { // items of stage st, union window of every band
-                if (st >= n_stage) return;
-                const int b0 = st * bps, nbs = min(bps, n_bands - b0), n_items = nbs * n_seg;
-                if (tid < n_items) {
-                    const int bl = tid / n_seg, sg = tid - bl * n_seg;
-                    TItem &I = items_all[buf * kSlots + tid];
-                    int *win = win_all + buf * 2 * kSlots;
-                    I.n_in = 0; I.n_lo = 0; I.n_end = 0;
-                    if (bstart[b0 + bl + 1] > bstart[b0 + bl] && segs[sg].n > 0) item_geometry(P, segs[sg], b0 + bl, I, GRAD);
-                    if (I.n_in > 0) {
-                        atomicMin(&win[bl], I.n_lo & ~3); // multiple of 4: 16-byte aligned row loads
-                        atomicMax(&win[kSlots + bl], I.n_end);
-                    }
-                    x1_all[buf * kSlots + tid] = segs[sg].x1;
+            // ---- geometry of every item (band, segment) of the round, union node window of every band:
+            // all threads at once, so the latency of its dependent loads is paid once per round
+            for (int it = tid; it < n_bands * n_seg; it += kThreads) {
+                const int b = it / n_seg, sg = it - b * n_seg;
+                TItem &I = items_all[it];
+                I.n_in = 0; I.n_lo = 0; I.n_end = 0;
+                if (bstart[b + 1] > bstart[b] && segs[sg].n > 0) item_geometry(P, segs[sg], b, I, GRAD);
+                if (I.n_in > 0) {
+                    atomicMin(&win_all[b], I.n_lo & ~3); // multiple of 4: 16-byte aligned row loads
+                    atomicMax(&win_all[kMaxBands + b], I.n_end);
                 }
-            };
-            stage_reset(0);
-            __syncthreads(); // sorted records, bstart and the reset are visible
-            stage_geometry(0, 0);
-            __syncthreads();
+            }
+            if (tid < NSL) x1_all[tid] = segs[tid % n_seg].x1; // item slot -> x1 of its segment
+            __syncthreads(); // sorted records, items and band windows are visible
+
+            // ---- stages: as many whole bands as fit the item slots; two CTA barriers per stage and
+            // window segment
+            const int n_stage = (n_bands + bps - 1) / bps;
             for (int st = 0; st < n_stage; ++st) {
-                const int buf = st & 1;
                 const int b0 = st * bps, nbs = min(bps, n_bands - b0), n_items = nbs * n_seg;
-                const TItem *items = items_all + buf * kSlots;
-                const int *win = win_all + buf * 2 * kSlots;
-                const float *s_x1 = x1_all + buf * kSlots;
+                const TItem *items = items_all + b0 * n_seg;
+                const int *win_lo = win_all + b0, *win_end = win_all + kMaxBands + b0;
+                const float *s_x1 = x1_all;
                 int n_wseg = 0; // window segments of kW nodes: the widest band of the stage decides
                 for (int bl = 0; bl < nbs; ++bl) {
-                    const int len = win[kSlots + bl] - win[bl];
+                    const int len = win_end[bl] - win_lo[bl];
                     if (len > 0) n_wseg = max(n_wseg, (len + kW - 1) / kW);
                 }
-                const int n_step = max(n_wseg, 1);
-                for (int wseg = 0; wseg < n_step; ++wseg) {
-                    if (wseg == 0) stage_reset(buf ^ 1);
+                for (int wseg = 0; wseg < n_wseg; ++wseg) {
                     // phase A: node weights of every item on its band's node grid
-                    if (wseg < n_wseg) {
-                        for (int it = warp; it < n_items; it += kWarps) {
-                            const int bl = it / n_seg, sg = it - bl * n_seg;
-                            const int w_lo = win[bl], len = win[kSlots + bl] - w_lo;
-                            if (len <= 0) continue;
-                            const int np_b = (len + 31) >> 5;
-                            const int q_lo = wseg * kPassSeg, q_hi = min(q_lo + kPassSeg, np_b);
-                            if (q_lo >= q_hi) continue;
-                            phase_a_item<NCL, GRAD>(mp, segs[sg], items[it], w_lo, q_lo, q_hi, s_w, s_at + (size_t)it * ATS, lane);
-                        }
+                    for (int it = warp; it < n_items; it += kWarps) {
+                        const int bl = it / n_seg, sg = it - bl * n_seg;
+                        const int w_lo = win_lo[bl], len = win_end[bl] - w_lo;
+                        if (len <= 0) continue;
+                        const int np_b = (len + 31) >> 5;
+                        const int q_lo = wseg * kPassSeg, q_hi = min(q_lo + kPassSeg, np_b);
+                        if (q_lo >= q_hi) continue;
+                        phase_a_item<NCL, GRAD>(mp, segs[sg], items[it], w_lo, q_lo, q_hi, s_w, s_at + (size_t)it * ATS, lane);
                     }
                     __syncthreads();
                     // phase B: contraction with the model rows, observations in (band, phase row) order
-                    if (wseg < n_wseg) {
-                        for (int bl = 0; bl < nbs; ++bl) {
-                            const int w_lo = win[bl], len = win[kSlots + bl] - w_lo;
-                            if (len <= 0) continue;
-                            const int np_w = min(kPassSeg, ((len + 31) >> 5) - wseg * kPassSeg);
-                            if (np_w <= 0) continue;
-                            const int lo = bstart[b0 + bl], n = bstart[b0 + bl + 1] - lo;
-                            const int per = (((n + kWarps - 1) / kWarps) + 3) & ~3;
-                            const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
-                            if (i_lo >= i_hi) continue;
-                            const int n_half = (np_w * 32 + 127) >> 7; // 128-node halves of this segment
-                            if constexpr (GRAD) {
-                                for (int h0 = 0; h0 < n_half; ++h0)
-                                    phase_b_window_grad(P, w_lo + wseg * kW + 128 * h0, s_at + 128 * h0 + 4 * lane, s_x1, s_ws,
-                                                        s_wd, s_info, res, CAP, i_lo, i_hi, lane);
-                            } else
+                    for (int bl = 0; bl < nbs; ++bl) {
+                        const int w_lo = win_lo[bl], len = win_end[bl] - w_lo;
+                        if (len <= 0) continue;
+                        const int np_w = min(kPassSeg, ((len + 31) >> 5) - wseg * kPassSeg);
+                        if (np_w <= 0) continue;
+                        const int lo = bstart[b0 + bl], n = bstart[b0 + bl + 1] - lo;
+                        const int per = (((n + kWarps - 1) / kWarps) + 3) & ~3;
+                        const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
+                        if (i_lo >= i_hi) continue;
+                        const int n_half = (np_w * 32 + 127) >> 7; // 128-node halves of this segment
+                        if constexpr (GRAD) {
+                            for (int h0 = 0; h0 < n_half; ++h0)
+                                phase_b_window_grad(P, w_lo + wseg * kW + 128 * h0, s_at + 128 * h0 + 4 * lane, s_x1, s_ws,
+                                                    s_wd, s_info, res, CAP, i_lo, i_hi, lane);
+                        } else {
                             for (int h0 = 0; h0 < n_half; h0 += 2) {
                                 const int n0 = w_lo + wseg * kW + 128 * h0;
                                 const float *at_l = s_at + 128 * h0 + 4 * lane;
@@ -820,7 +805,6 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                             }
                         }
                     }
-                    if (wseg == n_step - 1) stage_geometry(buf ^ 1, st + 1);
                     __syncthreads();
                 }
             }
