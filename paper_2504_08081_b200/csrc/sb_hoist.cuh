@@ -83,7 +83,6 @@ __global__ void __launch_bounds__(1024, 1) sb_zorder_kernel(const float *__restr
                                                             unsigned int *counter)
 {
     __shared__ int hist[kZBins];
-    __shared__ int lane_tot[32];
     const int tid = threadIdx.x;
     if (tid == 0) *counter = 0u;
     for (int i = tid; i < kZBins; i += blockDim.x) hist[i] = 0;
@@ -94,7 +93,17 @@ __global__ void __launch_bounds__(1024, 1) sb_zorder_kernel(const float *__restr
         if (!(key > 0.0f)) b = 0;
         return min(max(b, 0), kZBins - 1);
     };
-    for (int i = tid; i < n_sn; i += blockDim.x) atomicAdd(&hist[bin_of(i)], 1);
+    // eight independent loads in flight per thread: the kernel is one CTA and latency bound
+    constexpr int U = 8;
+    const int stride = (int)blockDim.x;
+    for (int i0 = tid; i0 < n_sn; i0 += U * stride) {
+        int bn[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) bn[u] = i0 + u * stride < n_sn ? bin_of(i0 + u * stride) : -1;
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (bn[u] >= 0) atomicAdd(&hist[bn[u]], 1);
+    }
     __syncthreads();
     if (tid < 32) { // exclusive scan: 64 bins per lane, then across lanes
         constexpr int PER = kZBins / 32;
@@ -114,7 +123,14 @@ __global__ void __launch_bounds__(1024, 1) sb_zorder_kernel(const float *__restr
         }
     }
     __syncthreads();
-    for (int i = tid; i < n_sn; i += blockDim.x) perm[atomicAdd(&hist[bin_of(i)], 1)] = i;
+    for (int i0 = tid; i0 < n_sn; i0 += U * stride) {
+        int bn[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) bn[u] = i0 + u * stride < n_sn ? bin_of(i0 + u * stride) : -1;
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (bn[u] >= 0) perm[atomicAdd(&hist[bn[u]], 1)] = i0 + u * stride;
+    }
 }
 
 // ---- colour law of one item: exponent argument (log2 units) as a function of the reduced wavelength

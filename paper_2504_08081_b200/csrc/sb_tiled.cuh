@@ -210,8 +210,23 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
         const int km = __reduce_max_sync(FULL, cnt);
         float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
         float d0 = 0.f, d1 = 0.f, d2 = 0.f, d3 = 0.f; // GRAD: moments weighted by CL
+        auto sample = [&](float e, float cl, float t) { // one band sample into the cell's moments
+            const float t2 = t * t, t3 = t2 * t;
+            s0 += e;
+            s1 = __fmaf_rn(e, t, s1);
+            s2 = __fmaf_rn(e, t2, s2);
+            s3 = __fmaf_rn(e, t3, s3);
+            if (GRAD) {
+                const float c = e * cl;
+                d0 += c;
+                d1 = __fmaf_rn(c, t, d1);
+                d2 = __fmaf_rn(c, t2, d2);
+                d3 = __fmaf_rn(c, t3, d3);
+            }
+        };
+        int k = 0;
 #pragma unroll 1
-        for (int k = 0; k < km; k += 2) { // two samples per trip: independent colour-law chains
+        for (; k + 2 <= km; k += 2) { // two samples per trip: independent colour-law chains
             float w0 = 0.f, w1 = 0.f;
             if (k < cnt) w0 = wp[0];
             if (k + 1 < cnt) w1 = wp[1];
@@ -220,30 +235,17 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
             const float cla = col.template arg<CM>(ra), clb = col.template arg<CM>(rb);
             const float ea = sb::exp_scaled(GRAD ? cla * cs : cla) * w0;
             const float eb = sb::exp_scaled(GRAD ? clb * cs : clb) * w1;
-            const float ta2 = ta * ta, tb2 = tb * tb;
-            const float ta3 = ta2 * ta, tb3 = tb2 * tb;
-            s0 += ea;
-            s1 = __fmaf_rn(ea, ta, s1);
-            s2 = __fmaf_rn(ea, ta2, s2);
-            s3 = __fmaf_rn(ea, ta3, s3);
-            s0 += eb;
-            s1 = __fmaf_rn(eb, tb, s1);
-            s2 = __fmaf_rn(eb, tb2, s2);
-            s3 = __fmaf_rn(eb, tb3, s3);
-            if (GRAD) {
-                const float ca = ea * cla, cb = eb * clb;
-                d0 += ca;
-                d1 = __fmaf_rn(ca, ta, d1);
-                d2 = __fmaf_rn(ca, ta2, d2);
-                d3 = __fmaf_rn(ca, ta3, d3);
-                d0 += cb;
-                d1 = __fmaf_rn(cb, tb, d1);
-                d2 = __fmaf_rn(cb, tb2, d2);
-                d3 = __fmaf_rn(cb, tb3, d3);
-            }
+            sample(ea, cla, ta);
+            sample(eb, clb, tb);
             tau += ha2;
             r += hal2;
             wp += 2;
+        }
+        if (k < km) { // odd trip count: one more sample
+            float w0 = 0.f;
+            if (k < cnt) w0 = wp[0];
+            const float cla = col.template arg<CM>(r);
+            sample(sb::exp_scaled(GRAD ? cla * cs : cla) * w0, cla, tau);
         }
         // moments -> weights on the cell's four nodes (Keys a = -1/2; linear in border cells, G2)
         const int g = I.g_first + gq;
