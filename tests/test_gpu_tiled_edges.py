@@ -1,0 +1,124 @@
+"""-m gpu edge cases of the grouped / tiled formulations (csrc/sb_hoist.cuh, csrc/sb_tiled.cuh), each
+against the fp64 oracle and in every formulation that applies: windows wider than one 512-node
+segment of the node-weight array, a unit with more observations than one round holds (the unit is
+split over rounds and its chi^2 carried), empty units inside a group, groups that mix very different
+redshifts (union node window much wider than any item's), bands that leave the model grid for
+part of a group, a single band, and phases outside the grid."""
+import numpy as np
+import pytest
+
+import oracle
+import sbgpu
+import workloads
+from test_gpu_edges import custom_workload
+
+pytestmark = pytest.mark.gpu
+
+CL = {"cl_coef": np.array([0.0, 0.8, -0.2, 0.05, -0.01]), "cl_wave_b": 4302.57, "cl_wave_v": 5428.55,
+      "cl_lo": 2800.0, "cl_hi": 7000.0}
+
+
+def smooth_model(n_phase, wave, seed=0):
+    phase = -6.0 + np.arange(n_phase, dtype=np.float64)
+    lam = wave[None, :]
+    taper = np.clip((lam - wave[0]) / 200.0, 0, 1) * np.clip((wave[-1] - lam) / 200.0, 0, 1)
+    m0 = (1.0 + 0.3 * np.sin(lam / 137.0 + seed)) * np.exp(-0.5 * (phase[:, None] / 7.0) ** 2) * taper
+    m1 = 0.1 * m0 * np.cos(lam / 291.0 + 0.3 * phase[:, None])
+    return dict(phase=phase, wave=wave, m0=m0, m1=m1, **CL)
+
+
+def attach(wl):
+    true = oracle.run_workload(wl, theta={k: v.copy() for k, v in wl.theta_true.items()}, want_flux=True)["flux"]
+    rng = np.random.default_rng(9)
+    wl.noise = rng.standard_normal(wl.n_obs_total)
+    workloads.attach_data(wl, np.where(np.isfinite(true), true, 0.0))
+    return wl
+
+
+def check_all_forms(wl, forms=("tiled", "grouped", "direct"), grad_forms=("tiled", "direct")):
+    ns = wl.n_samples
+    ref = oracle.run_workload(wl, want_flux=True, want_chi2=True, want_dflux=True, want_dchi2=True)
+    fin = np.isfinite(ref["flux"])
+    ref0 = {"flux": np.where(fin, ref["flux"], 0.0), "dflux": np.where(fin[:, None], ref["dflux"], 0.0)}
+    tol = sbgpu.flux_tolerance(wl, ref0["flux"], ns, False)
+    tolc = sbgpu.chi2_tolerance(wl, ref0["flux"], tol, ns, False)
+    tol_d = sbgpu.grad_tolerance(wl, ref0, wl.theta, ns, False)
+    okc = np.isfinite(ref["chi2"])
+    for form in forms:
+        try:
+            got = sbgpu.run_gpu(wl, mode="chi2", form=form)
+        except Exception as exc:  # include/saltband.h: SB_ELIMIT when a demanded formulation does not apply
+            assert form == "grouped" and "status -4" in str(exc), (form, exc)  # model wider than its table
+            continue
+        assert got["form"] == form
+        assert np.array_equal(np.isnan(got["flux"]), ~fin), form
+        err = np.abs(got["flux"] - ref["flux"])[fin]
+        assert np.all(err <= tol[fin]), (form, float(np.max(err / np.maximum(tol[fin], 1e-300))))
+        assert np.all(np.abs(got["chi2"] - ref["chi2"])[okc] <= tolc[okc]), form
+    for form in grad_forms:
+        got = sbgpu.run_gpu(wl, mode="grad", form=form)
+        assert got["form"] == form
+        assert np.all(np.abs(got["flux"] - ref["flux"])[fin] <= tol[fin]), form
+        errd = np.abs(got["dflux"] - ref["dflux"])[fin]
+        assert np.all(errd <= tol_d[fin]), (form, np.max(errd / np.maximum(tol_d[fin], 1e-300), axis=0))
+        tol_g = sbgpu.dchi2_tolerance(wl, {"flux": ref0["flux"], "dflux": ref0["dflux"]}, tol, tol_d, ns, False)
+        assert np.all(np.abs(got["dchi2"] - ref["dchi2"])[okc] <= tol_g[okc]), form
+        assert np.all(np.abs(got["chi2"] - ref["chi2"])[okc] <= tolc[okc]), form
+
+
+def test_windows_wider_than_one_segment(cuda_device):
+    """2 A model grid: a 3000 A band spans ~1400 nodes at z ~ 0.05 (three 512-node segments); the
+    second band leaves the grid on the blue side for the high-redshift units of the same group."""
+    wave = 3000.0 + 2.0 * np.arange(2501)  # 3000 .. 8000 A
+    md = smooth_model(14, wave)
+    w_a = 4000.0 + 5.0 * np.arange(601)    # 4000 .. 7000 A
+    w_b = 3050.0 + 5.0 * np.arange(241)    # 3050 .. 4250 A: rest frame < 3000 A for z > 0.42
+    bd = workloads.generators.pack_bands([(w_a, np.exp(-0.5 * ((w_a - 5500.0) / 700.0) ** 2)),
+                                          (w_b, np.full(w_b.size, 0.6))])
+    rng = np.random.default_rng(1)
+    n_sn, n_obs = 9, 12
+    z = np.array([0.05, 0.051, 0.30, 0.02, 0.5, 0.049, 0.31, 0.0, 0.8])
+    th = {"x0": rng.uniform(1e-5, 3e-5, n_sn), "x1": rng.normal(size=n_sn), "c": 0.1 * rng.normal(size=n_sn),
+          "t0": rng.uniform(-1, 1, n_sn)}
+    wl = custom_workload(md, bd, np.arange(n_sn + 1) * n_obs, rng.uniform(-5.0, 6.5, n_sn * n_obs),
+                         np.arange(n_sn * n_obs) % 2, z, th)
+    check_all_forms(attach(wl))
+
+
+def test_unit_larger_than_a_round_and_empty_units(cuda_device):
+    """One supernova with 3500 observations (> 3072 per forward round, > 1536 per gradient round), two
+    with none, the rest ragged: segments, chi^2 carry over rounds, empty units (chi^2 = 0)."""
+    wl0 = workloads.make_workload(2, n_sn=8)
+    rng = np.random.default_rng(2)
+    counts = np.array([5, 0, 3500, 17, 0, 60, 1, 33])
+    off = np.concatenate([[0], np.cumsum(counts)])
+    n = int(off[-1])
+    th = {k: v.astype(np.float64) for k, v in wl0.theta.items()}
+    wl = custom_workload(wl0.model, wl0.bands, off, rng.uniform(-15.0, 45.0, n), rng.integers(0, 6, n),
+                         wl0.z.astype(np.float64), th)
+    wl = attach(wl)
+    check_all_forms(wl)
+    got = sbgpu.run_gpu(wl, mode="chi2", form="tiled")
+    assert got["chi2"][1] == 0.0 and got["chi2"][4] == 0.0
+
+
+def test_single_band_phases_outside_grid_and_samples_axis(cuda_device):
+    """One band, several parameter samples per supernova (units of one object share observations),
+    t0 pushed so that part of the phases fall outside the phase grid (zero flux, G3)."""
+    wave = 2500.0 + 10.0 * np.arange(651)
+    md = smooth_model(9, wave, seed=2)  # phases -6 .. +2 d
+    w = 4500.0 + 5.0 * np.arange(301)
+    bd = workloads.generators.pack_bands([(w, np.exp(-0.5 * ((w - 5250.0) / 300.0) ** 2))])
+    rng = np.random.default_rng(4)
+    n_sn, n_samples, n_obs = 3, 21, 37
+    z = np.array([0.1, 0.45, 0.0])
+    nu = n_sn * n_samples
+    th = {"x0": rng.uniform(1e-5, 3e-5, nu), "x1": rng.normal(size=nu), "c": 0.1 * rng.normal(size=nu),
+          "t0": rng.uniform(-4, 4, nu)}
+    wl = custom_workload(md, bd, np.arange(n_sn + 1) * n_obs, rng.uniform(-9.0, 5.0, n_sn * n_obs),
+                         np.zeros(n_sn * n_obs, dtype=int), z, th, n_samples=n_samples)
+    wl.theta_true = {k: v.reshape(n_sn, n_samples)[:, 0].copy() for k, v in wl.theta.items()}
+    wl = attach(wl)
+    ref = oracle.run_workload(wl, want_flux=True)["flux"]
+    assert 0.05 < np.mean(ref == 0.0) < 0.9  # the case does exercise out-of-grid phases
+    check_all_forms(wl)
