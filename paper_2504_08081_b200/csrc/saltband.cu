@@ -382,8 +382,11 @@ int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, 
     }
     if (tiled) smem = sbt::TSmem(b->n_total, cap, grad, b->n_bands * (int)g).total;
 
-    unsigned char *ws = nullptr; // workspace: group counter + z-order permutation (stream-ordered)
-    const size_t ws_bytes = 256 + sizeof(int32_t) * (size_t)bt->n_sn;
+    // workspace (stream-ordered): [0] group counter, [256] bin totals, [4096] z-order permutation, then
+    // the per-segment bin counts of the sort
+    unsigned char *ws = nullptr;
+    const size_t perm_off = 4096, hist_off = perm_off + ((sizeof(int32_t) * (size_t)bt->n_sn + 255) & ~(size_t)255);
+    const size_t ws_bytes = hist_off + sizeof(uint32_t) * (size_t)sbh::kZSegs * sbh::kZBins;
     if (!cuda_ok(cudaMallocAsync((void **)&ws, ws_bytes, st))) return SB_ECUDA;
     SbHParams hp;
     memset(&hp, 0, sizeof(hp));
@@ -417,12 +420,20 @@ int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, 
     hp.out_dflux = (float *)out_dflux;
     hp.out_dchi2 = (float *)out_dchi2;
     hp.counter = reinterpret_cast<unsigned int *>(ws);
-    hp.perm = reinterpret_cast<const int32_t *>(ws + 256);
+    hp.perm = reinterpret_cast<const int32_t *>(ws + perm_off);
     hp.group_units = (int)g;
     hp.cap = cap;
     int rc = SB_OK;
-    sbh::sb_zorder_kernel<<<1, 1024, 0, st>>>(hp.z, hp.n_sn, reinterpret_cast<int32_t *>(ws + 256), hp.counter);
-    if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
+    static_assert(256 + sizeof(uint32_t) * sbh::kZBins <= 4096, "bin totals overlap the permutation");
+    uint32_t *z_tot = reinterpret_cast<uint32_t *>(ws + 256), *z_hist = reinterpret_cast<uint32_t *>(ws + hist_off);
+    if (!cuda_ok(cudaMemsetAsync(ws, 0, perm_off, st))) rc = SB_ECUDA;
+    if (rc == SB_OK) {
+        sbh::sb_zhist_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(hp.z, hp.n_sn, z_hist, z_tot, hp.counter);
+        sbh::sb_zscatter_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(hp.z, hp.n_sn, z_hist, z_tot,
+                                                                          reinterpret_cast<int32_t *>(ws + perm_off));
+        if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
+        else tl_launches += 1; // the second of the two; the first is counted below
+    }
     if (rc == SB_OK) {
         tl_launches += 1;
         const long long n_groups = (n_units + g - 1) / g;

@@ -33,7 +33,7 @@ constexpr int kWarps = 16;
 constexpr int kThreads = kWarps * 32;
 constexpr int kMaxSeg = 32;  // segments (units) per round
 constexpr int kOB = 8;       // observations sharing one pass
-constexpr int kZBins = 2048; // redshift bins of the z-order permutation
+constexpr int kZBins = 512;  // redshift bins of the z-order permutation
 
 // One segment = a contiguous run of observations of one unit (a whole unit unless it exceeds the
 // round capacity); lives in shared memory for the duration of a round.
@@ -76,60 +76,113 @@ struct HSmem {
     }
 };
 
-// ---- z-order permutation (counting sort of the supernovae by 1/(1+z)) + group counter reset -------
-// One CTA.  Order inside a bin is arbitrary (atomics): results do not depend on it, each unit is
-// computed independently of its neighbours.
-__global__ void __launch_bounds__(1024, 1) sb_zorder_kernel(const float *__restrict__ z, int n_sn, int32_t *perm,
-                                                            unsigned int *counter)
+// ---- z-order permutation: STABLE counting sort of the supernovae by 1/(1+z), two small kernels -----
+// The supernovae are cut into kZSegs contiguous segments, one per warp (kZCtas CTAs of kZWarps warps).
+// sb_zhist_kernel counts the bins of every segment (ranks inside a warp step come from
+// __match_any_sync, counters are warp private) into hist[segment][bin] and adds them to tot[bin];
+// sb_zscatter_kernel turns tot into bin offsets, adds the counts of the lower segments and scatters.
+// The permutation is stable, hence the same on every run: the groups of the tiled kernel, and with them
+// its rounding order, are reproducible.  Workspace: tot[kZBins] (zeroed by the caller), hist.
+constexpr int kZWarps = 8;
+constexpr int kZCtas = 32;
+constexpr int kZSegs = kZWarps * kZCtas;
+
+__device__ __forceinline__ int z_bin(const float *__restrict__ z, int i)
 {
-    __shared__ int hist[kZBins];
-    const int tid = threadIdx.x;
-    if (tid == 0) *counter = 0u;
-    for (int i = tid; i < kZBins; i += blockDim.x) hist[i] = 0;
+    const float key = 1.0f / (1.0f + __ldg(z + i)); // window position scales with 1/(1+z)
+    int b = (int)(key * (float)kZBins);
+    if (!(key > 0.0f)) b = 0;
+    return min(max(b, 0), kZBins - 1);
+}
+__device__ __forceinline__ int z_chunk(int n_sn) { return (((n_sn + kZSegs - 1) / kZSegs) + 31) & ~31; }
+
+__global__ void __launch_bounds__(kZWarps * 32, 1) sb_zhist_kernel(const float *__restrict__ z, int n_sn, uint32_t *hist,
+                                                                   uint32_t *tot, unsigned int *counter)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    __shared__ uint32_t cnt[kZWarps][kZBins]; // 16 KB
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (blockIdx.x == 0 && tid == 0) *counter = 0u; // group counter of the main kernel
+    for (int i = tid; i < kZWarps * kZBins; i += kZWarps * 32) (&cnt[0][0])[i] = 0u;
     __syncthreads();
-    auto bin_of = [&](int i) {
-        const float key = 1.0f / (1.0f + __ldg(z + i)); // window position scales with 1/(1+z)
-        int b = (int)(key * (float)kZBins);
-        if (!(key > 0.0f)) b = 0;
-        return min(max(b, 0), kZBins - 1);
-    };
-    // eight independent loads in flight per thread: the kernel is one CTA and latency bound
-    constexpr int U = 8;
-    const int stride = (int)blockDim.x;
-    for (int i0 = tid; i0 < n_sn; i0 += U * stride) {
+    const int seg = blockIdx.x * kZWarps + warp, chunk = z_chunk(n_sn);
+    const int lo = min(seg * chunk, n_sn), hi = min(lo + chunk, n_sn);
+    constexpr int U = 4; // steps whose loads are in flight together
+    uint32_t *mine = cnt[warp];
+    for (int i0 = lo; i0 < hi; i0 += 32 * U) {
         int bn[U];
 #pragma unroll
-        for (int u = 0; u < U; ++u) bn[u] = i0 + u * stride < n_sn ? bin_of(i0 + u * stride) : -1;
+        for (int u = 0; u < U; ++u) bn[u] = i0 + 32 * u + lane < hi ? z_bin(z, i0 + 32 * u + lane) : -1;
 #pragma unroll
-        for (int u = 0; u < U; ++u)
-            if (bn[u] >= 0) atomicAdd(&hist[bn[u]], 1);
-    }
-    __syncthreads();
-    if (tid < 32) { // exclusive scan: 64 bins per lane, then across lanes
-        constexpr int PER = kZBins / 32;
-        int s = 0;
-        for (int k = 0; k < PER; ++k) s += hist[tid * PER + k];
-        int incl = s;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int v = __shfl_up_sync(0xffffffffu, incl, o);
-            if (tid >= o) incl += v;
-        }
-        int run = incl - s;
-        for (int k = 0; k < PER; ++k) {
-            const int c = hist[tid * PER + k];
-            hist[tid * PER + k] = run;
-            run += c;
+        for (int u = 0; u < U; ++u) {
+            const unsigned m = __match_any_sync(FULL, bn[u]);
+            if (bn[u] >= 0 && lane == __ffs(m) - 1) mine[bn[u]] += (uint32_t)__popc(m);
+            __syncwarp();
         }
     }
     __syncthreads();
-    for (int i0 = tid; i0 < n_sn; i0 += U * stride) {
+    for (int i = tid; i < kZWarps * kZBins; i += kZWarps * 32) {
+        const int w = i / kZBins, b = i - w * kZBins;
+        const uint32_t c = cnt[w][b];
+        hist[(size_t)(blockIdx.x * kZWarps + w) * kZBins + b] = c;
+        if (c) atomicAdd(tot + b, c); // integer sums: order does not matter
+    }
+}
+
+__global__ void __launch_bounds__(kZWarps * 32, 1) sb_zscatter_kernel(const float *__restrict__ z, int n_sn,
+                                                                      const uint32_t *__restrict__ hist,
+                                                                      const uint32_t *__restrict__ tot, int32_t *perm)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    constexpr int NT = kZWarps * 32, PER = kZBins / NT; // bins per thread in the prefix steps
+    __shared__ uint32_t cnt[kZWarps][kZBins];
+    __shared__ uint32_t wsum[kZWarps];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // offset of every bin: exclusive scan of tot (thread t owns bins PER t .. PER t + PER - 1)
+    uint32_t bt[PER], run = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { bt[k] = tot[tid * PER + k]; run += bt[k]; }
+    uint32_t incl = run;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(FULL, incl, o);
+        if (lane >= o) incl += v;
+    }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    uint32_t base = incl - run;
+    for (int w = 0; w < warp; ++w) base += wsum[w];
+    // plus the counts of all lower segments, then of the lower warps of this CTA
+    const int seg0 = blockIdx.x * kZWarps;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int b = tid * PER + k;
+        uint32_t a = base;
+        for (int sgm = 0; sgm < seg0; ++sgm) a += hist[(size_t)sgm * kZBins + b];
+        for (int w = 0; w < kZWarps; ++w) {
+            cnt[w][b] = a;
+            a += hist[(size_t)(seg0 + w) * kZBins + b];
+        }
+        base += bt[k];
+    }
+    __syncthreads();
+    const int seg = seg0 + warp, chunk = z_chunk(n_sn);
+    const int lo = min(seg * chunk, n_sn), hi = min(lo + chunk, n_sn);
+    constexpr int U = 4;
+    uint32_t *mine = cnt[warp];
+    for (int i0 = lo; i0 < hi; i0 += 32 * U) {
         int bn[U];
 #pragma unroll
-        for (int u = 0; u < U; ++u) bn[u] = i0 + u * stride < n_sn ? bin_of(i0 + u * stride) : -1;
+        for (int u = 0; u < U; ++u) bn[u] = i0 + 32 * u + lane < hi ? z_bin(z, i0 + 32 * u + lane) : -1;
 #pragma unroll
-        for (int u = 0; u < U; ++u)
-            if (bn[u] >= 0) perm[atomicAdd(&hist[bn[u]], 1)] = i0 + u * stride;
+        for (int u = 0; u < U; ++u) {
+            const unsigned m = __match_any_sync(FULL, bn[u]);
+            const uint32_t at = bn[u] >= 0 ? mine[bn[u]] : 0u;
+            __syncwarp();
+            if (bn[u] >= 0 && lane == __ffs(m) - 1) mine[bn[u]] = at + (uint32_t)__popc(m);
+            __syncwarp();
+            if (bn[u] >= 0) perm[at + (uint32_t)__popc(m & ((1u << lane) - 1u))] = i0 + 32 * u + lane;
+        }
     }
 }
 

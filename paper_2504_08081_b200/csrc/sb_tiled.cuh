@@ -588,12 +588,15 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
     const int nq = max(1, min(nP - 3, kBins / n_bands)); // phase-row bins per band
     constexpr uint16_t kNoKey = 0xffffu;
 
+    // Groups are claimed one ahead (misc[5] = the next group of this CTA) so that the records of the
+    // next group can be pulled into L2 while the current one is computed.
+    if (tid == 0) misc[5] = (int)atomicAdd(P.counter, 1u);
     for (;;) {
         __syncthreads();
-        if (tid == 0) misc[0] = (int)atomicAdd(P.counter, 1u);
+        const long long group = (long long)(unsigned)misc[5];
         __syncthreads();
-        const long long group = (long long)(unsigned)misc[0];
         if (group >= n_groups) break;
+        if (tid == kThreads - 1) misc[5] = (int)atomicAdd(P.counter, 1u); // read again after many barriers
         const long long pos0 = group * G;
         const int npos = (int)min((long long)G, n_units - pos0);
         if (tid < npos) { // unit -> supernova (z-ordered), observation range
@@ -757,6 +760,27 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
             }
             if (tid < NSL) x1_all[tid] = segs[tid % n_seg].x1; // item slot -> x1 of its segment
             __syncthreads(); // sorted records, items and band windows are visible
+
+            // ---- L2 prefetch of the next group's records (one lane per unit, last warp, first round)
+            if (warp == kWarps - 1 && cur_u == 0) {
+                const long long pos = (long long)(unsigned)misc[5] * G + lane;
+                if (lane < G && (long long)(unsigned)misc[5] < n_groups && pos < n_units) {
+                    const int si = (int)(pos / P.n_samples);
+                    const int sn = P.perm ? __ldg(P.perm + si) : si;
+                    const int o_lo = __ldg(P.obs_offset + sn), n = __ldg(P.obs_offset + sn + 1) - o_lo;
+                    auto pf = [](const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); };
+                    const long long unit = (long long)sn * P.n_samples + (pos - (long long)si * P.n_samples);
+                    pf(P.z + sn); pf(P.x0 + unit); pf(P.x1 + unit); pf(P.c + unit); pf(P.t0 + unit);
+                    for (int o = 0; o < n + 31; o += 32) { // one 128-byte line of every array per step
+                        const int oo = o_lo + min(o, n - 1);
+                        if (n <= 0) break;
+                        pf(P.time + oo);
+                        pf(P.band + oo);
+                        if (P.zp) pf(P.zp + oo);
+                        if (P.flux) { pf(P.flux + oo); pf(P.fluxerr + oo); }
+                    }
+                }
+            }
 
             // ---- stages: as many whole bands as fit the item slots; two CTA barriers per stage and
             // window segment
