@@ -63,7 +63,8 @@ typedef enum { SB_F32 = 0, SB_F64 = 1 } sb_dtype;
  *                    SB_ELIMIT.
  *   SB_FORM_TILED    as SB_FORM_GROUPED, and the observations of a group of units that are neighbours
  *                    in redshift are ordered by phase so that the model rows they read stay in
- *                    registers; same applicability and error behaviour. */
+ *                    registers; fp32 forward AND gradient calls with uniform
+ *                    band grids, same error behaviour. */
 enum { SB_FORM_DIRECT = 0x100, SB_FORM_GROUPED = 0x200, SB_FORM_TILED = 0x400 };
 
 typedef enum {

@@ -1,6 +1,6 @@
-// sb_tiled.cuh -- the register-tiled node-weight kernel (sm_100a), fp32 forward.
+// sb_tiled.cuh -- the register-tiled node-weight kernel (sm_100a), fp32, forward and gradient.
 //
-// Same sums per evaluation as sb_kernels.cuh / sb_hoist.cuh (SURVEY.md section 8(a) rows a1-a7), with
+// Same sums per evaluation as sb_kernels.cuh / sb_hoist.cuh (SURVEY.md section 8(a) rows a1-a8), with
 // the band integral re-associated as in sb_hoist.cuh (an exact exchange of two finite sums):
 //     raw_o = sum_l At[l] * R_o[l],   At[l] = sum_j ew_j w_{l-i_j}(tau_j)   (NODE WEIGHTS of (unit, band)),
 //     R_o[l] = sum_k wp_k(o) (M0 + x1 M1)[rb_o + k][l]                      (phase-collapsed row of o),
@@ -8,21 +8,27 @@
 //
 // What differs from sb_hoist.cuh is WHO holds WHAT.  There a lane reloaded the four phase rows of
 // {M0, M1} for every observation (four LDG.64 per eight FFMA: bound by the L1 data pipe).  Here a CTA
-// works on a GROUP of up to 32 units that are neighbours in redshift, one STAGE (a set of bands) at a
-// time, in two phases separated by a CTA barrier:
-//   phase A  one warp per ITEM (unit, band): lanes own model cells, walk the band samples of their
-//            cell (colour factor x folded weight, moments sum ew tau^p), turn the moments into node
-//            weights and store At[item][node] in SHARED MEMORY (<= 512 nodes per item and pass);
-//   phase B  the observations of the stage, sorted by (band, first phase row rb), are cut into equal
-//            contiguous chunks, one per warp.  A lane owns 8 nodes of a 256-node window and keeps the
-//            four phase rows of M0 and of M1 at those nodes in REGISTERS (64 values, row r in slot
-//            r mod 4); moving to the next observation only reloads the rows that changed.  Per
-//            observation a lane reads its 8 node weights (two LDS.128) and issues 72 FFMA; four
-//            observations share one transposed warp reduction.
-// HBM sees only the per-observation records; the model window is read from L2/L1 about once per
-// (warp, stage) instead of once per observation.
-// Requirements (checked by the host, otherwise sb_hoist.cuh / sb_kernels.cuh run): fp32, forward
-// only, uniform band grids, n_phase in [4, 4096], n_cl <= NCL, n_bands <= 64.
+// works on a GROUP of up to 32 units that are neighbours in redshift (stable z-order, sb_hoist.cuh),
+// in ROUNDS of at most `cap` observations.  Per round: the observations are counting-sorted in shared
+// memory by (band, first phase row rb); the geometry of every (band, unit) item and the union node
+// window of every band are computed by all threads; then, one STAGE (a set of bands) at a time, two
+// phases separated by a CTA barrier:
+//   phase A  one warp per ITEM (unit, band): lanes own model cells of the band's common node grid,
+//            walk the band samples of their cell (colour factor x folded weight, moments sum ew tau^p),
+//            turn the moments into node weights and store At[item][node] in SHARED MEMORY (512 nodes
+//            per item and window segment; wider windows take several segments);
+//   phase B  the observations of a band, sorted by rb, are cut into equal contiguous chunks, one per
+//            warp.  A lane owns 8 nodes of a 256-node window and keeps the four phase rows of M0 and of
+//            M1 at those nodes in REGISTERS (64 values, row r in slot r mod 4); moving to the next
+//            observation only reloads the rows that changed.  Per observation a lane reads its 8 node
+//            weights (two LDS.128) and issues 72 FFMA; four observations share one transposed warp
+//            reduction.
+// and an epilogue per unit in fp64 (zero point, coalesced stores, chi^2 in a fixed order).  The
+// gradient variant (GRAD) adds CL-weighted node weights (d/dc), M1-only and phase-derivative row sums
+// (d/dx1, d/dt0) and d chi^2/d theta.  HBM sees only the per-observation records (the next group's are
+// prefetched into L2); the model window is read from L2/L1 about once per (warp, stage).
+// Requirements (checked by the host, otherwise sb_hoist.cuh / sb_kernels.cuh run): fp32, uniform band
+// grids, n_phase in [4, 4096], n_cl <= NCL, n_bands <= 64.
 #pragma once
 #include "sb_internal.h"
 #include "sb_kernels.cuh"
