@@ -143,6 +143,23 @@ int sb_bandflux_grad(const sb_model *m, const sb_bands *b, const sb_batch *batch
                      const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2,
                      void *out_dchi2, void *stream);
 
+/* sb_chi2_host / sb_bandflux_grad_host -- the same operations for data that lives in HOST memory
+ * (the end-to-end path of a fit driver that keeps its light curves on the host).  Every pointer of
+ * `batch`, flux, fluxerr and every output is a HOST pointer with the layout of the device call;
+ * pinned (page-locked) buffers give the full PCIe rate, pageable ones work.  The library cuts the
+ * supernovae into chunks, stages each chunk through device buffers of its own (stream-ordered
+ * allocations, released before return) and overlaps host->device copies, kernels and device->host
+ * copies of consecutive chunks on internal streams.  Results are those of the device call on each
+ * chunk: identical to the whole-batch device call in the direct formulation, and within rounding
+ * (the parity tolerance) in the tiled one, whose summation order depends on which supernovae share
+ * a group.  The call returns when all outputs are complete (it synchronises its streams);
+ * sb_last_launch_count() then reports the kernels of all chunks.  Errors as for the device calls. */
+int sb_chi2_host(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+                 const void *fluxerr, void *out_chi2, void *out_flux);
+int sb_bandflux_grad_host(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+                          const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2,
+                          void *out_dchi2);
+
 /* Introspection (host side, cheap). */
 int32_t sb_bands_count(const sb_bands *b);
 /* ZPAB_b as computed at load (fp64), or NaN for a bad index. */

@@ -19,7 +19,9 @@ from .api import (  # noqa: F401
     lib_path,
     sb_bandflux,
     sb_bandflux_grad,
+    sb_bandflux_grad_host,
     sb_chi2,
+    sb_chi2_host,
     sb_load_bandpasses,
     sb_load_model,
     version,

@@ -62,6 +62,10 @@ def _load():
     L.sb_chi2.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp, vp]
     L.sb_bandflux_grad.restype = C.c_int
     L.sb_bandflux_grad.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp, vp, vp, vp]
+    L.sb_chi2_host.restype = C.c_int
+    L.sb_chi2_host.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp]
+    L.sb_bandflux_grad_host.restype = C.c_int
+    L.sb_bandflux_grad_host.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp, vp, vp]
     L.sb_bands_count.restype = C.c_int32
     L.sb_bands_count.argtypes = [vp]
     L.sb_bands_zpab.restype = C.c_double
@@ -244,3 +248,60 @@ def sb_bandflux_grad(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_sam
         _ptr(out_chi2, ft, n_units, "out_chi2", allow_none=True),
         _ptr(out_dchi2, ft, n_units * 4, "out_dchi2", allow_none=True), _stream())
     _check(rc, "sb_bandflux_grad")
+
+
+# ---------------------------------------------------------------- host-buffer calls
+def _hptr(t, dtype, n: Optional[int], name: str, allow_none: bool = False):
+    """Host pointer of a CPU torch tensor (pinned or pageable) of the given dtype and size."""
+    import torch
+
+    if t is None:
+        if allow_none:
+            return None
+        raise ValueError(f"{name} is required")
+    if not isinstance(t, torch.Tensor) or t.is_cuda:
+        raise ValueError(f"{name} must be a CPU torch tensor (pin it for the full PCIe rate)")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise ValueError(f"{name} must be a contiguous tensor of dtype {dtype}")
+    if n is not None and t.numel() != n:
+        raise ValueError(f"{name} must have {n} elements, got {t.numel()}")
+    return t.data_ptr()
+
+
+def _host_batch(dtype, n_sn, n_samples, n_obs_total, obs_offset, time, band, zp, z, x0, x1, c, t0):
+    import torch
+
+    ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
+    n_units = n_sn * n_samples
+    return ft, _Batch(
+        dtype, n_sn, n_samples, n_obs_total, _hptr(obs_offset, torch.int32, n_sn + 1, "obs_offset"),
+        _hptr(time, ft, n_obs_total, "time"), _hptr(band, torch.int32, n_obs_total, "band"),
+        _hptr(zp, ft, n_obs_total, "zp", allow_none=True), _hptr(z, ft, n_sn, "z"), _hptr(x0, ft, n_units, "x0"),
+        _hptr(x1, ft, n_units, "x1"), _hptr(c, ft, n_units, "c"), _hptr(t0, ft, n_units, "t0"))
+
+
+def sb_chi2_host(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,
+                 obs_offset, time, band, zp, z, x0, x1, c, t0, flux, fluxerr, out_chi2, out_flux=None) -> None:
+    """include/saltband.h: sb_chi2_host.  Every array is a CPU tensor; returns when the outputs are complete."""
+    ft, bt = _host_batch(dtype, n_sn, n_samples, n_obs_total, obs_offset, time, band, zp, z, x0, x1, c, t0)
+    rc = _load().sb_chi2_host(model._h, bands._h, C.byref(bt), _hptr(flux, ft, n_obs_total, "flux"),
+                              _hptr(fluxerr, ft, n_obs_total, "fluxerr"),
+                              _hptr(out_chi2, ft, n_sn * n_samples, "out_chi2"),
+                              _hptr(out_flux, ft, n_obs_total * n_samples, "out_flux", allow_none=True))
+    _check(rc, "sb_chi2_host")
+
+
+def sb_bandflux_grad_host(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,
+                          obs_offset, time, band, zp, z, x0, x1, c, t0, flux=None, fluxerr=None, out_flux=None,
+                          out_dflux=None, out_chi2=None, out_dchi2=None) -> None:
+    """include/saltband.h: sb_bandflux_grad_host.  Gradient order: (x0, x1, c, t0)."""
+    ft, bt = _host_batch(dtype, n_sn, n_samples, n_obs_total, obs_offset, time, band, zp, z, x0, x1, c, t0)
+    n_ev, n_units = n_obs_total * n_samples, n_sn * n_samples
+    rc = _load().sb_bandflux_grad_host(
+        model._h, bands._h, C.byref(bt), _hptr(flux, ft, n_obs_total, "flux", allow_none=True),
+        _hptr(fluxerr, ft, n_obs_total, "fluxerr", allow_none=True),
+        _hptr(out_flux, ft, n_ev, "out_flux", allow_none=True),
+        _hptr(out_dflux, ft, n_ev * 4, "out_dflux", allow_none=True),
+        _hptr(out_chi2, ft, n_units, "out_chi2", allow_none=True),
+        _hptr(out_dchi2, ft, n_units * 4, "out_dchi2", allow_none=True))
+    _check(rc, "sb_bandflux_grad_host")

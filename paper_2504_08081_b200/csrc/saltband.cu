@@ -5,6 +5,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <type_traits>
 #include <vector>
 
 #include "sb_internal.h"
@@ -70,6 +71,21 @@ int device_smem_optin()
     if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) return 0;
     return v;
 }
+// Stream-ordered allocations (workspaces, staging buffers) come from the device's default memory pool;
+// keep freed blocks in the pool across synchronisation points instead of returning them to the driver.
+void keep_pool_memory()
+{
+    static thread_local int done_for_device = -1;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev == done_for_device) return;
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        unsigned long long thr = ~0ULL;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+    }
+    done_for_device = dev;
+}
+
 int device_sm_count()
 {
     int dev = 0, v = 0;
@@ -384,6 +400,7 @@ int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, 
 
     // workspace (stream-ordered): [0] group counter, [256] bin totals, [4096] z-order permutation, then
     // the per-segment bin counts of the sort
+    keep_pool_memory();
     unsigned char *ws = nullptr;
     const size_t perm_off = 4096, hist_off = perm_off + ((sizeof(int32_t) * (size_t)bt->n_sn + 255) & ~(size_t)255);
     const size_t ws_bytes = hist_off + sizeof(uint32_t) * (size_t)sbh::kZSegs * sbh::kZBins;
@@ -554,6 +571,184 @@ int sb_bandflux_grad(const sb_model *m, const sb_bands *b, const sb_batch *batch
                      void *stream)
 {
     return run(m, b, batch, flux, fluxerr, out_flux, out_dflux, out_chi2, out_dchi2, stream, true);
+}
+
+} // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// Host-buffer entry points: chunked staging with copy / compute overlap
+// ------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kHostStreams = 3;
+
+struct ChunkBufs {
+    int32_t *obs_offset = nullptr, *band = nullptr;
+    unsigned char *time = nullptr, *zp = nullptr, *flux = nullptr, *fluxerr = nullptr;
+    unsigned char *z = nullptr, *x0 = nullptr, *x1 = nullptr, *c = nullptr, *t0 = nullptr;
+    unsigned char *o_flux = nullptr, *o_dflux = nullptr, *o_chi2 = nullptr, *o_dchi2 = nullptr;
+};
+
+int run_host(const sb_model *m, const sb_bands *b, const sb_batch *hb, const void *flux, const void *fluxerr,
+             void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2, bool grad)
+{
+    tl_launches = 0;
+    tl_form = 0;
+    if (!m || !b || !hb) return SB_EINVAL;
+    const int32_t base_dtype = hb->dtype & 0xff;
+    if (base_dtype != SB_F32 && base_dtype != SB_F64) return SB_EINVAL;
+    if (hb->n_sn < 0 || hb->n_samples < 1 || hb->n_obs_total < 0) return SB_EINVAL;
+    if ((out_chi2 || out_dchi2) && (!flux || !fluxerr)) return SB_EINVAL;
+    if (!out_flux && !out_dflux && !out_chi2 && !out_dchi2) return SB_EINVAL;
+    if (hb->n_sn == 0) return SB_OK;
+    if (!hb->obs_offset || !hb->z || !hb->x0 || !hb->x1 || !hb->c || !hb->t0) return SB_EINVAL;
+    if (hb->n_obs_total > 0 && (!hb->time || !hb->band)) return SB_EINVAL;
+    if (hb->obs_offset[0] != 0 || hb->obs_offset[hb->n_sn] != hb->n_obs_total) return SB_EINVAL;
+    const size_t es = base_dtype == SB_F32 ? 4 : 8;
+    const long long ns = hb->n_samples;
+    const int n_sm = device_sm_count();
+    if (n_sm <= 0) return SB_ECUDA;
+
+    // chunks of supernovae: about 24 MB of inputs + outputs each, at most 32 chunks, and (one sample per
+    // supernova) a multiple of n_sm * 32 supernovae so that every chunk fills whole waves of groups
+    const double bytes_per_sn =
+        ((double)hb->n_obs_total / hb->n_sn) * (double)((hb->zp ? 3 : 2) * es + 4 + (flux ? 2 * es : 0) +
+                                                        (out_flux ? ns * es : 0) + (out_dflux ? 4 * ns * es : 0)) +
+        (double)(5 * ns * es);
+    long long chunk_sn = (long long)(24.0 * 1024 * 1024 / (bytes_per_sn > 1.0 ? bytes_per_sn : 1.0));
+    if (chunk_sn * 32 < hb->n_sn) chunk_sn = (hb->n_sn + 31) / 32;
+    const long long wave = (long long)n_sm * 32;
+    if (ns == 1 && chunk_sn > wave) chunk_sn = (chunk_sn / wave) * wave;
+    if (chunk_sn < 1) chunk_sn = 1;
+    if (chunk_sn > hb->n_sn) chunk_sn = hb->n_sn;
+    long long max_obs = 0; // observations of the largest chunk
+    for (long long s0 = 0; s0 < hb->n_sn; s0 += chunk_sn) {
+        const long long s1 = s0 + chunk_sn < hb->n_sn ? s0 + chunk_sn : hb->n_sn;
+        const long long n = (long long)hb->obs_offset[s1] - hb->obs_offset[s0];
+        if (n < 0) return SB_EINVAL;
+        if (n > max_obs) max_obs = n;
+    }
+
+    keep_pool_memory();
+    // internal streams: created once per host thread and device, then reused
+    static thread_local cudaStream_t tl_streams[kHostStreams] = {};
+    static thread_local int tl_streams_dev = -1;
+    int dev = 0;
+    if (!cuda_ok(cudaGetDevice(&dev))) return SB_ECUDA;
+    if (tl_streams_dev != dev) {
+        for (int i = 0; i < kHostStreams; ++i)
+            if (!cuda_ok(cudaStreamCreateWithFlags(&tl_streams[i], cudaStreamNonBlocking))) return SB_ECUDA;
+        tl_streams_dev = dev;
+    }
+    cudaStream_t *st = tl_streams;
+    // one stream-ordered allocation per stream, carved into the chunk's arrays (256-byte aligned)
+    ChunkBufs bufs[kHostStreams];
+    unsigned char *slab[kHostStreams] = {};
+    int rc = SB_OK;
+    const int n_streams = kHostStreams;
+    const size_t mo = (size_t)max_obs, mu = (size_t)(chunk_sn * ns);
+    for (int pass = 0; pass < 2 && rc == SB_OK; ++pass) { // pass 0: size, pass 1: carve
+        size_t total = 0;
+        for (int i = 0; i < (pass == 0 ? 1 : n_streams); ++i) {
+            size_t off = 0;
+            auto carve = [&](auto &ptr, size_t bytes) {
+                if (pass == 1) ptr = reinterpret_cast<std::remove_reference_t<decltype(ptr)>>(slab[i] + off);
+                off += (bytes + 255) & ~(size_t)255;
+            };
+            ChunkBufs &B = bufs[i];
+            carve(B.obs_offset, sizeof(int32_t) * (size_t)(chunk_sn + 1));
+            carve(B.band, sizeof(int32_t) * mo);
+            carve(B.time, es * mo);
+            if (hb->zp) carve(B.zp, es * mo);
+            if (flux) { carve(B.flux, es * mo); carve(B.fluxerr, es * mo); }
+            carve(B.z, es * (size_t)chunk_sn);
+            carve(B.x0, es * mu); carve(B.x1, es * mu); carve(B.c, es * mu); carve(B.t0, es * mu);
+            if (out_flux) carve(B.o_flux, es * mo * (size_t)ns);
+            if (out_dflux) carve(B.o_dflux, 4 * es * mo * (size_t)ns);
+            if (out_chi2) carve(B.o_chi2, es * mu);
+            if (out_dchi2) carve(B.o_dchi2, 4 * es * mu);
+            total = off;
+        }
+        if (pass == 0) {
+            for (int i = 0; i < n_streams && rc == SB_OK; ++i)
+                if (!cuda_ok(cudaMallocAsync((void **)&slab[i], total ? total : 256, st[i])))
+                    rc = tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+        }
+    }
+    int32_t launches = 0, form = 0;
+    int k = 0;
+    for (long long s0 = 0; s0 < hb->n_sn && rc == SB_OK; s0 += chunk_sn, ++k) {
+        const long long s1 = s0 + chunk_sn < hb->n_sn ? s0 + chunk_sn : hb->n_sn;
+        const long long o0 = hb->obs_offset[s0], o1 = hb->obs_offset[s1];
+        const size_t nsn = (size_t)(s1 - s0), nob = (size_t)(o1 - o0), nun = nsn * (size_t)ns;
+        cudaStream_t s = st[k % kHostStreams];
+        ChunkBufs &B = bufs[k % kHostStreams];
+        auto h2d = [&](void *dst, const void *src, size_t off, size_t bytes) {
+            if (rc == SB_OK && bytes && !cuda_ok(cudaMemcpyAsync(dst, (const unsigned char *)src + off, bytes, cudaMemcpyHostToDevice, s)))
+                rc = SB_ECUDA;
+        };
+        auto d2h = [&](void *dst, size_t off, const void *src, size_t bytes) {
+            if (rc == SB_OK && bytes && !cuda_ok(cudaMemcpyAsync((unsigned char *)dst + off, src, bytes, cudaMemcpyDeviceToHost, s)))
+                rc = SB_ECUDA;
+        };
+        h2d(B.obs_offset, hb->obs_offset, sizeof(int32_t) * (size_t)s0, sizeof(int32_t) * (nsn + 1));
+        h2d(B.band, hb->band, sizeof(int32_t) * (size_t)o0, sizeof(int32_t) * nob);
+        h2d(B.time, hb->time, es * (size_t)o0, es * nob);
+        if (hb->zp) h2d(B.zp, hb->zp, es * (size_t)o0, es * nob);
+        if (flux) { h2d(B.flux, flux, es * (size_t)o0, es * nob); h2d(B.fluxerr, fluxerr, es * (size_t)o0, es * nob); }
+        h2d(B.z, hb->z, es * (size_t)s0, es * nsn);
+        h2d(B.x0, hb->x0, es * (size_t)(s0 * ns), es * nun);
+        h2d(B.x1, hb->x1, es * (size_t)(s0 * ns), es * nun);
+        h2d(B.c, hb->c, es * (size_t)(s0 * ns), es * nun);
+        h2d(B.t0, hb->t0, es * (size_t)(s0 * ns), es * nun);
+        if (rc != SB_OK) break;
+        // the chunk keeps the caller's (absolute) observation offsets: per-observation device arrays are
+        // addressed through pointers shifted back by the chunk's first observation
+        sb_batch cb = *hb;
+        cb.n_sn = (int32_t)nsn;
+        cb.n_obs_total = (int32_t)nob;
+        cb.obs_offset = B.obs_offset;
+        cb.band = B.band - o0;
+        cb.time = B.time - es * (size_t)o0;
+        cb.zp = hb->zp ? B.zp - es * (size_t)o0 : nullptr;
+        cb.z = B.z; cb.x0 = B.x0; cb.x1 = B.x1; cb.c = B.c; cb.t0 = B.t0;
+        const void *d_flux = flux ? B.flux - es * (size_t)o0 : nullptr;
+        const void *d_err = flux ? B.fluxerr - es * (size_t)o0 : nullptr;
+        void *d_oflux = out_flux ? B.o_flux - es * (size_t)(o0 * ns) : nullptr;
+        void *d_odflux = out_dflux ? B.o_dflux - 4 * es * (size_t)(o0 * ns) : nullptr;
+        rc = run(m, b, &cb, d_flux, d_err, d_oflux, d_odflux, B.o_chi2, B.o_dchi2, (void *)s, grad);
+        launches += tl_launches;
+        if (tl_form) form = tl_form;
+        if (rc != SB_OK) break;
+        if (out_flux) d2h(out_flux, es * (size_t)(o0 * ns), B.o_flux, es * nob * (size_t)ns);
+        if (out_dflux) d2h(out_dflux, 4 * es * (size_t)(o0 * ns), B.o_dflux, 4 * es * nob * (size_t)ns);
+        if (out_chi2) d2h(out_chi2, es * (size_t)(s0 * ns), B.o_chi2, es * nun);
+        if (out_dchi2) d2h(out_dchi2, 4 * es * (size_t)(s0 * ns), B.o_dchi2, 4 * es * nun);
+    }
+    for (int i = 0; i < n_streams; ++i) {
+        if (slab[i]) cudaFreeAsync(slab[i], st[i]);
+        if (!cuda_ok(cudaStreamSynchronize(st[i])) && rc == SB_OK) rc = SB_ECUDA;
+    }
+    tl_launches = rc == SB_OK ? launches : 0;
+    tl_form = rc == SB_OK ? form : 0;
+    return rc;
+}
+
+} // namespace
+
+extern "C" {
+
+int sb_chi2_host(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux, const void *fluxerr,
+                 void *out_chi2, void *out_flux)
+{
+    if ((!out_chi2 || !flux || !fluxerr) && !(batch && batch->n_sn == 0)) { tl_launches = 0; return SB_EINVAL; }
+    return run_host(m, b, batch, flux, fluxerr, out_flux, nullptr, out_chi2, nullptr, false);
+}
+
+int sb_bandflux_grad_host(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+                          const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2)
+{
+    return run_host(m, b, batch, flux, fluxerr, out_flux, out_dflux, out_chi2, out_dchi2, true);
 }
 
 } // extern "C"

@@ -101,3 +101,36 @@ def test_full_size_config4_gradient_sampled_units(cuda_device):
     tol_g = sbgpu.dchi2_tolerance(sub, ref, tol_f, tol_d, 1, False)
     assert np.all(np.abs(g_dchi - ref["dchi2"]) <= tol_g)
     assert np.all(np.isfinite(got["dchi2"]))
+
+
+def test_full_size_config5_host_buffer_call_in_chunks(cuda_device):
+    """sb_chi2_host on the whole of config 5 (195 MB of pinned host buffers: eight chunks staged with
+    copy / compute overlap, the call bench.py's `e2e` times), sampled units against the oracle."""
+    import torch
+
+    import paper_2504_08081_b200 as sb
+
+    wl = workloads.make_workload(5)
+    idx = _sample_indices(wl.n_sn, 200, 91)
+    sub = _attach_sampled(wl, idx)
+    ref = oracle.run_workload(sub, want_flux=True, want_chi2=True)
+    model, bands = sbgpu.load_handles(wl)
+    ft = torch.float32
+
+    def pin(a, dtype=ft):
+        return torch.as_tensor(np.ascontiguousarray(a)).to(dtype).contiguous().pin_memory()
+
+    o_flux = torch.full((wl.n_evals,), float("nan"), dtype=ft).pin_memory()
+    o_chi = torch.full((wl.n_sn,), float("nan"), dtype=ft).pin_memory()
+    sb.sb_chi2_host(model, bands, dtype=sb.SB_F32, n_sn=wl.n_sn, n_samples=1, n_obs_total=wl.n_obs_total,
+                    obs_offset=pin(wl.obs_offset, torch.int32), time=pin(wl.time), band=pin(wl.band, torch.int32),
+                    zp=pin(wl.zp), z=pin(wl.z), x0=pin(wl.theta["x0"]), x1=pin(wl.theta["x1"]), c=pin(wl.theta["c"]),
+                    t0=pin(wl.theta["t0"]), flux=pin(wl.flux), fluxerr=pin(wl.fluxerr), out_chi2=o_chi, out_flux=o_flux)
+    assert sb.last_launch_count() >= 6 and sb.last_form() == "tiled"  # several chunks, three kernels each
+    got_flux, got_chi = o_flux.double().numpy(), o_chi.double().numpy()
+    assert np.all(np.isfinite(got_flux)) and np.all(np.isfinite(got_chi))  # every chunk wrote its outputs
+    tol = sbgpu.flux_tolerance(sub, ref["flux"], 1, False)
+    err = np.abs(_gather_units(wl, idx, got_flux, True) - ref["flux"])
+    assert np.all(err <= tol), f"worst flux err/tol {np.max(err / np.maximum(tol, 1e-300)):.3g}"
+    tolc = sbgpu.chi2_tolerance(sub, ref["flux"], tol, 1, False)
+    assert np.all(np.abs(_gather_units(wl, idx, got_chi, False) - ref["chi2"]) <= tolc)

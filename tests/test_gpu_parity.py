@@ -177,3 +177,47 @@ def test_gradient_formulations_on_samples_axis_and_ragged_units(cuda_device):
             tol_g = sbgpu.dchi2_tolerance(wl, ref, tol_f, tol_d, ns, False)
             errg = np.abs(got["dchi2"] - ref["dchi2"])
             assert np.all(errg <= tol_g), (config, form, np.max(errg / np.maximum(tol_g, 1e-300), axis=0))
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_host_buffer_calls_equal_device_calls(cuda_device, fp64):
+    """include/saltband.h sb_chi2_host / sb_bandflux_grad_host: staging of HOST buffers (pinned and
+    pageable) through the library's device buffers; a workload that fits one chunk gives bit-identical
+    results to the device calls, and matches the oracle.  (Several chunks: test_gpu_fullsize.py.)"""
+    import torch
+
+    import paper_2504_08081_b200 as sb
+
+    wl = prepare(2, n_sn=700, ragged=True)
+    ref = oracle_all(wl, grad=True)
+    dev = sbgpu.run_gpu(wl, mode="grad", fp64=fp64)
+    ft = torch.float64 if fp64 else torch.float32
+    model, bands = sbgpu.load_handles(wl)
+
+    def host(a, dtype=ft, pin=True):
+        t = torch.as_tensor(np.ascontiguousarray(np.asarray(a, dtype=np.float64))).to(dtype).contiguous()
+        return t.pin_memory() if pin else t
+
+    n_tot, n_units = wl.n_obs_total, wl.n_sn * wl.n_samples
+    for pin in (True, False):
+        common = dict(dtype=sb.SB_F64 if fp64 else sb.SB_F32, n_sn=wl.n_sn, n_samples=wl.n_samples, n_obs_total=n_tot,
+                      obs_offset=host(wl.obs_offset, torch.int32, pin), time=host(wl.time, ft, pin),
+                      band=host(wl.band, torch.int32, pin), zp=host(wl.zp, ft, pin), z=host(wl.z, ft, pin),
+                      x0=host(wl.theta["x0"], ft, pin), x1=host(wl.theta["x1"], ft, pin), c=host(wl.theta["c"], ft, pin),
+                      t0=host(wl.theta["t0"], ft, pin))
+        o_flux, o_dflux = torch.full((n_tot,), float("nan"), dtype=ft), torch.full((n_tot * 4,), float("nan"), dtype=ft)
+        o_chi, o_dchi = torch.full((n_units,), float("nan"), dtype=ft), torch.full((n_units * 4,), float("nan"), dtype=ft)
+        sb.sb_bandflux_grad_host(model, bands, flux=host(wl.flux, ft, pin), fluxerr=host(wl.fluxerr, ft, pin),
+                                 out_flux=o_flux, out_dflux=o_dflux, out_chi2=o_chi, out_dchi2=o_dchi, **common)
+        assert sb.last_launch_count() >= 1
+        assert np.array_equal(o_flux.double().numpy(), dev["flux"])
+        assert np.array_equal(o_dflux.double().numpy().reshape(-1, 4), dev["dflux"])
+        assert np.array_equal(o_chi.double().numpy(), dev["chi2"])
+        assert np.array_equal(o_dchi.double().numpy().reshape(-1, 4), dev["dchi2"])
+        o_chi2 = torch.full((n_units,), float("nan"), dtype=ft)
+        sb.sb_chi2_host(model, bands, flux=host(wl.flux, ft, pin), fluxerr=host(wl.fluxerr, ft, pin), out_chi2=o_chi2,
+                        **common)
+        tol = sbgpu.flux_tolerance(wl, ref["flux"], 1, fp64)
+        tolc = sbgpu.chi2_tolerance(wl, ref["flux"], tol, 1, fp64)
+        assert np.all(np.abs(o_chi2.double().numpy() - ref["chi2"]) <= tolc)
+    check_flux_chi2(wl, dev, ref, fp64)
