@@ -122,3 +122,38 @@ def test_single_band_phases_outside_grid_and_samples_axis(cuda_device):
     ref = oracle.run_workload(wl, want_flux=True)["flux"]
     assert 0.05 < np.mean(ref == 0.0) < 0.9  # the case does exercise out-of-grid phases
     check_all_forms(wl)
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13, 14, 15, 16])
+def test_random_grids_band_steps_and_redshifts(cuda_device, seed):
+    """Seeded random cases: model grid steps 2-25 A, band steps from a tenth of a model cell to
+    three cells (cells with no band sample at all), 1-5 bands partly outside the grid, redshifts
+    -0.05 .. 2, 1-40 units with 0-30 observations, 1-3 samples per supernova; every formulation."""
+    rng = np.random.default_rng(seed)
+    dw = float(rng.choice([2.0, 5.0, 10.0, 25.0]))
+    n_wave = int(rng.integers(40, 900))
+    wave = 2500.0 + dw * np.arange(n_wave)
+    md = smooth_model(int(rng.integers(4, 12)), wave, seed=seed)
+    bands = []
+    for _ in range(int(rng.integers(1, 6))):
+        h = dw * float(rng.choice([0.1, 0.37, 0.5, 1.0, 1.7, 3.0]))
+        lo = float(rng.uniform(wave[0] - 400.0, wave[-1] * 1.5))
+        n = int(rng.integers(5, 400))
+        w = lo + h * np.arange(n)
+        bands.append((w, 0.2 + 0.8 * np.exp(-0.5 * ((w - w.mean()) / (0.3 * (w[-1] - w[0]) + 1.0)) ** 2)))
+    bd = workloads.generators.pack_bands(bands)
+    n_sn, ns = int(rng.integers(1, 41)), int(rng.integers(1, 4))
+    counts = rng.integers(0, 31, n_sn)
+    off = np.concatenate([[0], np.cumsum(counts)])
+    n = int(off[-1])
+    nu = n_sn * ns
+    z = rng.uniform(-0.05, 2.0, n_sn)
+    th = {"x0": rng.uniform(1e-5, 3e-5, nu), "x1": rng.normal(size=nu), "c": 0.15 * rng.normal(size=nu),
+          "t0": rng.uniform(-2, 2, nu)}
+    phase = md["phase"]
+    wl = custom_workload(md, bd, off, rng.uniform(phase[0] - 2.0, (phase[-1] + 2.0) * 1.5, n),
+                         rng.integers(0, len(bands), n), z, th, n_samples=ns)
+    wl.theta_true = {k: v.reshape(n_sn, ns)[:, 0].copy() for k, v in wl.theta.items()}
+    if n == 0:
+        return
+    check_all_forms(attach(wl))
