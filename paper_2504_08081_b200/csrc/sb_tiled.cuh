@@ -289,6 +289,105 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
     }
 }
 
+// Forward variant that walks TWO passes (cells gq and gq + 32 of the lane) per iteration: the two cells'
+// colour-law / ex2 / moment chains are independent, which hides their fixed latencies with only four
+// warps per scheduler.  Same sums in the same order per cell as phase_a_passes.
+template <int NCL, int CM>
+__device__ __forceinline__ void phase_a_passes2(const SbModelParams &mp, const HSeg &S, const TItem &I, int w_lo,
+                                                int q_start, int q_a, int q_b, int q_lo,
+                                                const float *__restrict__ s_w, float *__restrict__ at_slot, int lane)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    HColour<NCL> col;
+#pragma unroll
+    for (int q = 0; q < NCL; ++q) col.a[q] = S.cl[q];
+    col.r_lo = (float)mp.r_lo;
+    col.r_hi = (float)mp.r_hi;
+    col.s_lo = S.s_lo;
+    col.s_hi = S.s_hi;
+    col.lin_a = I.lin_a;
+    col.lin_b = I.lin_b;
+    const int nW = mp.n_wave;
+    const float c0 = I.c0, inv_ha = I.inv_ha, ha_hi = I.ha_hi, ha_lo = I.ha_lo, hal = I.hal, r_first = I.r_first;
+    const int n_in = I.n_in, ncell = I.ncell;
+    auto jstart = [&](int x) {
+        int j = (int)ceilf(((float)x - c0) * inv_ha);
+        j = min(max(j, 0), n_in);
+        if (x >= ncell) j = n_in;
+        return j;
+    };
+    float pa0 = 0.f, pa1 = 0.f, pa2 = 0.f;
+    int gq = w_lo + 32 * q_start + lane + 1 - I.g_first;
+    int carry = jstart(gq);
+    const float *wbase = s_w + I.wbase;
+    float *outp = at_slot + (q_start - q_lo) * 32 + lane;
+    auto from_left = [&](float cur, float prev, int d) {
+        const float a = __shfl_up_sync(FULL, cur, d);
+        const float b = __shfl_sync(FULL, prev, (lane - d) & 31);
+        return lane >= d ? a : b;
+    };
+    auto node_weight = [&](int g, float m0, float m1, float m2, float m3) {
+        float am = 0.5f * (__fmaf_rn(2.0f, m2, -m3) - m1);
+        float a0 = __fmaf_rn(1.5f, m3, __fmaf_rn(-2.5f, m2, m0));
+        float a1 = 0.5f * (__fmaf_rn(4.0f, m2, m1) - 3.0f * m3);
+        float a2 = 0.5f * (m3 - m2);
+        if (g <= 0 || g >= nW - 2) { // linear border cells (G2)
+            am = 0.f;
+            a0 = m0 - m1;
+            a1 = m1;
+            a2 = 0.f;
+        }
+        const float at = am + from_left(a0, pa0, 1) + from_left(a1, pa1, 2) + from_left(a2, pa2, 3);
+        pa0 = a0;
+        pa1 = a1;
+        pa2 = a2;
+        return at;
+    };
+#pragma unroll 1
+    for (int q = q_start; q < q_b; q += 2) {
+        const int jeA = jstart(gq + 1), jeB = jstart(gq + 33);
+        int jsA = __shfl_up_sync(FULL, jeA, 1), jsB = __shfl_up_sync(FULL, jeB, 1);
+        const int lastA = __shfl_sync(FULL, jeA, 31);
+        if (lane == 0) { jsA = carry; jsB = lastA; }
+        carry = __shfl_sync(FULL, jeB, 31);
+        const int cntA = jeA - jsA, cntB = jeB - jsB;
+        const float fA = (float)jsA, fB = (float)jsB;
+        float tA = __fmaf_rn(fA, ha_lo, __fmaf_rn(fA, ha_hi, -(float)gq)) + c0;
+        float tB = __fmaf_rn(fB, ha_lo, __fmaf_rn(fB, ha_hi, -(float)(gq + 32))) + c0;
+        float rA = __fmaf_rn(fA, hal, r_first), rB = __fmaf_rn(fB, hal, r_first);
+        const float *wpA = wbase + jsA, *wpB = wbase + jsB;
+        const int km = __reduce_max_sync(FULL, max(cntA, cntB));
+        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, b0 = 0.f, b1 = 0.f, b2 = 0.f, b3 = 0.f;
+#pragma unroll 1
+        for (int k = 0; k < km; ++k) { // one sample of each of the two cells per trip
+            float wA = 0.f, wB = 0.f;
+            if (k < cntA) wA = wpA[k];
+            if (k < cntB) wB = wpB[k];
+            const float eA = sb::exp_scaled(col.template arg<CM>(rA)) * wA;
+            const float eB = sb::exp_scaled(col.template arg<CM>(rB)) * wB;
+            const float tA2 = tA * tA, tB2 = tB * tB;
+            a0 += eA;
+            b0 += eB;
+            a1 = __fmaf_rn(eA, tA, a1);
+            b1 = __fmaf_rn(eB, tB, b1);
+            a2 = __fmaf_rn(eA, tA2, a2);
+            b2 = __fmaf_rn(eB, tB2, b2);
+            a3 = __fmaf_rn(eA, tA2 * tA, a3);
+            b3 = __fmaf_rn(eB, tB2 * tB, b3);
+            tA += ha_hi;
+            tB += ha_hi;
+            rA += hal;
+            rB += hal;
+        }
+        const float atA = node_weight(I.g_first + gq, a0, a1, a2, a3);
+        const float atB = node_weight(I.g_first + gq + 32, b0, b1, b2, b3);
+        if (q >= q_a) outp[0] = atA;
+        if (q + 1 >= q_a && q + 1 < q_b) outp[32] = atB;
+        outp += 64;
+        gq += 64;
+    }
+}
+
 template <int NCL, bool GRAD>
 __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg &S, const TItem &I, int w_lo,
                                              int q_lo, int q_hi, const float *__restrict__ s_w,
@@ -314,6 +413,15 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg
     }
     if (q_a >= q_b) return;
     const int q_start = q_a > qa ? q_a - 1 : q_a;
+    if constexpr (!GRAD) {
+        if (I.cmode == sb::CM_INSIDE)
+            phase_a_passes2<NCL, sb::CM_INSIDE>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+        else if (I.cmode == sb::CM_LINEAR)
+            phase_a_passes2<NCL, sb::CM_LINEAR>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+        else
+            phase_a_passes2<NCL, sb::CM_GENERIC>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+        return;
+    }
     if (I.cmode == sb::CM_INSIDE)
         phase_a_passes<NCL, sb::CM_INSIDE, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
     else if (I.cmode == sb::CM_LINEAR)
