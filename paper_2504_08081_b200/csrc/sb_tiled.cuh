@@ -168,8 +168,10 @@ __device__ __forceinline__ void item_geometry(const SbHParams &P, const HSeg &S,
 // and w_2 of cell n-2 (lane - 3); lanes 0..2 take them from the previous pass (carried in registers;
 // when the segment starts inside the item's window the pass before it is recomputed for its carries).
 // Passes outside the item's own nodes [n_lo, n_end) are zero filled.
-// GRAD: the colour law is evaluated unscaled (CL itself; exponent = CL * c log2(e)) and a second set
-// of moments, weighted by CL, gives the node weights of d/dc (at_slot + kW).
+// The loop walks TWO passes (cells gq and gq + 32 of the lane) per iteration: the two cells' colour-law /
+// ex2 / moment chains are independent, which hides their fixed latencies with only four warps per
+// scheduler.  GRAD: the colour law is evaluated unscaled (CL itself; exponent = CL * c log2(e)) and a
+// second set of moments, weighted by CL, gives the node weights of d/dc (at_slot + kW).
 template <int NCL, int CM, bool GRAD>
 __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HSeg &S, const TItem &I, int w_lo,
                                                int q_start, int q_a, int q_b, int q_lo,
@@ -188,7 +190,6 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
     const float cs = (float)(S.cc * 1.4426950408889634); // GRAD: exponent in log2 units = CL * cs
     const int nW = mp.n_wave;
     const float c0 = I.c0, inv_ha = I.inv_ha, ha_hi = I.ha_hi, ha_lo = I.ha_lo, hal = I.hal, r_first = I.r_first;
-    const float ha2 = 2.0f * ha_hi, hal2 = 2.0f * hal;
     const int n_in = I.n_in, ncell = I.ncell;
     auto jstart = [&](int x) { // first band sample (relative to the first in-range one) of cell x
         int j = (int)ceilf(((float)x - c0) * inv_ha);
@@ -198,127 +199,8 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
     };
     float pa0 = 0.f, pa1 = 0.f, pa2 = 0.f;
     float pc0 = 0.f, pc1 = 0.f, pc2 = 0.f; // GRAD: carries of the d/dc weights
-    int gq = w_lo + 32 * q_start + lane + 1 - I.g_first; // this lane's cell relative to g_first
+    int gq = w_lo + 32 * q_start + lane + 1 - I.g_first; // this lane's cell (first pass) relative to g_first
     int carry = jstart(gq);                                // lane 0: start of its cell
-    const float *wbase = s_w + I.wbase;
-    float *outp = at_slot + (q_start - q_lo) * 32 + lane;
-#pragma unroll 1
-    for (int q = q_start; q < q_b; ++q) {
-        const int je = jstart(gq + 1);
-        int js = __shfl_up_sync(FULL, je, 1);
-        if (lane == 0) js = carry;
-        carry = __shfl_sync(FULL, je, 31);
-        const int cnt = je - js;
-        const float jsf = (float)js;
-        float tau = __fmaf_rn(jsf, ha_lo, __fmaf_rn(jsf, ha_hi, -(float)gq)) + c0; // u_js - cell
-        float r = __fmaf_rn(jsf, hal, r_first);
-        const float *wp = wbase + js;
-        const int km = __reduce_max_sync(FULL, cnt);
-        float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-        float d0 = 0.f, d1 = 0.f, d2 = 0.f, d3 = 0.f; // GRAD: moments weighted by CL
-        auto sample = [&](float e, float cl, float t) { // one band sample into the cell's moments
-            const float t2 = t * t, t3 = t2 * t;
-            s0 += e;
-            s1 = __fmaf_rn(e, t, s1);
-            s2 = __fmaf_rn(e, t2, s2);
-            s3 = __fmaf_rn(e, t3, s3);
-            if (GRAD) {
-                const float c = e * cl;
-                d0 += c;
-                d1 = __fmaf_rn(c, t, d1);
-                d2 = __fmaf_rn(c, t2, d2);
-                d3 = __fmaf_rn(c, t3, d3);
-            }
-        };
-        int k = 0;
-#pragma unroll 1
-        for (; k + 2 <= km; k += 2) { // two samples per trip: independent colour-law chains
-            float w0 = 0.f, w1 = 0.f;
-            if (k < cnt) w0 = wp[0];
-            if (k + 1 < cnt) w1 = wp[1];
-            const float ra = r, rb = r + hal;
-            const float ta = tau, tb = tau + ha_hi;
-            const float cla = col.template arg<CM>(ra), clb = col.template arg<CM>(rb);
-            const float ea = sb::exp_scaled(GRAD ? cla * cs : cla) * w0;
-            const float eb = sb::exp_scaled(GRAD ? clb * cs : clb) * w1;
-            sample(ea, cla, ta);
-            sample(eb, clb, tb);
-            tau += ha2;
-            r += hal2;
-            wp += 2;
-        }
-        if (k < km) { // odd trip count: one more sample
-            float w0 = 0.f;
-            if (k < cnt) w0 = wp[0];
-            const float cla = col.template arg<CM>(r);
-            sample(sb::exp_scaled(GRAD ? cla * cs : cla) * w0, cla, tau);
-        }
-        // moments -> weights on the cell's four nodes (Keys a = -1/2; linear in border cells, G2)
-        const int g = I.g_first + gq;
-        const bool border = g <= 0 || g >= nW - 2;
-        auto from_left = [&](float cur, float prev, int d) {
-            const float a = __shfl_up_sync(FULL, cur, d);
-            const float b = __shfl_sync(FULL, prev, (lane - d) & 31);
-            return lane >= d ? a : b;
-        };
-        auto node_weight = [&](float m0, float m1, float m2, float m3, float &p0, float &p1, float &p2) {
-            float am = 0.5f * (__fmaf_rn(2.0f, m2, -m3) - m1);
-            float a0 = __fmaf_rn(1.5f, m3, __fmaf_rn(-2.5f, m2, m0));
-            float a1 = 0.5f * (__fmaf_rn(4.0f, m2, m1) - 3.0f * m3);
-            float a2 = 0.5f * (m3 - m2);
-            if (border) {
-                am = 0.f;
-                a0 = m0 - m1;
-                a1 = m1;
-                a2 = 0.f;
-            }
-            const float at = am + from_left(a0, p0, 1) + from_left(a1, p1, 2) + from_left(a2, p2, 3);
-            p0 = a0;
-            p1 = a1;
-            p2 = a2;
-            return at;
-        };
-        const float at = node_weight(s0, s1, s2, s3, pa0, pa1, pa2);
-        if (q >= q_a) *outp = at;
-        if (GRAD) {
-            const float atc = node_weight(d0, d1, d2, d3, pc0, pc1, pc2);
-            if (q >= q_a) outp[kW] = atc;
-        }
-        outp += 32;
-        gq += 32;
-    }
-}
-
-// Forward variant that walks TWO passes (cells gq and gq + 32 of the lane) per iteration: the two cells'
-// colour-law / ex2 / moment chains are independent, which hides their fixed latencies with only four
-// warps per scheduler.  Same sums in the same order per cell as phase_a_passes.
-template <int NCL, int CM>
-__device__ __forceinline__ void phase_a_passes2(const SbModelParams &mp, const HSeg &S, const TItem &I, int w_lo,
-                                                int q_start, int q_a, int q_b, int q_lo,
-                                                const float *__restrict__ s_w, float *__restrict__ at_slot, int lane)
-{
-    constexpr unsigned FULL = 0xffffffffu;
-    HColour<NCL> col;
-#pragma unroll
-    for (int q = 0; q < NCL; ++q) col.a[q] = S.cl[q];
-    col.r_lo = (float)mp.r_lo;
-    col.r_hi = (float)mp.r_hi;
-    col.s_lo = S.s_lo;
-    col.s_hi = S.s_hi;
-    col.lin_a = I.lin_a;
-    col.lin_b = I.lin_b;
-    const int nW = mp.n_wave;
-    const float c0 = I.c0, inv_ha = I.inv_ha, ha_hi = I.ha_hi, ha_lo = I.ha_lo, hal = I.hal, r_first = I.r_first;
-    const int n_in = I.n_in, ncell = I.ncell;
-    auto jstart = [&](int x) {
-        int j = (int)ceilf(((float)x - c0) * inv_ha);
-        j = min(max(j, 0), n_in);
-        if (x >= ncell) j = n_in;
-        return j;
-    };
-    float pa0 = 0.f, pa1 = 0.f, pa2 = 0.f;
-    int gq = w_lo + 32 * q_start + lane + 1 - I.g_first;
-    int carry = jstart(gq);
     const float *wbase = s_w + I.wbase;
     float *outp = at_slot + (q_start - q_lo) * 32 + lane;
     auto from_left = [&](float cur, float prev, int d) {
@@ -326,21 +208,23 @@ __device__ __forceinline__ void phase_a_passes2(const SbModelParams &mp, const H
         const float b = __shfl_sync(FULL, prev, (lane - d) & 31);
         return lane >= d ? a : b;
     };
-    auto node_weight = [&](int g, float m0, float m1, float m2, float m3) {
+    // moments of cell g -> weights on its four nodes (Keys a = -1/2; linear in border cells, G2); the
+    // lane's node takes this cell's w_-1 and w_0, w_1, w_2 of the three cells to the left
+    auto node_weight = [&](int g, float m0, float m1, float m2, float m3, float &p0, float &p1, float &p2) {
         float am = 0.5f * (__fmaf_rn(2.0f, m2, -m3) - m1);
         float a0 = __fmaf_rn(1.5f, m3, __fmaf_rn(-2.5f, m2, m0));
         float a1 = 0.5f * (__fmaf_rn(4.0f, m2, m1) - 3.0f * m3);
         float a2 = 0.5f * (m3 - m2);
-        if (g <= 0 || g >= nW - 2) { // linear border cells (G2)
+        if (g <= 0 || g >= nW - 2) {
             am = 0.f;
             a0 = m0 - m1;
             a1 = m1;
             a2 = 0.f;
         }
-        const float at = am + from_left(a0, pa0, 1) + from_left(a1, pa1, 2) + from_left(a2, pa2, 3);
-        pa0 = a0;
-        pa1 = a1;
-        pa2 = a2;
+        const float at = am + from_left(a0, p0, 1) + from_left(a1, p1, 2) + from_left(a2, p2, 3);
+        p0 = a0;
+        p1 = a1;
+        p2 = a2;
         return at;
     };
 #pragma unroll 1
@@ -352,37 +236,58 @@ __device__ __forceinline__ void phase_a_passes2(const SbModelParams &mp, const H
         carry = __shfl_sync(FULL, jeB, 31);
         const int cntA = jeA - jsA, cntB = jeB - jsB;
         const float fA = (float)jsA, fB = (float)jsB;
-        float tA = __fmaf_rn(fA, ha_lo, __fmaf_rn(fA, ha_hi, -(float)gq)) + c0;
+        float tA = __fmaf_rn(fA, ha_lo, __fmaf_rn(fA, ha_hi, -(float)gq)) + c0; // u_js - cell
         float tB = __fmaf_rn(fB, ha_lo, __fmaf_rn(fB, ha_hi, -(float)(gq + 32))) + c0;
         float rA = __fmaf_rn(fA, hal, r_first), rB = __fmaf_rn(fB, hal, r_first);
         const float *wpA = wbase + jsA, *wpB = wbase + jsB;
         const int km = __reduce_max_sync(FULL, max(cntA, cntB));
         float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, b0 = 0.f, b1 = 0.f, b2 = 0.f, b3 = 0.f;
+        float ca0 = 0.f, ca1 = 0.f, ca2 = 0.f, ca3 = 0.f, cb0 = 0.f, cb1 = 0.f, cb2 = 0.f, cb3 = 0.f; // GRAD
 #pragma unroll 1
         for (int k = 0; k < km; ++k) { // one sample of each of the two cells per trip
             float wA = 0.f, wB = 0.f;
             if (k < cntA) wA = wpA[k];
             if (k < cntB) wB = wpB[k];
-            const float eA = sb::exp_scaled(col.template arg<CM>(rA)) * wA;
-            const float eB = sb::exp_scaled(col.template arg<CM>(rB)) * wB;
+            const float clA = col.template arg<CM>(rA), clB = col.template arg<CM>(rB);
+            const float eA = sb::exp_scaled(GRAD ? clA * cs : clA) * wA;
+            const float eB = sb::exp_scaled(GRAD ? clB * cs : clB) * wB;
             const float tA2 = tA * tA, tB2 = tB * tB;
+            const float tA3 = tA2 * tA, tB3 = tB2 * tB;
             a0 += eA;
             b0 += eB;
             a1 = __fmaf_rn(eA, tA, a1);
             b1 = __fmaf_rn(eB, tB, b1);
             a2 = __fmaf_rn(eA, tA2, a2);
             b2 = __fmaf_rn(eB, tB2, b2);
-            a3 = __fmaf_rn(eA, tA2 * tA, a3);
-            b3 = __fmaf_rn(eB, tB2 * tB, b3);
+            a3 = __fmaf_rn(eA, tA3, a3);
+            b3 = __fmaf_rn(eB, tB3, b3);
+            if (GRAD) {
+                const float gA = eA * clA, gB = eB * clB;
+                ca0 += gA;
+                cb0 += gB;
+                ca1 = __fmaf_rn(gA, tA, ca1);
+                cb1 = __fmaf_rn(gB, tB, cb1);
+                ca2 = __fmaf_rn(gA, tA2, ca2);
+                cb2 = __fmaf_rn(gB, tB2, cb2);
+                ca3 = __fmaf_rn(gA, tA3, ca3);
+                cb3 = __fmaf_rn(gB, tB3, cb3);
+            }
             tA += ha_hi;
             tB += ha_hi;
             rA += hal;
             rB += hal;
         }
-        const float atA = node_weight(I.g_first + gq, a0, a1, a2, a3);
-        const float atB = node_weight(I.g_first + gq + 32, b0, b1, b2, b3);
-        if (q >= q_a) outp[0] = atA;
-        if (q + 1 >= q_a && q + 1 < q_b) outp[32] = atB;
+        const bool stA = q >= q_a, stB = q + 1 >= q_a && q + 1 < q_b;
+        const float atA = node_weight(I.g_first + gq, a0, a1, a2, a3, pa0, pa1, pa2);
+        const float atB = node_weight(I.g_first + gq + 32, b0, b1, b2, b3, pa0, pa1, pa2);
+        if (stA) outp[0] = atA;
+        if (stB) outp[32] = atB;
+        if (GRAD) {
+            const float acA = node_weight(I.g_first + gq, ca0, ca1, ca2, ca3, pc0, pc1, pc2);
+            const float acB = node_weight(I.g_first + gq + 32, cb0, cb1, cb2, cb3, pc0, pc1, pc2);
+            if (stA) outp[kW] = acA;
+            if (stB) outp[kW + 32] = acB;
+        }
         outp += 64;
         gq += 64;
     }
@@ -413,15 +318,6 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg
     }
     if (q_a >= q_b) return;
     const int q_start = q_a > qa ? q_a - 1 : q_a;
-    if constexpr (!GRAD) {
-        if (I.cmode == sb::CM_INSIDE)
-            phase_a_passes2<NCL, sb::CM_INSIDE>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
-        else if (I.cmode == sb::CM_LINEAR)
-            phase_a_passes2<NCL, sb::CM_LINEAR>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
-        else
-            phase_a_passes2<NCL, sb::CM_GENERIC>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
-        return;
-    }
     if (I.cmode == sb::CM_INSIDE)
         phase_a_passes<NCL, sb::CM_INSIDE, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
     else if (I.cmode == sb::CM_LINEAR)
