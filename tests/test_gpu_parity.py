@@ -221,3 +221,42 @@ def test_host_buffer_calls_equal_device_calls(cuda_device, fp64):
         tolc = sbgpu.chi2_tolerance(wl, ref["flux"], tol, 1, fp64)
         assert np.all(np.abs(o_chi2.double().numpy() - ref["chi2"]) <= tolc)
     check_flux_chi2(wl, dev, ref, fp64)
+
+
+def test_host_buffer_call_chunks_with_samples_axis(cuda_device):
+    """sb_chi2_host with several parameter samples per supernova and several chunks (the flux output
+    of one supernova is 0.9 MB, so the 24 MB chunk target cuts 90 supernovae into four chunks).  In
+    fp64 the library runs the per-evaluation kernel, whose results do not depend on how units are
+    grouped: the chunked host call must equal the whole-batch device call bit for bit (flux) and to
+    rounding of the per-unit sum (chi^2)."""
+    import torch
+
+    import paper_2504_08081_b200 as sb
+
+    wl = workloads.make_workload(2, n_sn=90, ragged=True)
+    ns = 2000
+    rng = np.random.default_rng(17)
+    nu = wl.n_sn * ns
+    th = {"x0": np.repeat(wl.theta["x0"], ns) * rng.uniform(0.8, 1.2, nu), "x1": rng.normal(size=nu),
+          "c": 0.1 * rng.normal(size=nu), "t0": rng.uniform(-3, 3, nu)}
+    th = {k: v.astype(np.float32).astype(np.float64) for k, v in th.items()}
+    wl.flux = (1e-3 * wl.noise).astype(np.float32)
+    wl.fluxerr = np.full(wl.n_obs_total, 1e-3, dtype=np.float32)
+    dev = sbgpu.run_gpu(wl, mode="chi2", fp64=True, theta=th)
+    model, bands = sbgpu.load_handles(wl)
+    ft = torch.float64
+
+    def host(a, dtype=ft):
+        return torch.as_tensor(np.ascontiguousarray(np.asarray(a, dtype=np.float64))).to(dtype).contiguous().pin_memory()
+
+    n_tot = wl.n_obs_total
+    o_flux = torch.full((n_tot * ns,), float("nan"), dtype=ft).pin_memory()
+    o_chi = torch.full((nu,), float("nan"), dtype=ft).pin_memory()
+    sb.sb_chi2_host(model, bands, dtype=sb.SB_F64, n_sn=wl.n_sn, n_samples=ns, n_obs_total=n_tot,
+                    obs_offset=host(wl.obs_offset, torch.int32), time=host(wl.time), band=host(wl.band, torch.int32),
+                    zp=host(wl.zp), z=host(wl.z), x0=host(th["x0"]), x1=host(th["x1"]), c=host(th["c"]),
+                    t0=host(th["t0"]), flux=host(wl.flux), fluxerr=host(wl.fluxerr), out_chi2=o_chi, out_flux=o_flux)
+    assert sb.last_launch_count() >= 3  # one direct-kernel launch per chunk
+    assert np.array_equal(o_flux.numpy(), dev["flux"])
+    # chi^2: the partial sums of a unit follow the kernel's evaluation chunks, which depend on the batch
+    assert np.all(np.abs(o_chi.numpy() - dev["chi2"]) <= 1e-13 * np.abs(dev["chi2"]))
