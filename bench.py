@@ -204,9 +204,12 @@ def oracle_sample_samples(wl, k: int):
         theta_true=wl.theta_true, theta=th, noise=wl.noise)
 
 
-def time_oracle(wl, evals_target: int, steps: int, warmup: int):
-    """Time the oracle, as it stands, on a bounded prefix of the workload (host cores of this box)."""
+def time_oracle(wl, evals_target: int, steps: int, warmup: int, threads=None):
+    """Time the oracle, as it stands, on a bounded prefix of the workload (host cores of this box;
+    `threads` = None: all of them)."""
     import oracle
+
+    kw = {"threads": int(threads) if threads else len(os.sched_getaffinity(0))}
 
     if wl.n_samples > 1:
         k = max(1, min(wl.n_samples, evals_target // max(wl.n_obs_total, 1)))
@@ -220,11 +223,11 @@ def time_oracle(wl, evals_target: int, steps: int, warmup: int):
     true = oracle.run_workload(sub, theta={k_: v.copy() for k_, v in sub.theta_true.items()})["flux"]
     workloads.attach_data(sub, true)
     for _ in range(warmup):
-        oracle.run_workload(sub, want_flux=True, want_chi2=True)
+        oracle.run_workload(sub, want_flux=True, want_chi2=True, **kw)
     t = []
     for _ in range(steps):
         t0 = time.perf_counter()
-        oracle.run_workload(sub, want_flux=True, want_chi2=True)
+        oracle.run_workload(sub, want_flux=True, want_chi2=True, **kw)
         t.append(time.perf_counter() - t0)
     sec = float(np.mean(t))
     return sub.n_evals / sec, sec, oracle.num_threads(), sample
@@ -474,6 +477,8 @@ def main():
     if world == 1 and not args.no_cpu_baseline:
         v, sec, cores, sample = time_oracle(wl, args.cpu_evals, 1, 0)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": sec}
+        v1, sec1, _, sample1 = time_oracle(wl, max(args.cpu_evals // 48, 4000), 1, 0, threads=1)
+        cpu["single_thread"] = {"value": v1, "unit": UNIT, "cores": 1, "sample": sample1, "seconds": sec1}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
