@@ -443,13 +443,18 @@ int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, 
     int rc = SB_OK;
     static_assert(256 + sizeof(uint32_t) * sbh::kZBins <= 4096, "bin totals overlap the permutation");
     uint32_t *z_tot = reinterpret_cast<uint32_t *>(ws + 256), *z_hist = reinterpret_cast<uint32_t *>(ws + hist_off);
-    if (!cuda_ok(cudaMemsetAsync(ws, 0, perm_off, st))) rc = SB_ECUDA;
-    if (rc == SB_OK) {
-        sbh::sb_zhist_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(hp.z, hp.n_sn, z_hist, z_tot, hp.counter);
-        sbh::sb_zscatter_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(hp.z, hp.n_sn, z_hist, z_tot,
-                                                                          reinterpret_cast<int32_t *>(ws + perm_off));
+    if (hp.n_sn <= sbh::kZSmall) { // one launch; the main kernel's launch is counted below
+        sbh::sb_zorder_small_kernel<<<1, 512, 0, st>>>(hp.z, hp.n_sn, reinterpret_cast<int32_t *>(ws + perm_off), hp.counter);
         if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
-        else tl_launches += 1; // the second of the two; the first is counted below
+    } else {
+        if (!cuda_ok(cudaMemsetAsync(ws, 0, perm_off, st))) rc = SB_ECUDA;
+        if (rc == SB_OK) {
+            sbh::sb_zhist_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(hp.z, hp.n_sn, z_hist, z_tot, hp.counter);
+            sbh::sb_zscatter_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(hp.z, hp.n_sn, z_hist, z_tot,
+                                                                              reinterpret_cast<int32_t *>(ws + perm_off));
+            if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
+            else tl_launches += 1; // the second of the two; the first is counted below
+        }
     }
     if (rc == SB_OK) {
         tl_launches += 1;

@@ -186,6 +186,65 @@ __global__ void __launch_bounds__(kZWarps * 32, 1) sb_zscatter_kernel(const floa
     }
 }
 
+// Small batches (n_sn <= kZSmall): the same stable sort in ONE CTA of 16 warps (no workspace, no memset,
+// one launch instead of two): warp w owns a contiguous range and a private counter row.
+constexpr int kZSmall = 8192;
+__global__ void __launch_bounds__(512, 1) sb_zorder_small_kernel(const float *__restrict__ z, int n_sn, int32_t *perm,
+                                                                 unsigned int *counter)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    constexpr int NWZ = 16;
+    __shared__ uint32_t cnt[NWZ][kZBins]; // 32 KB
+    __shared__ uint32_t wsum[NWZ];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) *counter = 0u;
+    for (int i = tid; i < NWZ * kZBins; i += NWZ * 32) (&cnt[0][0])[i] = 0u;
+    __syncthreads();
+    const int chunk = (((n_sn + NWZ - 1) / NWZ) + 31) & ~31;
+    const int lo = min(warp * chunk, n_sn), hi = min(lo + chunk, n_sn);
+    uint32_t *mine = cnt[warp];
+    for (int i0 = lo; i0 < hi; i0 += 32) {
+        const int bn = i0 + lane < hi ? z_bin(z, i0 + lane) : -1;
+        const unsigned m = __match_any_sync(FULL, bn);
+        if (bn >= 0 && lane == __ffs(m) - 1) mine[bn] += (uint32_t)__popc(m);
+        __syncwarp();
+    }
+    __syncthreads();
+    { // bin t: exclusive prefix over the warps, then over the bins (NWZ * 32 == kZBins threads)
+        const int t = tid;
+        uint32_t s = 0;
+#pragma unroll
+        for (int w = 0; w < NWZ; ++w) {
+            const uint32_t c = cnt[w][t];
+            cnt[w][t] = s;
+            s += c;
+        }
+        uint32_t incl = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(FULL, incl, o);
+            if (lane >= o) incl += v;
+        }
+        if (lane == 31) wsum[warp] = incl;
+        __syncthreads();
+        uint32_t base = incl - s;
+        for (int w = 0; w < warp; ++w) base += wsum[w];
+#pragma unroll
+        for (int w = 0; w < NWZ; ++w) cnt[w][t] += base;
+    }
+    __syncthreads();
+    for (int i0 = lo; i0 < hi; i0 += 32) {
+        const int bn = i0 + lane < hi ? z_bin(z, i0 + lane) : -1;
+        const unsigned m = __match_any_sync(FULL, bn);
+        const uint32_t at = bn >= 0 ? mine[bn] : 0u;
+        __syncwarp();
+        if (bn >= 0 && lane == __ffs(m) - 1) mine[bn] = at + (uint32_t)__popc(m);
+        __syncwarp();
+        if (bn >= 0) perm[at + (uint32_t)__popc(m & ((1u << lane) - 1u))] = i0 + lane;
+    }
+}
+static_assert(kZBins == 512, "sb_zorder_small_kernel: one thread per bin");
+
 // ---- colour law of one item: exponent argument (log2 units) as a function of the reduced wavelength
 template <int NCL> struct HColour {
     float a[NCL];
