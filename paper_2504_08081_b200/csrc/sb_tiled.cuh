@@ -329,8 +329,11 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const HSeg
 // ---- phase B: observations [i_lo, i_hi) of the sorted list (all of one band) on one warp ----------
 // Node window of 256 (TWO = true) or 128 nodes starting at node n0, whose weights start at float
 // a_off of every item slot: lane l owns nodes n0 + 4 l .. + 3 and n0 + 128 + 4 l .. + 3.
+// All products of the contraction are issued as packed FP32 pairs (FFMA2 / FMUL2, sm_100): the kernel is
+// bound by instruction issue, not by the FMA pipe, and a pair takes one issue slot.  A pair is two
+// neighbouring nodes of the lane; each element sees exactly the scalar sequence of fused multiply-adds.
 struct RowRegs {
-    float m0[4][kNPL], m1[4][kNPL]; // [slot = row mod 4][node]
+    float2 m0[4][kNPL / 2], m1[4][kNPL / 2]; // [slot = row mod 4][node pair]
 };
 
 template <bool TWO>
@@ -346,11 +349,11 @@ __device__ __forceinline__ void load_row(RowRegs &R, int s, const float *__restr
         b = __ldg(reinterpret_cast<const float4 *>(p0 + 128));
         d = __ldg(reinterpret_cast<const float4 *>(p1 + 128));
     }
-    R.m0[s][0] = a.x; R.m0[s][1] = a.y; R.m0[s][2] = a.z; R.m0[s][3] = a.w;
-    R.m1[s][0] = c.x; R.m1[s][1] = c.y; R.m1[s][2] = c.z; R.m1[s][3] = c.w;
+    R.m0[s][0] = make_float2(a.x, a.y); R.m0[s][1] = make_float2(a.z, a.w);
+    R.m1[s][0] = make_float2(c.x, c.y); R.m1[s][1] = make_float2(c.z, c.w);
     if (TWO) {
-        R.m0[s][4] = b.x; R.m0[s][5] = b.y; R.m0[s][6] = b.z; R.m0[s][7] = b.w;
-        R.m1[s][4] = d.x; R.m1[s][5] = d.y; R.m1[s][6] = d.z; R.m1[s][7] = d.w;
+        R.m0[s][2] = make_float2(b.x, b.y); R.m0[s][3] = make_float2(b.z, b.w);
+        R.m1[s][2] = make_float2(d.x, d.y); R.m1[s][3] = make_float2(d.z, d.w);
     }
 }
 
@@ -371,7 +374,7 @@ __device__ __forceinline__ void phase_b_window(const SbHParams &P, int n0, const
 #pragma unroll
     for (int s = 0; s < 4; ++s)
 #pragma unroll
-        for (int q = 0; q < kNPL; ++q) { R.m0[s][q] = 0.f; R.m1[s][q] = 0.f; }
+        for (int q = 0; q < kNPL / 2; ++q) { R.m0[s][q] = make_float2(0.f, 0.f); R.m1[s][q] = make_float2(0.f, 0.f); }
 
     auto one = [&](int i) -> float { // the window's share of observation i of the sorted list
         const uint32_t info = s_info[i];
@@ -390,36 +393,39 @@ __device__ __forceinline__ void phase_b_window(const SbHParams &P, int n0, const
         }
         const float4 w4 = s_ws[i];
         const float x1 = s_x1[slot];
-        const float ws[4] = {w4.x, w4.y, w4.z, w4.w};
-        const float vs[4] = {w4.x * x1, w4.y * x1, w4.z * x1, w4.w * x1};
+        const float2 xx = make_float2(x1, x1);
+        const float2 ws[4] = {make_float2(w4.x, w4.x), make_float2(w4.y, w4.y), make_float2(w4.z, w4.z),
+                              make_float2(w4.w, w4.w)};
+        const float2 vs[4] = {__fmul2_rn(ws[0], xx), __fmul2_rn(ws[1], xx), __fmul2_rn(ws[2], xx), __fmul2_rn(ws[3], xx)};
         const float *ap = s_at_l + slot * kW;
-        float a = 0.f;
+        float2 a2 = make_float2(0.f, 0.f); // even / odd nodes of the lane
         {
             const float4 t = lds128(ap);
-            const float av[4] = {t.x, t.y, t.z, t.w};
+            const float2 av[2] = {make_float2(t.x, t.y), make_float2(t.z, t.w)};
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                float r = ws[0] * R.m0[0][q];
+            for (int q = 0; q < 2; ++q) {
+                float2 r = __fmul2_rn(ws[0], R.m0[0][q]);
 #pragma unroll
-                for (int s = 1; s < 4; ++s) r = __fmaf_rn(ws[s], R.m0[s][q], r);
+                for (int s = 1; s < 4; ++s) r = __ffma2_rn(ws[s], R.m0[s][q], r);
 #pragma unroll
-                for (int s = 0; s < 4; ++s) r = __fmaf_rn(vs[s], R.m1[s][q], r);
-                a = __fmaf_rn(av[q], r, a);
+                for (int s = 0; s < 4; ++s) r = __ffma2_rn(vs[s], R.m1[s][q], r);
+                a2 = __ffma2_rn(av[q], r, a2);
             }
         }
         if (TWO) {
             const float4 t = lds128(ap + 128);
-            const float av[4] = {t.x, t.y, t.z, t.w};
+            const float2 av[2] = {make_float2(t.x, t.y), make_float2(t.z, t.w)};
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                float r = ws[0] * R.m0[0][4 + q];
+            for (int q = 0; q < 2; ++q) {
+                float2 r = __fmul2_rn(ws[0], R.m0[0][2 + q]);
 #pragma unroll
-                for (int s = 1; s < 4; ++s) r = __fmaf_rn(ws[s], R.m0[s][4 + q], r);
+                for (int s = 1; s < 4; ++s) r = __ffma2_rn(ws[s], R.m0[s][2 + q], r);
 #pragma unroll
-                for (int s = 0; s < 4; ++s) r = __fmaf_rn(vs[s], R.m1[s][4 + q], r);
-                a = __fmaf_rn(av[q], r, a);
+                for (int s = 0; s < 4; ++s) r = __ffma2_rn(vs[s], R.m1[s][2 + q], r);
+                a2 = __ffma2_rn(av[q], r, a2);
             }
         }
+        const float a = a2.x + a2.y;
         return a;
     };
 
