@@ -269,6 +269,26 @@ template <int NCL> struct HColour {
             return __fmaf_rn(slope, d, p);
         }
     }
+    // the same for two wavelengths at once, as packed FP32 pairs (one issue slot per pair of FMAs)
+    template <int CM> __device__ __forceinline__ float2 arg2(float2 r) const
+    {
+        if constexpr (CM == sb::CM_LINEAR) {
+            return __ffma2_rn(r, make_float2(lin_b, lin_b), make_float2(lin_a, lin_a));
+        } else if constexpr (CM == sb::CM_INSIDE) {
+            float2 p = make_float2(a[NCL - 1], a[NCL - 1]);
+#pragma unroll
+            for (int q = NCL - 2; q >= 0; --q) p = __ffma2_rn(p, r, make_float2(a[q], a[q]));
+            return p;
+        } else {
+            const float2 rc = make_float2(fminf(fmaxf(r.x, r_lo), r_hi), fminf(fmaxf(r.y, r_lo), r_hi));
+            const float2 d = make_float2(r.x - rc.x, r.y - rc.y);
+            const float2 slope = make_float2(d.x > 0.0f ? s_hi : s_lo, d.y > 0.0f ? s_hi : s_lo);
+            float2 p = make_float2(a[NCL - 1], a[NCL - 1]);
+#pragma unroll
+            for (int q = NCL - 2; q >= 0; --q) p = __ffma2_rn(p, rc, make_float2(a[q], a[q]));
+            return __ffma2_rn(slope, d, p);
+        }
+    }
 };
 
 // Geometry of one item (unit, band): warp-uniform values.

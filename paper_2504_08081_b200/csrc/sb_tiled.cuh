@@ -241,42 +241,38 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
         float rA = __fmaf_rn(fA, hal, r_first), rB = __fmaf_rn(fB, hal, r_first);
         const float *wpA = wbase + jsA, *wpB = wbase + jsB;
         const int km = __reduce_max_sync(FULL, max(cntA, cntB));
-        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, b0 = 0.f, b1 = 0.f, b2 = 0.f, b3 = 0.f;
-        float ca0 = 0.f, ca1 = 0.f, ca2 = 0.f, ca3 = 0.f, cb0 = 0.f, cb1 = 0.f, cb2 = 0.f, cb3 = 0.f; // GRAD
+        // moments of the two cells as packed FP32 pairs (.x: cell gq, .y: cell gq + 32): FFMA2 / FMUL2 /
+        // FADD2 take one issue slot per pair and give each element the scalar sequence of operations
+        float2 m0 = make_float2(0.f, 0.f), m1 = m0, m2 = m0, m3 = m0;
+        float2 n0 = m0, n1 = m0, n2 = m0, n3 = m0; // GRAD: weighted by CL
+        float2 t2v = make_float2(tA, tB), r2v = make_float2(rA, rB);
+        const float2 hh = make_float2(ha_hi, ha_hi), ll = make_float2(hal, hal), cc2 = make_float2(cs, cs);
 #pragma unroll 1
         for (int k = 0; k < km; ++k) { // one sample of each of the two cells per trip
-            float wA = 0.f, wB = 0.f;
-            if (k < cntA) wA = wpA[k];
-            if (k < cntB) wB = wpB[k];
-            const float clA = col.template arg<CM>(rA), clB = col.template arg<CM>(rB);
-            const float eA = sb::exp_scaled(GRAD ? clA * cs : clA) * wA;
-            const float eB = sb::exp_scaled(GRAD ? clB * cs : clB) * wB;
-            const float tA2 = tA * tA, tB2 = tB * tB;
-            const float tA3 = tA2 * tA, tB3 = tB2 * tB;
-            a0 += eA;
-            b0 += eB;
-            a1 = __fmaf_rn(eA, tA, a1);
-            b1 = __fmaf_rn(eB, tB, b1);
-            a2 = __fmaf_rn(eA, tA2, a2);
-            b2 = __fmaf_rn(eB, tB2, b2);
-            a3 = __fmaf_rn(eA, tA3, a3);
-            b3 = __fmaf_rn(eB, tB3, b3);
+            float2 w = make_float2(0.f, 0.f);
+            if (k < cntA) w.x = wpA[k];
+            if (k < cntB) w.y = wpB[k];
+            const float2 cl = col.template arg2<CM>(r2v);
+            const float2 ar = GRAD ? __fmul2_rn(cl, cc2) : cl;
+            const float2 e = __fmul2_rn(make_float2(sb::exp_scaled(ar.x), sb::exp_scaled(ar.y)), w);
+            const float2 tt = __fmul2_rn(t2v, t2v);
+            const float2 ttt = __fmul2_rn(tt, t2v);
+            m0 = __fadd2_rn(m0, e);
+            m1 = __ffma2_rn(e, t2v, m1);
+            m2 = __ffma2_rn(e, tt, m2);
+            m3 = __ffma2_rn(e, ttt, m3);
             if (GRAD) {
-                const float gA = eA * clA, gB = eB * clB;
-                ca0 += gA;
-                cb0 += gB;
-                ca1 = __fmaf_rn(gA, tA, ca1);
-                cb1 = __fmaf_rn(gB, tB, cb1);
-                ca2 = __fmaf_rn(gA, tA2, ca2);
-                cb2 = __fmaf_rn(gB, tB2, cb2);
-                ca3 = __fmaf_rn(gA, tA3, ca3);
-                cb3 = __fmaf_rn(gB, tB3, cb3);
+                const float2 g = __fmul2_rn(e, cl);
+                n0 = __fadd2_rn(n0, g);
+                n1 = __ffma2_rn(g, t2v, n1);
+                n2 = __ffma2_rn(g, tt, n2);
+                n3 = __ffma2_rn(g, ttt, n3);
             }
-            tA += ha_hi;
-            tB += ha_hi;
-            rA += hal;
-            rB += hal;
+            t2v = __fadd2_rn(t2v, hh);
+            r2v = __fadd2_rn(r2v, ll);
         }
+        const float a0 = m0.x, a1 = m1.x, a2 = m2.x, a3 = m3.x, b0 = m0.y, b1 = m1.y, b2 = m2.y, b3 = m3.y;
+        const float ca0 = n0.x, ca1 = n1.x, ca2 = n2.x, ca3 = n3.x, cb0 = n0.y, cb1 = n1.y, cb2 = n2.y, cb3 = n3.y;
         const bool stA = q >= q_a, stB = q + 1 >= q_a && q + 1 < q_b;
         const float atA = node_weight(I.g_first + gq, a0, a1, a2, a3, pa0, pa1, pa2);
         const float atB = node_weight(I.g_first + gq + 32, b0, b1, b2, b3, pa0, pa1, pa2);
