@@ -454,7 +454,7 @@ __device__ __forceinline__ void phase_b_window_grad(const SbHParams &P, int n0, 
                                                     int cap, int i_lo, int i_hi, int lane)
 {
     const int ld = P.mp.ld;
-    float m0[4][4], m1[4][4]; // [slot = row mod 4][node]
+    float2 m0[4][2], m1[4][2]; // [slot = row mod 4][node pair]: packed FP32 pairs as in phase_b_window
     int held[4] = {-1, -1, -1, -1};
     int rb_held = -1;
     const int col = n0 + SB_PAD_L + 4 * lane;
@@ -463,7 +463,7 @@ __device__ __forceinline__ void phase_b_window_grad(const SbHParams &P, int n0, 
 #pragma unroll
     for (int s = 0; s < 4; ++s)
 #pragma unroll
-        for (int q = 0; q < 4; ++q) { m0[s][q] = 0.f; m1[s][q] = 0.f; }
+        for (int q = 0; q < 2; ++q) { m0[s][q] = make_float2(0.f, 0.f); m1[s][q] = make_float2(0.f, 0.f); }
 
     auto one = [&](int i, float *acc) { // acc[0..3] = value, M1-only, d/dc, d/dt0 shares of observation i
         const uint32_t info = s_info[i];
@@ -480,39 +480,43 @@ __device__ __forceinline__ void phase_b_window_grad(const SbHParams &P, int n0, 
                         a = __ldg(reinterpret_cast<const float4 *>(p0 + ro));
                         c = __ldg(reinterpret_cast<const float4 *>(p1 + ro));
                     }
-                    m0[s][0] = a.x; m0[s][1] = a.y; m0[s][2] = a.z; m0[s][3] = a.w;
-                    m1[s][0] = c.x; m1[s][1] = c.y; m1[s][2] = c.z; m1[s][3] = c.w;
+                    m0[s][0] = make_float2(a.x, a.y); m0[s][1] = make_float2(a.z, a.w);
+                    m1[s][0] = make_float2(c.x, c.y); m1[s][1] = make_float2(c.z, c.w);
                     held[s] = row;
                 }
             }
         }
         const float4 w4 = s_ws[i], d4 = s_wd[i];
         const float x1 = s_x1[slot];
-        const float ws[4] = {w4.x, w4.y, w4.z, w4.w};
-        const float wd[4] = {d4.x, d4.y, d4.z, d4.w};
-        const float vd[4] = {d4.x * x1, d4.y * x1, d4.z * x1, d4.w * x1};
+        const float2 xx = make_float2(x1, x1);
+        const float2 ws[4] = {make_float2(w4.x, w4.x), make_float2(w4.y, w4.y), make_float2(w4.z, w4.z),
+                              make_float2(w4.w, w4.w)};
+        const float2 wd[4] = {make_float2(d4.x, d4.x), make_float2(d4.y, d4.y), make_float2(d4.z, d4.z),
+                              make_float2(d4.w, d4.w)};
+        const float2 vd[4] = {__fmul2_rn(wd[0], xx), __fmul2_rn(wd[1], xx), __fmul2_rn(wd[2], xx), __fmul2_rn(wd[3], xx)};
         const float *ap = s_at_l + slot * (2 * kW);
         const float4 t = lds128(ap), tc = lds128(ap + kW);
-        const float av[4] = {t.x, t.y, t.z, t.w};
-        const float ac[4] = {tc.x, tc.y, tc.z, tc.w};
-        float a = 0.f, a1 = 0.f, a_c = 0.f, a_d = 0.f;
+        const float2 av[2] = {make_float2(t.x, t.y), make_float2(t.z, t.w)};
+        const float2 ac[2] = {make_float2(tc.x, tc.y), make_float2(tc.z, tc.w)};
+        float2 s_a = make_float2(0.f, 0.f), s_1 = s_a, s_c = s_a, s_d = s_a; // even / odd nodes
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            float r0 = ws[0] * m0[0][q], r1 = ws[0] * m1[0][q], rd = wd[0] * m0[0][q];
+        for (int q = 0; q < 2; ++q) {
+            float2 r0 = __fmul2_rn(ws[0], m0[0][q]), r1 = __fmul2_rn(ws[0], m1[0][q]), rd = __fmul2_rn(wd[0], m0[0][q]);
 #pragma unroll
             for (int s = 1; s < 4; ++s) {
-                r0 = __fmaf_rn(ws[s], m0[s][q], r0);
-                r1 = __fmaf_rn(ws[s], m1[s][q], r1);
-                rd = __fmaf_rn(wd[s], m0[s][q], rd);
+                r0 = __ffma2_rn(ws[s], m0[s][q], r0);
+                r1 = __ffma2_rn(ws[s], m1[s][q], r1);
+                rd = __ffma2_rn(wd[s], m0[s][q], rd);
             }
 #pragma unroll
-            for (int s = 0; s < 4; ++s) rd = __fmaf_rn(vd[s], m1[s][q], rd);
-            const float r = __fmaf_rn(x1, r1, r0);
-            a = __fmaf_rn(av[q], r, a);
-            a1 = __fmaf_rn(av[q], r1, a1);
-            a_c = __fmaf_rn(ac[q], r, a_c);
-            a_d = __fmaf_rn(av[q], rd, a_d);
+            for (int s = 0; s < 4; ++s) rd = __ffma2_rn(vd[s], m1[s][q], rd);
+            const float2 r = __ffma2_rn(xx, r1, r0);
+            s_a = __ffma2_rn(av[q], r, s_a);
+            s_1 = __ffma2_rn(av[q], r1, s_1);
+            s_c = __ffma2_rn(ac[q], r, s_c);
+            s_d = __ffma2_rn(av[q], rd, s_d);
         }
+        const float a = s_a.x + s_a.y, a1 = s_1.x + s_1.y, a_c = s_c.x + s_c.y, a_d = s_d.x + s_d.y;
         acc[0] = a; acc[1] = a1; acc[2] = a_c; acc[3] = a_d;
     };
 
