@@ -208,24 +208,30 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
         const float b = __shfl_sync(FULL, prev, (lane - d) & 31);
         return lane >= d ? a : b;
     };
-    // moments of cell g -> weights on its four nodes (Keys a = -1/2; linear in border cells, G2); the
-    // lane's node takes this cell's w_-1 and w_0, w_1, w_2 of the three cells to the left
-    auto node_weight = [&](int g, float m0, float m1, float m2, float m3, float &p0, float &p1, float &p2) {
-        float am = 0.5f * (__fmaf_rn(2.0f, m2, -m3) - m1);
-        float a0 = __fmaf_rn(1.5f, m3, __fmaf_rn(-2.5f, m2, m0));
-        float a1 = 0.5f * (__fmaf_rn(4.0f, m2, m1) - 3.0f * m3);
-        float a2 = 0.5f * (m3 - m2);
+    // moments of the lane's two cells (.x: cell g, .y: cell g + 32) -> weights on their four nodes (Keys
+    // a = -1/2; linear in border cells, G2), packed; the lane's node of each pass takes its cell's w_-1
+    // and w_0, w_1, w_2 of the three cells to the left (previous pass for lanes 0..2: p0..p2, which for
+    // the second cell are the first cell's values)
+    auto node_weights = [&](int g, float2 m0, float2 m1, float2 m2, float2 m3, float &p0, float &p1, float &p2) {
+        const float2 half = make_float2(0.5f, 0.5f);
+        float2 am = __fmul2_rn(half, __fadd2_rn(__ffma2_rn(make_float2(2.0f, 2.0f), m2, make_float2(-m3.x, -m3.y)),
+                                                 make_float2(-m1.x, -m1.y)));
+        float2 a0 = __ffma2_rn(make_float2(1.5f, 1.5f), m3, __ffma2_rn(make_float2(-2.5f, -2.5f), m2, m0));
+        float2 a1 = __fmul2_rn(half, __ffma2_rn(make_float2(-3.0f, -3.0f), m3, __ffma2_rn(make_float2(4.0f, 4.0f), m2, m1)));
+        float2 a2 = __fmul2_rn(half, __fadd2_rn(m3, make_float2(-m2.x, -m2.y)));
         if (g <= 0 || g >= nW - 2) {
-            am = 0.f;
-            a0 = m0 - m1;
-            a1 = m1;
-            a2 = 0.f;
+            am.x = 0.f; a0.x = m0.x - m1.x; a1.x = m1.x; a2.x = 0.f;
         }
-        const float at = am + from_left(a0, p0, 1) + from_left(a1, p1, 2) + from_left(a2, p2, 3);
-        p0 = a0;
-        p1 = a1;
-        p2 = a2;
-        return at;
+        if (g + 32 <= 0 || g + 32 >= nW - 2) {
+            am.y = 0.f; a0.y = m0.y - m1.y; a1.y = m1.y; a2.y = 0.f;
+        }
+        const float2 l0 = make_float2(from_left(a0.x, p0, 1), from_left(a0.y, a0.x, 1));
+        const float2 l1 = make_float2(from_left(a1.x, p1, 2), from_left(a1.y, a1.x, 2));
+        const float2 l2 = make_float2(from_left(a2.x, p2, 3), from_left(a2.y, a2.x, 3));
+        p0 = a0.y;
+        p1 = a1.y;
+        p2 = a2.y;
+        return __fadd2_rn(__fadd2_rn(__fadd2_rn(am, l0), l1), l2);
     };
 #pragma unroll 1
     for (int q = q_start; q < q_b; q += 2) {
@@ -236,17 +242,19 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
         carry = __shfl_sync(FULL, jeB, 31);
         const int cntA = jeA - jsA, cntB = jeB - jsB;
         const float fA = (float)jsA, fB = (float)jsB;
-        float tA = __fmaf_rn(fA, ha_lo, __fmaf_rn(fA, ha_hi, -(float)gq)) + c0; // u_js - cell
-        float tB = __fmaf_rn(fB, ha_lo, __fmaf_rn(fB, ha_hi, -(float)(gq + 32))) + c0;
-        float rA = __fmaf_rn(fA, hal, r_first), rB = __fmaf_rn(fB, hal, r_first);
+        const float2 f2 = make_float2(fA, fB);
         const float *wpA = wbase + jsA, *wpB = wbase + jsB;
         const int km = __reduce_max_sync(FULL, max(cntA, cntB));
         // moments of the two cells as packed FP32 pairs (.x: cell gq, .y: cell gq + 32): FFMA2 / FMUL2 /
         // FADD2 take one issue slot per pair and give each element the scalar sequence of operations
         float2 m0 = make_float2(0.f, 0.f), m1 = m0, m2 = m0, m3 = m0;
         float2 n0 = m0, n1 = m0, n2 = m0, n3 = m0; // GRAD: weighted by CL
-        float2 t2v = make_float2(tA, tB), r2v = make_float2(rA, rB);
         const float2 hh = make_float2(ha_hi, ha_hi), ll = make_float2(hal, hal), cc2 = make_float2(cs, cs);
+        // u_js - cell, and the reduced wavelength of the first sample, of both cells
+        float2 t2v = __fadd2_rn(__ffma2_rn(f2, make_float2(ha_lo, ha_lo),
+                                           __ffma2_rn(f2, hh, make_float2(-(float)gq, -(float)(gq + 32)))),
+                                make_float2(c0, c0));
+        float2 r2v = __ffma2_rn(f2, ll, make_float2(r_first, r_first));
 #pragma unroll 1
         for (int k = 0; k < km; ++k) { // one sample of each of the two cells per trip
             float2 w = make_float2(0.f, 0.f);
@@ -271,18 +279,14 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const HS
             t2v = __fadd2_rn(t2v, hh);
             r2v = __fadd2_rn(r2v, ll);
         }
-        const float a0 = m0.x, a1 = m1.x, a2 = m2.x, a3 = m3.x, b0 = m0.y, b1 = m1.y, b2 = m2.y, b3 = m3.y;
-        const float ca0 = n0.x, ca1 = n1.x, ca2 = n2.x, ca3 = n3.x, cb0 = n0.y, cb1 = n1.y, cb2 = n2.y, cb3 = n3.y;
         const bool stA = q >= q_a, stB = q + 1 >= q_a && q + 1 < q_b;
-        const float atA = node_weight(I.g_first + gq, a0, a1, a2, a3, pa0, pa1, pa2);
-        const float atB = node_weight(I.g_first + gq + 32, b0, b1, b2, b3, pa0, pa1, pa2);
-        if (stA) outp[0] = atA;
-        if (stB) outp[32] = atB;
+        const float2 at = node_weights(I.g_first + gq, m0, m1, m2, m3, pa0, pa1, pa2);
+        if (stA) outp[0] = at.x;
+        if (stB) outp[32] = at.y;
         if (GRAD) {
-            const float acA = node_weight(I.g_first + gq, ca0, ca1, ca2, ca3, pc0, pc1, pc2);
-            const float acB = node_weight(I.g_first + gq + 32, cb0, cb1, cb2, cb3, pc0, pc1, pc2);
-            if (stA) outp[kW] = acA;
-            if (stB) outp[kW + 32] = acB;
+            const float2 ac = node_weights(I.g_first + gq, n0, n1, n2, n3, pc0, pc1, pc2);
+            if (stA) outp[kW] = ac.x;
+            if (stB) outp[kW + 32] = ac.y;
         }
         outp += 64;
         gq += 64;
