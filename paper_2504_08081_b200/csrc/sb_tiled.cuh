@@ -376,64 +376,85 @@ __device__ __forceinline__ void phase_b_window(const SbHParams &P, int n0, const
 #pragma unroll
         for (int q = 0; q < kNPL / 2; ++q) { R.m0[s][q] = make_float2(0.f, 0.f); R.m1[s][q] = make_float2(0.f, 0.f); }
 
-    auto one = [&](int i) -> float { // the window's share of observation i of the sorted list
-        const uint32_t info = s_info[i];
-        const int slot = (int)(info & 31u), rb = (int)((info >> 5) & 4095u);
-        if (rb != rb_held) { // rows rb .. rb+3, row r in register slot r mod 4: reload only what changed
-            rb_held = rb;
+    auto rows = [&](int rb) { // rows rb .. rb+3, row r in register slot r mod 4: reload only what changed
+        if (rb == rb_held) return;
+        rb_held = rb;
 #pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                const int row = rb + ((s - rb) & 3);
-                if (held[s] != row) {
-                    const ptrdiff_t ro = (ptrdiff_t)row * ld;
-                    load_row<TWO>(R, s, p0 + ro, p1 + ro, ok_lo, ok_hi);
-                    held[s] = row;
+        for (int s = 0; s < 4; ++s) {
+            const int row = rb + ((s - rb) & 3);
+            if (held[s] != row) {
+                const ptrdiff_t ro = (ptrdiff_t)row * ld;
+                load_row<TWO>(R, s, p0 + ro, p1 + ro, ok_lo, ok_hi);
+                held[s] = row;
+            }
+        }
+    };
+    // NOBS observations that use the same four rows (already in R) at once: 4 NOBS independent chains of
+    // packed pairs per 128-node half.  x1 is applied to M1 first (t = M0 + x1 M1), so an observation
+    // keeps only its four row weights and x1 in registers.
+    auto compute = [&](auto nobs_tag, int i, float *out) {
+        constexpr int NOBS = decltype(nobs_tag)::value;
+        float2 ws[NOBS][4], xx[NOBS], a2[NOBS];
+        const float *ap[NOBS];
+#pragma unroll
+        for (int o = 0; o < NOBS; ++o) {
+            const int slot = (int)(s_info[i + o] & 31u);
+            const float4 w4 = s_ws[i + o];
+            const float x1 = s_x1[slot];
+            xx[o] = make_float2(x1, x1);
+            ws[o][0] = make_float2(w4.x, w4.x); ws[o][1] = make_float2(w4.y, w4.y);
+            ws[o][2] = make_float2(w4.z, w4.z); ws[o][3] = make_float2(w4.w, w4.w);
+            ap[o] = s_at_l + slot * kW;
+            a2[o] = make_float2(0.f, 0.f); // even / odd nodes of the lane
+        }
+#pragma unroll
+        for (int hf = 0; hf < (TWO ? 2 : 1); ++hf) {
+            float2 av[NOBS][2];
+#pragma unroll
+            for (int o = 0; o < NOBS; ++o) {
+                const float4 t = lds128(ap[o] + 128 * hf);
+                av[o][0] = make_float2(t.x, t.y);
+                av[o][1] = make_float2(t.z, t.w);
+            }
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+#pragma unroll
+                for (int o = 0; o < NOBS; ++o) {
+                    float2 r = __fmul2_rn(ws[o][0], __ffma2_rn(xx[o], R.m1[0][2 * hf + q], R.m0[0][2 * hf + q]));
+#pragma unroll
+                    for (int s = 1; s < 4; ++s)
+                        r = __ffma2_rn(ws[o][s], __ffma2_rn(xx[o], R.m1[s][2 * hf + q], R.m0[s][2 * hf + q]), r);
+                    a2[o] = __ffma2_rn(av[o][q], r, a2[o]);
                 }
             }
         }
-        const float4 w4 = s_ws[i];
-        const float x1 = s_x1[slot];
-        const float2 xx = make_float2(x1, x1);
-        const float2 ws[4] = {make_float2(w4.x, w4.x), make_float2(w4.y, w4.y), make_float2(w4.z, w4.z),
-                              make_float2(w4.w, w4.w)};
-        const float2 vs[4] = {__fmul2_rn(ws[0], xx), __fmul2_rn(ws[1], xx), __fmul2_rn(ws[2], xx), __fmul2_rn(ws[3], xx)};
-        const float *ap = s_at_l + slot * kW;
-        float2 a2 = make_float2(0.f, 0.f); // even / odd nodes of the lane
-        {
-            const float4 t = lds128(ap);
-            const float2 av[2] = {make_float2(t.x, t.y), make_float2(t.z, t.w)};
 #pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                float2 r = __fmul2_rn(ws[0], R.m0[0][q]);
-#pragma unroll
-                for (int s = 1; s < 4; ++s) r = __ffma2_rn(ws[s], R.m0[s][q], r);
-#pragma unroll
-                for (int s = 0; s < 4; ++s) r = __ffma2_rn(vs[s], R.m1[s][q], r);
-                a2 = __ffma2_rn(av[q], r, a2);
-            }
+        for (int o = 0; o < NOBS; ++o) out[o] = a2[o].x + a2[o].y;
+    };
+    auto rb_of = [&](int i) { return (int)((s_info[i] >> 5) & 4095u); };
+    auto pair_of = [&](int i, float *out) { // observations i and i + 1
+        const int rbA = rb_of(i), rbB = rb_of(i + 1);
+        rows(rbA);
+        if (rbA == rbB) {
+            compute(std::integral_constant<int, 2>{}, i, out);
+        } else {
+            compute(std::integral_constant<int, 1>{}, i, out);
+            rows(rbB);
+            compute(std::integral_constant<int, 1>{}, i + 1, out + 1);
         }
-        if (TWO) {
-            const float4 t = lds128(ap + 128);
-            const float2 av[2] = {make_float2(t.x, t.y), make_float2(t.z, t.w)};
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                float2 r = __fmul2_rn(ws[0], R.m0[0][2 + q]);
-#pragma unroll
-                for (int s = 1; s < 4; ++s) r = __ffma2_rn(ws[s], R.m0[s][2 + q], r);
-#pragma unroll
-                for (int s = 0; s < 4; ++s) r = __ffma2_rn(vs[s], R.m1[s][2 + q], r);
-                a2 = __ffma2_rn(av[q], r, a2);
-            }
-        }
-        const float a = a2.x + a2.y;
-        return a;
+    };
+    auto one = [&](int i) -> float {
+        float v;
+        rows(rb_of(i));
+        compute(std::integral_constant<int, 1>{}, i, &v);
+        return v;
     };
 
     int i = i_lo;
     for (; i + 4 <= i_hi; i += 4) {
         float acc[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[j] = one(i + j);
+        pair_of(i, acc);
+        pair_of(i + 2, acc + 2);
         const float v = sbh::warp_reduce_transpose<4>(acc, lane); // lane L: total of observation i + (L >> 3)
         if ((lane & 7) == 0) res[s_info[i + (lane >> 3)] >> 17] += v;
     }
