@@ -143,6 +143,7 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
     p.n_cl = n_cl;
     p.p0 = phase[0];
     p.dp = (phase[n_phase - 1] - phase[0]) / (double)(n_phase - 1);
+    p.inv_dp = 1.0 / p.dp;
     p.l0 = wave[0];
     p.dl = (wave[n_wave - 1] - wave[0]) / (double)(n_wave - 1);
     for (int q = 0; q < SB_MAX_CL; ++q) p.cl[q] = q < n_cl ? cl_coef[q] : 0.0;

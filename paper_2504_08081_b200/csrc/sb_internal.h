@@ -27,6 +27,7 @@ struct SbModelParams {
     double cl_b, cl_inv_span;          // reduced wavelength r = (l - cl_b) * cl_inv_span
     double r_lo, r_hi;                 // images of cl_lo, cl_hi
     double p_lo, s_lo, p_hi, s_hi;     // polynomial value and slope at r_lo, r_hi
+    double inv_dp;                     // 1 / dp (the tiled kernel multiplies instead of dividing)
 };
 
 // Interleaved {M0, M1} fp32 table of the band-grouped kernel (sb_hoist.cuh): [n_phase][SBH_LDN]

@@ -568,12 +568,12 @@ __device__ __forceinline__ bool obs_phase(const SbModelParams &mp, const HSeg &S
 {
     const int nP = mp.n_phase;
     const double p = ((double)t - S.t0) * S.inv_opz;
-    const double up = (p - mp.p0) / mp.dp;
+    const double up = (p - mp.p0) * mp.inv_dp;
     if (!((up >= 0.0) && (up <= (double)(nP - 1)))) return false;
     const int kp = min((int)floor(up), nP - 2);
     double wv[4], wd[4];
     // d/dt0 of the weights: d tau/d t0 = -1/((1+z) dP)
-    sb::phase_weights(up - (double)kp, (kp == 0) || (kp == nP - 2), -S.inv_opz / mp.dp, wv, wd);
+    sb::phase_weights(up - (double)kp, (kp == 0) || (kp == nP - 2), -S.inv_opz * mp.inv_dp, wv, wd);
     rb = min(max(kp - 1, 0), nP - 4);
     const int shift = (kp - 1) - rb; // row rb + k carries Keys weight index k - shift
 #pragma unroll
@@ -878,6 +878,8 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
 
             // ---- epilogue: one warp per segment; a6 zero point (fp64), flux [, gradient] out (coalesced),
             // a7 chi^2 [, a8 d chi^2/d theta = -2 sum (f - m)/sigma^2 dm/dtheta] in a fixed order
+            float zp_last = __int_as_float(0x7fc00000); // NaN: never equal
+            double zp_pow = 1.0;
             for (int sg = warp; sg < n_seg; sg += kWarps) {
                 const HSeg &S = segs[sg];
                 constexpr int NS = GRAD ? 5 : 1;
@@ -891,7 +893,14 @@ __global__ void __launch_bounds__(kThreads, 1) sb_tiled_kernel(const __grid_cons
                     double m = qnan, dm[4] = {qnan, qnan, qnan, qnan};
                     if ((unsigned)b < (unsigned)P.n_bands) {
                         double sc = 1.0;
-                        if (P.zp != nullptr) sc = exp10(0.4 * (double)__ldg(P.zp + o)) * __ldg(P.band_zpab_inv + b);
+                        if (P.zp != nullptr) { // 10^(0.4 zp): recomputed only when zp changes (usually never)
+                            const float zpv = __ldg(P.zp + o);
+                            if (zpv != zp_last) {
+                                zp_last = zpv;
+                                zp_pow = exp10(0.4 * (double)zpv);
+                            }
+                            sc = zp_pow * __ldg(P.band_zpab_inv + b);
+                        }
                         const double raw = (double)res[S.e_begin + i];
                         m = sc * S.x0 * raw;
                         if (GRAD) {
