@@ -26,16 +26,24 @@
  *
  * Conventions
  *   - Loaders take HOST pointers and copy; compute calls take DEVICE pointers owned by the caller
- *     (e.g. torch tensors) and a cudaStream_t passed as void*.  Compute calls only enqueue work:
- *     no allocation visible to the caller, no host synchronisation, no retained pointers.
+ *     (e.g. torch tensors) and a cudaStream_t passed as void*.  Compute calls only enqueue work on
+ *     that stream: no host synchronisation, no retained pointers, no allocation visible to the
+ *     caller.  A call with sb_batch.pack set touches no memory but its arguments.  A call without a
+ *     pack needs a few hundred KB of scratch (redshift order of the batch); it lives in a workspace
+ *     owned by the sb_bands handle, one per stream, allocated (cudaMalloc) by the first call on that
+ *     stream or when a larger batch arrives, never by later calls -- so a warmed-up call can be
+ *     captured into a CUDA graph -- and released by sb_free_bands.
  *   - dtype selects the element type of every floating-point array of a compute call (inputs and
  *     outputs): SB_F32 (production: per-sample arithmetic in fp32) or SB_F64 (verification).
  *   - All functions return SB_OK (0) or a negative sb_status; sb_strerror() names it.  Device data
  *     are not validated (that would need a sync): a band index outside [0, n_bands) gives NaN for
  *     that evaluation; fluxerr <= 0 propagates inf/NaN into chi^2; a phase or wavelength outside
  *     the model grid is not an error and contributes zero flux [G3].
- *   - No global mutable state.  Handles are immutable after creation; concurrent compute calls on
- *     distinct streams with the same handles are allowed.
+ *   - No global mutable state.  Model, band and pack tables are immutable after creation;
+ *     concurrent compute calls from several host threads on distinct streams with the same handles
+ *     are allowed (the per-stream workspaces above are the only thing a call may create, under a
+ *     lock).  Handles belong to the device that was current when they were created: a compute call
+ *     made with another current device returns SB_EINVAL.
  *   - There is no CPU fallback: without a CUDA device every compute call returns SB_ECUDA.
  */
 #ifndef SALTBAND_H
@@ -49,6 +57,7 @@ extern "C" {
 
 typedef struct sb_model sb_model; /* opaque: device-resident M0, M1 tables and the colour law */
 typedef struct sb_bands sb_bands; /* opaque: device-resident band tables, folded weights, ZPAB */
+typedef struct sb_pack sb_pack;   /* opaque: theta-independent precompute of one batch (optional) */
 
 typedef enum { SB_F32 = 0, SB_F64 = 1 } sb_dtype;
 
@@ -61,10 +70,11 @@ typedef enum { SB_F32 = 0, SB_F64 = 1 } sb_dtype;
  *                    the rest-frame geometry and the colour factor; fp32 forward calls with uniform
  *                    band grids only -- a call that demands it where it does not apply returns
  *                    SB_ELIMIT.
- *   SB_FORM_TILED    as SB_FORM_GROUPED, and the observations of a group of units that are neighbours
- *                    in redshift are ordered by phase so that the model rows they read stay in
- *                    registers; fp32 forward AND gradient calls with uniform
- *                    band grids, same error behaviour. */
+ *   SB_FORM_TILED    the node-weight kernel (csrc/sb_nw.cuh): as SB_FORM_GROUPED, and the observations
+ *                    of a group of units that are neighbours in redshift are ordered by phase so
+ *                    that the model rows they read stay in registers; fp32
+ *                    forward AND gradient calls with uniform band grids, same error behaviour.
+ *                    The only formulation that uses sb_batch.pack. */
 enum { SB_FORM_DIRECT = 0x100, SB_FORM_GROUPED = 0x200, SB_FORM_TILED = 0x400 };
 
 typedef enum {
@@ -113,7 +123,25 @@ typedef struct {
     const void *zp;            /* [n_obs_total] zero point, or NULL => S_i = 1 (raw photon flux) */
     const void *z;             /* [n_sn] redshift, > -1 */
     const void *x0, *x1, *c, *t0; /* [n_sn*n_samples], sample fastest */
+    const sb_pack *pack;       /* NULL, or the pack built by sb_pack_observations from this batch's
+                                  n_sn and z (same model and bands); DEVICE calls only */
 } sb_batch;
+
+/* sb_pack_observations -- optional: everything the hot path needs that does not depend on the
+ * free parameters (in a fit or a sampling run the observations and redshifts are
+ * fixed over thousands of calls, only x0, x1, c, t0 change).  Holds the redshift order of the
+ * supernovae (stable sort: neighbours in z share their window of the model surfaces) and, per
+ * (supernova, band), the rest-frame geometry of the band integral (in-range samples decided in
+ * fp64 [G9], model cells spanned, colour-law regime).  Reads batch->n_sn, batch->dtype (SB_F32
+ * only) and the DEVICE array batch->z; the other fields are ignored.  Allocates the pack's device
+ * memory and enqueues its build on `stream` (no host synchronisation: use the pack on the same
+ * stream, or synchronise first).  A compute call whose batch points to the pack must pass the
+ * same n_sn, model and bands (else SB_EINVAL) and the same z values (not checked).  Kernels that
+ * do not use a pack (fp64, SB_FORM_DIRECT, SB_FORM_GROUPED) ignore it.  SB_ELIMIT when the band set is
+ * one the node-weight kernel does not handle (non-uniform band grids, more than 64 bands). */
+int sb_pack_observations(const sb_model *m, const sb_bands *b, const sb_batch *batch, void *stream,
+                         sb_pack **out);
+void sb_free_pack(sb_pack *p); /* NULL is allowed; free after the work that uses it has finished */
 
 /* sb_bandflux -- the band flux m of every evaluation.
  *   out_flux  DEVICE [n_obs_total*n_samples]: supernova s occupies the block starting at
@@ -133,7 +161,9 @@ int sb_chi2(const sb_model *m, const sb_bands *b, const sb_batch *batch, const v
 /* sb_bandflux_grad -- forward plus analytic gradient with respect to (x0, x1, c, t0), in that
  * order (north_star; "fully differentiable").
  *   out_flux   DEVICE, layout as in sb_bandflux, or NULL
- *   out_dflux  DEVICE [n_obs_total*n_samples][4] d m / d(x0, x1, c, t0), same eval order, or NULL
+ *   out_dflux  DEVICE [n_obs_total*n_samples][4] d m / d(x0, x1, c, t0), same eval order, or NULL;
+ *              out_dflux and out_dchi2 must be aligned to 4 elements (16 bytes in fp32): they are
+ *              written as vectors (SB_EINVAL otherwise)
  *   flux, fluxerr  DEVICE [n_obs_total], required iff out_chi2 or out_dchi2 is non-NULL
  *   out_chi2   DEVICE [n_sn*n_samples] or NULL
  *   out_dchi2  DEVICE [n_sn*n_samples][4] = -2 sum_i (flux_i - m_i)/fluxerr_i^2 * dm_i, or NULL
@@ -147,9 +177,10 @@ int sb_bandflux_grad(const sb_model *m, const sb_bands *b, const sb_batch *batch
  * (the end-to-end path of a fit driver that keeps its light curves on the host).  Every pointer of
  * `batch`, flux, fluxerr and every output is a HOST pointer with the layout of the device call;
  * pinned (page-locked) buffers give the full PCIe rate, pageable ones work.  The library cuts the
- * supernovae into chunks, stages each chunk through device buffers of its own (stream-ordered
- * allocations, released before return) and overlaps host->device copies, kernels and device->host
- * copies of consecutive chunks on internal streams.  Results are those of the device call on each
+ * supernovae into chunks, stages each chunk through device buffers owned by the sb_bands handle
+ * (one set per concurrent host call, grown on demand, released by sb_free_bands) and overlaps
+ * host->device copies, kernels and device->host copies of consecutive chunks on internal streams;
+ * batch->pack must be NULL.  Results are those of the device call on each
  * chunk: identical to the whole-batch device call in the direct formulation, and within rounding
  * (the parity tolerance) in the tiled one, whose summation order depends on which supernovae share
  * a group.  The call returns when all outputs are complete (it synchronises its streams);

@@ -13,6 +13,7 @@ from .api import (  # noqa: F401
     SB_FORM_TILED,
     Bands,
     Model,
+    Pack,
     SaltbandError,
     last_form,
     last_launch_count,
@@ -24,5 +25,6 @@ from .api import (  # noqa: F401
     sb_chi2_host,
     sb_load_bandpasses,
     sb_load_model,
+    sb_pack_observations,
     version,
 )

@@ -27,6 +27,7 @@ class _Batch(C.Structure):
         ("dtype", C.c_int32), ("n_sn", C.c_int32), ("n_samples", C.c_int32), ("n_obs_total", C.c_int32),
         ("obs_offset", C.c_void_p), ("time", C.c_void_p), ("band", C.c_void_p), ("zp", C.c_void_p),
         ("z", C.c_void_p), ("x0", C.c_void_p), ("x1", C.c_void_p), ("c", C.c_void_p), ("t0", C.c_void_p),
+        ("pack", C.c_void_p),
     ]
 
 
@@ -62,6 +63,10 @@ def _load():
     L.sb_chi2.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp, vp]
     L.sb_bandflux_grad.restype = C.c_int
     L.sb_bandflux_grad.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp, vp, vp, vp]
+    L.sb_pack_observations.restype = C.c_int
+    L.sb_pack_observations.argtypes = [vp, vp, C.POINTER(_Batch), vp, C.POINTER(vp)]
+    L.sb_free_pack.argtypes = [vp]
+    L.sb_free_pack.restype = None
     L.sb_chi2_host.restype = C.c_int
     L.sb_chi2_host.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp]
     L.sb_bandflux_grad_host.restype = C.c_int
@@ -139,6 +144,19 @@ class Bands:
         return float(_load().sb_bands_zpab(self._h, band))
 
 
+class Pack:
+    """Owner of an `sb_pack*` (theta-independent precompute of one batch: redshift order, item geometry)."""
+
+    def __init__(self, handle: int, keep):
+        self._h = C.c_void_p(handle)
+        self._keep = keep  # the model and bands handles (and z) must outlive the pack
+
+    def __del__(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h and _lib is not None:
+            _lib.sb_free_pack(h)
+
+
 def sb_load_model(phase, wave, m0, m1, cl_coef, cl_wave_b, cl_wave_v, cl_lo, cl_hi) -> Model:
     """include/saltband.h: sb_load_model.  Host fp64 arrays; m0/m1 are [n_phase][n_wave]."""
     L = _load()
@@ -185,18 +203,32 @@ def _ptr(t, dtype, n: Optional[int], name: str, allow_none: bool = False):
 
 
 def _batch(dtype: int, n_sn: int, n_samples: int, obs_offset, time, band, zp, z, x0, x1, c, t0,
-           n_obs_total: int):
+           n_obs_total: int, pack=None):
     import torch
 
     ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
     n_units = n_sn * n_samples
+    if pack is not None and not isinstance(pack, Pack):
+        raise ValueError("pack must be a Pack from sb_pack_observations")
     return _Batch(
         dtype, n_sn, n_samples, n_obs_total,
         _ptr(obs_offset, torch.int32, n_sn + 1, "obs_offset"),
         _ptr(time, ft, n_obs_total, "time"), _ptr(band, torch.int32, n_obs_total, "band"),
         _ptr(zp, ft, n_obs_total, "zp", allow_none=True), _ptr(z, ft, n_sn, "z"),
         _ptr(x0, ft, n_units, "x0"), _ptr(x1, ft, n_units, "x1"), _ptr(c, ft, n_units, "c"),
-        _ptr(t0, ft, n_units, "t0"))
+        _ptr(t0, ft, n_units, "t0"), pack._h if pack is not None else None)
+
+
+def sb_pack_observations(model: Model, bands: Bands, *, dtype: int, n_sn: int, z) -> Pack:
+    """include/saltband.h: sb_pack_observations.  z: [n_sn] CUDA fp32 tensor; built on the current stream."""
+    import torch
+
+    bt = _Batch(dtype, n_sn, 1, 0, None, None, None, None, _ptr(z, torch.float32, n_sn, "z"), None, None, None, None,
+                None)
+    out = C.c_void_p()
+    rc = _load().sb_pack_observations(model._h, bands._h, C.byref(bt), _stream(), C.byref(out))
+    _check(rc, "sb_pack_observations")
+    return Pack(out.value, (model, bands, z))
 
 
 def _stream() -> int:
@@ -206,24 +238,25 @@ def _stream() -> int:
 
 
 def sb_bandflux(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,
-                obs_offset, time, band, zp, z, x0, x1, c, t0, out_flux) -> None:
+                obs_offset, time, band, zp, z, x0, x1, c, t0, out_flux, pack=None) -> None:
     """include/saltband.h: sb_bandflux.  out_flux: [n_obs_total*n_samples] CUDA tensor (written)."""
     import torch
 
     ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
-    bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total)
+    bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total, pack)
     rc = _load().sb_bandflux(model._h, bands._h, C.byref(bt), _ptr(out_flux, ft, n_obs_total * n_samples, "out_flux"),
                              _stream())
     _check(rc, "sb_bandflux")
 
 
 def sb_chi2(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,
-            obs_offset, time, band, zp, z, x0, x1, c, t0, flux, fluxerr, out_chi2, out_flux=None) -> None:
+            obs_offset, time, band, zp, z, x0, x1, c, t0, flux, fluxerr, out_chi2, out_flux=None,
+            pack=None) -> None:
     """include/saltband.h: sb_chi2.  out_chi2: [n_sn*n_samples]; out_flux optional."""
     import torch
 
     ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
-    bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total)
+    bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total, pack)
     rc = _load().sb_chi2(model._h, bands._h, C.byref(bt), _ptr(flux, ft, n_obs_total, "flux"),
                          _ptr(fluxerr, ft, n_obs_total, "fluxerr"),
                          _ptr(out_chi2, ft, n_sn * n_samples, "out_chi2"),
@@ -233,12 +266,12 @@ def sb_chi2(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int
 
 def sb_bandflux_grad(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,
                      obs_offset, time, band, zp, z, x0, x1, c, t0, flux=None, fluxerr=None, out_flux=None,
-                     out_dflux=None, out_chi2=None, out_dchi2=None) -> None:
+                     out_dflux=None, out_chi2=None, out_dchi2=None, pack=None) -> None:
     """include/saltband.h: sb_bandflux_grad.  Gradient order: (x0, x1, c, t0)."""
     import torch
 
     ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
-    bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total)
+    bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total, pack)
     n_ev, n_units = n_obs_total * n_samples, n_sn * n_samples
     rc = _load().sb_bandflux_grad(
         model._h, bands._h, C.byref(bt), _ptr(flux, ft, n_obs_total, "flux", allow_none=True),
@@ -277,7 +310,7 @@ def _host_batch(dtype, n_sn, n_samples, n_obs_total, obs_offset, time, band, zp,
         dtype, n_sn, n_samples, n_obs_total, _hptr(obs_offset, torch.int32, n_sn + 1, "obs_offset"),
         _hptr(time, ft, n_obs_total, "time"), _hptr(band, torch.int32, n_obs_total, "band"),
         _hptr(zp, ft, n_obs_total, "zp", allow_none=True), _hptr(z, ft, n_sn, "z"), _hptr(x0, ft, n_units, "x0"),
-        _hptr(x1, ft, n_units, "x1"), _hptr(c, ft, n_units, "c"), _hptr(t0, ft, n_units, "t0"))
+        _hptr(x1, ft, n_units, "x1"), _hptr(c, ft, n_units, "c"), _hptr(t0, ft, n_units, "t0"), None)
 
 
 def sb_chi2_host(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,

@@ -4,14 +4,42 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <type_traits>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "sb_internal.h"
 #include "sb_kernels.cuh"
 #include "sb_hoist.cuh"
-#include "sb_tiled.cuh"
+#include "sb_nw.cuh"
+
+// Per-stream workspaces and host-call contexts of a bands handle.  This is the only mutable state
+// behind the handles: a cache, guarded by `mu`.  A compute call without a pack needs a few hundred KB
+// of scratch (z-order permutation, sort counters); it is taken from the slot of the call's stream,
+// which the handle allocates on the first call on that stream (or when a larger batch arrives) and
+// keeps until sb_free_bands.  Calls on distinct streams never share a slot; calls on the same stream
+// are ordered by the stream.  Replaced buffers are retired, not freed: earlier work may still use them.
+struct SbScratch {
+    struct Slot { cudaStream_t stream; unsigned char *buf; size_t bytes; };
+    struct HostCtx { // one per concurrent host-buffer call: three streams and their staging slabs
+        cudaStream_t st[3];
+        unsigned char *slab[3];
+        size_t slab_bytes;
+        bool busy;
+    };
+    std::mutex mu;
+    std::vector<Slot> slots;
+    std::vector<void *> retired;
+    std::vector<HostCtx *> host;
+};
+
+struct NvtxRange { // NVTX range around every sb_* call
+    explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 namespace {
 
@@ -64,41 +92,59 @@ double poly_der(const double *a, int n, double x)
     return s;
 }
 
-int device_smem_optin()
+bool device_limits(int *n_sm, int *smem_optin)
 {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
-    if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) return 0;
-    return v;
-}
-// Stream-ordered allocations (workspaces, staging buffers) come from the device's default memory pool;
-// keep freed blocks in the pool across synchronisation points instead of returning them to the driver.
-void keep_pool_memory()
-{
-    static thread_local int done_for_device = -1;
     int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev == done_for_device) return;
-    cudaMemPool_t pool;
-    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-        unsigned long long thr = ~0ULL;
-        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-    }
-    done_for_device = dev;
+    if (!cuda_ok(cudaGetDevice(&dev))) return false;
+    if (!cuda_ok(cudaDeviceGetAttribute(n_sm, cudaDevAttrMultiProcessorCount, dev))) return false;
+    if (!cuda_ok(cudaDeviceGetAttribute(smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev))) return false;
+    return true;
 }
 
-int device_sm_count()
+// Opt-in dynamic shared memory of a kernel: set once per (kernel, device) to the device maximum.
+bool allow_max_smem(const void *kern, int device, int smem_optin)
 {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
-    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    return v;
+    static std::mutex mu;
+    static std::vector<std::pair<const void *, int>> done;
+    std::lock_guard<std::mutex> lock(mu);
+    for (const auto &d : done)
+        if (d.first == kern && d.second == device) return true;
+    cudaFuncAttributes fa;
+    if (!cuda_ok(cudaFuncGetAttributes(&fa, kern))) return false;
+    const int dyn = smem_optin - (int)fa.sharedSizeBytes; // static + dynamic <= the opt-in limit
+    if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn))) return false;
+    done.emplace_back(kern, device);
+    return true;
+}
+
+// Workspace of at least `bytes` for calls on `stream` (see SbScratch).  Allocates only when the stream
+// has no slot yet or its slot is too small.
+unsigned char *scratch_for(const sb_bands *b, cudaStream_t stream, size_t bytes)
+{
+    SbScratch *sc = b->scratch;
+    std::lock_guard<std::mutex> lock(sc->mu);
+    for (auto &s : sc->slots)
+        if (s.stream == stream) {
+            if (s.bytes >= bytes) return s.buf;
+            unsigned char *nb = nullptr;
+            const size_t want = bytes + bytes / 2;
+            if (!cuda_ok(cudaMalloc((void **)&nb, want))) return nullptr;
+            sc->retired.push_back(s.buf);
+            s.buf = nb;
+            s.bytes = want;
+            return nb;
+        }
+    unsigned char *nb = nullptr;
+    if (!cuda_ok(cudaMalloc((void **)&nb, bytes))) return nullptr;
+    sc->slots.push_back({stream, nb, bytes});
+    return nb;
 }
 
 } // namespace
 
 extern "C" {
 
-const char *sb_version(void) { return "saltband 0.1 (sm_100a)"; }
+const char *sb_version(void) { return "saltband 0.2 (sm_100a)"; }
 
 const char *sb_strerror(int status)
 {
@@ -120,6 +166,7 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
                   const double *m1, const double *cl_coef, int32_t n_cl, double cl_wave_b, double cl_wave_v,
                   double cl_lo, double cl_hi, sb_model **out)
 {
+    NvtxRange nvtx("sb_load_model");
     if (out) *out = nullptr;
     if (!phase || !wave || !m0 || !m1 || !cl_coef || !out) return SB_EINVAL;
     if (n_phase < 2 || n_wave < 2 || n_cl < 1 || n_cl > SB_MAX_CL) return SB_EINVAL;
@@ -166,6 +213,7 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
         }
     std::vector<float> f0(t0.begin(), t0.end()), f1(t1.begin(), t1.end());
     cudaGetDevice(&h->device);
+    if (!device_limits(&h->n_sm, &h->smem_optin)) { delete h; return SB_ECUDA; }
     if (!upload(&h->m0_f64, t0) || !upload(&h->m1_f64, t1) || !upload(&h->m0_f32, f0) || !upload(&h->m1_f32, f1)) {
         sb_free_model(h);
         return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
@@ -199,6 +247,7 @@ void sb_free_model(sb_model *m)
 int sb_load_bandpasses(int32_t n_bands, const int64_t *offset, const double *wave, const double *trans,
                        sb_bands **out)
 {
+    NvtxRange nvtx("sb_load_bandpasses");
     if (out) *out = nullptr;
     if (!offset || !wave || !trans || !out || n_bands < 1) return SB_EINVAL;
     if (offset[0] != 0) return SB_EINVAL;
@@ -218,7 +267,8 @@ int sb_load_bandpasses(int32_t n_bands, const int64_t *offset, const double *wav
     h->n_bands = n_bands;
     h->n_total = (int32_t)total;
     h->h_zpab = (double *)malloc(sizeof(double) * (size_t)n_bands);
-    if (!h->h_zpab) { delete h; return SB_ENOMEM; }
+    h->scratch = new (std::nothrow) SbScratch();
+    if (!h->h_zpab || !h->scratch) { free(h->h_zpab); delete h->scratch; delete h; return SB_ENOMEM; }
 
     const double hc = SB_H_PLANCK * SB_C_ANGSTROM;
     std::vector<int32_t> off(n_bands + 1);
@@ -283,6 +333,18 @@ void sb_free_bands(sb_bands *b)
     cudaFree(b->d_dlam_f64);
     cudaFree(b->d_h);
     free(b->h_zpab);
+    if (b->scratch) {
+        for (auto &sl : b->scratch->slots) cudaFree(sl.buf);
+        for (void *p : b->scratch->retired) cudaFree(p);
+        for (auto *c : b->scratch->host) {
+            for (int i = 0; i < 3; ++i) {
+                if (c->slab[i]) cudaFree(c->slab[i]);
+                if (c->st[i]) cudaStreamDestroy(c->st[i]);
+            }
+            delete c;
+        }
+        delete b->scratch;
+    }
     delete b;
 }
 
@@ -301,10 +363,10 @@ double sb_bands_zpab(const sb_bands *b, int32_t band)
 namespace {
 
 template <typename T, bool GRAD, int NCL, bool STAGE, int NWARPS>
-int launch_inst(const SbKParams &kp, size_t smem, int grid, cudaStream_t st)
+int launch_inst(const sb_model *m, const SbKParams &kp, size_t smem, int grid, cudaStream_t st)
 {
     auto kern = sb::sb_fused_kernel<T, GRAD, NCL, STAGE, NWARPS>;
-    if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) return SB_ECUDA;
+    if (!allow_max_smem((const void *)kern, m->device, m->smem_optin)) return SB_ECUDA;
     kern<<<grid, NWARPS * 32, smem, st>>>(kp);
     if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
     tl_launches += 1;
@@ -313,11 +375,9 @@ int launch_inst(const SbKParams &kp, size_t smem, int grid, cudaStream_t st)
 }
 
 template <typename T, bool GRAD, int NWARPS>
-int launch_typed(SbKParams &kp, const sb_bands *b, int n_obs_total, cudaStream_t st)
+int launch_typed(const sb_model *m, SbKParams &kp, const sb_bands *b, int n_obs_total, cudaStream_t st)
 {
-    const int smem_max = device_smem_optin();
-    const int n_sm = device_sm_count();
-    if (smem_max <= 0 || n_sm <= 0) return SB_ECUDA;
+    const int smem_max = m->smem_optin, n_sm = m->n_sm;
     constexpr int NSET = GRAD ? 3 : 1;
     const size_t cell_bytes = sizeof(T) * 4 * NSET;
     // evaluation records per chunk and units per group: about `cap` evaluations per CTA pass
@@ -351,61 +411,71 @@ int launch_typed(SbKParams &kp, const sb_bands *b, int n_obs_total, cudaStream_t
     if (grid < 1) return SB_OK;
     const bool small_cl = kp.mp.n_cl <= 5;
     if (stage) {
-        if (small_cl) return launch_inst<T, GRAD, 5, sizeof(T) == 4, NWARPS>(kp, smem, grid, st);
-        return launch_inst<T, GRAD, SB_MAX_CL, sizeof(T) == 4, NWARPS>(kp, smem, grid, st);
+        if (small_cl) return launch_inst<T, GRAD, 5, sizeof(T) == 4, NWARPS>(m, kp, smem, grid, st);
+        return launch_inst<T, GRAD, SB_MAX_CL, sizeof(T) == 4, NWARPS>(m, kp, smem, grid, st);
     }
-    if (small_cl) return launch_inst<T, GRAD, 5, false, NWARPS>(kp, smem, grid, st);
-    return launch_inst<T, GRAD, SB_MAX_CL, false, NWARPS>(kp, smem, grid, st);
+    if (small_cl) return launch_inst<T, GRAD, 5, false, NWARPS>(m, kp, smem, grid, st);
+    return launch_inst<T, GRAD, SB_MAX_CL, false, NWARPS>(m, kp, smem, grid, st);
 }
 
-// Band-grouped kernels: fp32 forward, uniform band grids.  tiled = true: sb_tiled.cuh (register-tiled
-// node contraction), false: sb_hoist.cuh.  Returns 1 when the kernel is not applicable (the caller
-// then tries the next formulation), SB_OK or an error otherwise.
-int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux,
-                   const void *fluxerr, void *out_flux, void *out_chi2, void *out_dflux, void *out_dchi2,
-                   cudaStream_t st)
+// Workspace layout of the z-order sort: [0] group counter (grouped kernel), [256] bin totals, [4096]
+// permutation, then the per-segment bin counts.
+struct ZWork {
+    size_t perm_off, hist_off, bytes;
+    explicit ZWork(int n_sn)
+    {
+        perm_off = 4096;
+        hist_off = perm_off + ((sizeof(int32_t) * (size_t)n_sn + 255) & ~(size_t)255);
+        bytes = hist_off + sizeof(uint32_t) * (size_t)sbh::kZSegs * sbh::kZBins;
+    }
+};
+static_assert(256 + sizeof(uint32_t) * sbh::kZBins <= 4096, "bin totals overlap the permutation");
+
+// Stable z-order permutation of the supernovae into ws (one or two small kernels + a 4 KB memset).
+int enqueue_zorder(const float *z, int n_sn, unsigned char *ws, cudaStream_t st, int32_t *launches)
 {
-    if (grad && !tiled) return 1;
+    const ZWork zw(n_sn);
+    unsigned int *counter = reinterpret_cast<unsigned int *>(ws);
+    int32_t *perm = reinterpret_cast<int32_t *>(ws + zw.perm_off);
+    if (n_sn <= sbh::kZSmall) {
+        sbh::sb_zorder_small_kernel<<<1, 512, 0, st>>>(z, n_sn, perm, counter);
+        if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
+        *launches += 1;
+        return SB_OK;
+    }
+    uint32_t *z_tot = reinterpret_cast<uint32_t *>(ws + 256), *z_hist = reinterpret_cast<uint32_t *>(ws + zw.hist_off);
+    if (!cuda_ok(cudaMemsetAsync(ws, 0, zw.perm_off, st))) return SB_ECUDA;
+    sbh::sb_zhist_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(z, n_sn, z_hist, z_tot, counter);
+    sbh::sb_zscatter_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(z, n_sn, z_hist, z_tot, perm);
+    if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
+    *launches += 2;
+    return SB_OK;
+}
+
+// Band-grouped kernel (sb_hoist.cuh): fp32 forward, uniform band grids.  Returns 1 when it does not
+// apply (the caller then tries the next formulation), SB_OK or an error otherwise.
+int launch_hoist(const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux, const void *fluxerr,
+                 void *out_flux, void *out_chi2, cudaStream_t st)
+{
     constexpr int NCL = 5;
-    if (!b->all_uniform || m->prm.n_cl > NCL || b->n_bands > 64) return 1;
-    if (tiled && (m->prm.n_phase < 4 || m->prm.n_phase > 4096)) return 1;
-    if (!tiled && !m->m01_f32) return 1;
-    const int smem_max = device_smem_optin();
-    const int n_sm = device_sm_count();
-    if (smem_max <= 0 || n_sm <= 0) return SB_ECUDA;
+    if (!b->all_uniform || m->prm.n_cl > NCL || b->n_bands > 64 || !m->m01_f32) return 1;
+    const int smem_max = m->smem_optin, n_sm = m->n_sm;
     const long long n_units = (long long)bt->n_sn * bt->n_samples;
     const double mean_obs = bt->n_sn > 0 ? (double)bt->n_obs_total / (double)bt->n_sn : 1.0;
-    // units per group: enough groups for every SM (>= 4 per CTA), at most kMaxSeg, about <= cap observations
-    const int gmax = tiled ? (grad ? sbt::kSlots / 2 : sbt::kSlots) : sbh::kMaxSeg;
-    int cap = tiled ? (grad ? 1536 : 3072) : 4096;
-    size_t smem = 0;
-    if (tiled) {
-        while (cap >= 512 && sbt::TSmem(b->n_total, cap, grad, b->n_bands * gmax).total > (size_t)smem_max) cap -= 256;
-        if (cap < 512) return 1;
-    } else {
-        smem = sbh::HSmem(b->n_total, cap).total;
-        if (smem > (size_t)smem_max || smem > 100 * 1024) return 1;
-    }
-    // units per group g: the busiest CTA gets ceil(n_groups / n_sm) groups and a group costs about
-    // g + 4 unit-times (per-group work that does not shrink with g: sort, barriers, short chunks --
-    // measured on configs 2, 4, 5), so minimise that product; at most gmax units and cap observations
+    const int gmax = sbh::kMaxSeg, cap = 4096;
+    const size_t smem = sbh::HSmem(b->n_total, cap).total;
+    if (smem > (size_t)smem_max || smem > 100 * 1024) return 1;
     long long g = 1;
     double best = 0.0;
-    for (long long c = 1; c <= gmax; ++c) {
+    for (long long c = 1; c <= gmax; ++c) { // busiest CTA: ceil(n_groups / n_sm) groups of about g + 4 unit-times
         if (c > 1 && (double)c * mean_obs > (double)cap) break;
         const long long ng = (n_units + c - 1) / c;
         const double load = (double)((ng + n_sm - 1) / n_sm) * (double)(c + 4);
         if (c == 1 || load <= best) { best = load; g = c; }
     }
-    if (tiled) smem = sbt::TSmem(b->n_total, cap, grad, b->n_bands * (int)g).total;
-
-    // workspace (stream-ordered): [0] group counter, [256] bin totals, [4096] z-order permutation, then
-    // the per-segment bin counts of the sort
-    keep_pool_memory();
-    unsigned char *ws = nullptr;
-    const size_t perm_off = 4096, hist_off = perm_off + ((sizeof(int32_t) * (size_t)bt->n_sn + 255) & ~(size_t)255);
-    const size_t ws_bytes = hist_off + sizeof(uint32_t) * (size_t)sbh::kZSegs * sbh::kZBins;
-    if (!cuda_ok(cudaMallocAsync((void **)&ws, ws_bytes, st))) return SB_ECUDA;
+    const ZWork zw(bt->n_sn);
+    unsigned char *ws = scratch_for(b, st, zw.bytes);
+    if (!ws) return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
     SbHParams hp;
     memset(&hp, 0, sizeof(hp));
     hp.mp = m->prm;
@@ -435,52 +505,116 @@ int launch_grouped(bool tiled, bool grad, const sb_model *m, const sb_bands *b, 
     hp.fluxerr = (const float *)fluxerr;
     hp.out_flux = (float *)out_flux;
     hp.out_chi2 = (float *)out_chi2;
-    hp.out_dflux = (float *)out_dflux;
-    hp.out_dchi2 = (float *)out_dchi2;
     hp.counter = reinterpret_cast<unsigned int *>(ws);
-    hp.perm = reinterpret_cast<const int32_t *>(ws + perm_off);
+    hp.perm = reinterpret_cast<const int32_t *>(ws + zw.perm_off);
     hp.group_units = (int)g;
     hp.cap = cap;
-    int rc = SB_OK;
-    static_assert(256 + sizeof(uint32_t) * sbh::kZBins <= 4096, "bin totals overlap the permutation");
-    uint32_t *z_tot = reinterpret_cast<uint32_t *>(ws + 256), *z_hist = reinterpret_cast<uint32_t *>(ws + hist_off);
-    if (hp.n_sn <= sbh::kZSmall) { // one launch; the main kernel's launch is counted below
-        sbh::sb_zorder_small_kernel<<<1, 512, 0, st>>>(hp.z, hp.n_sn, reinterpret_cast<int32_t *>(ws + perm_off), hp.counter);
-        if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
-    } else {
-        if (!cuda_ok(cudaMemsetAsync(ws, 0, perm_off, st))) rc = SB_ECUDA;
-        if (rc == SB_OK) {
-            sbh::sb_zhist_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(hp.z, hp.n_sn, z_hist, z_tot, hp.counter);
-            sbh::sb_zscatter_kernel<<<sbh::kZCtas, sbh::kZWarps * 32, 0, st>>>(hp.z, hp.n_sn, z_hist, z_tot,
-                                                                              reinterpret_cast<int32_t *>(ws + perm_off));
-            if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
-            else tl_launches += 1; // the second of the two; the first is counted below
-        }
+    int rc = enqueue_zorder(hp.z, hp.n_sn, ws, st, &tl_launches);
+    if (rc != SB_OK) return rc;
+    const long long n_groups = (n_units + g - 1) / g;
+    const int grid = (int)(n_groups < (long long)n_sm ? n_groups : (long long)n_sm);
+    auto kern = sbh::sb_hoist_kernel<NCL, SBH_LDN>;
+    if (!allow_max_smem((const void *)kern, m->device, m->smem_optin)) return SB_ECUDA;
+    kern<<<grid, sbh::kThreads, smem, st>>>(hp);
+    if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
+    tl_launches += 1;
+    tl_form = SB_FORM_GROUPED;
+    return SB_OK;
+}
+
+template <int NCL, bool GRAD>
+int launch_nw_inst(const sb_model *m, const sbn::SbNParams &np, size_t smem, int grid, cudaStream_t st)
+{
+    auto kern = sbn::sb_nw_kernel<NCL, GRAD>;
+    if (!allow_max_smem((const void *)kern, m->device, m->smem_optin)) return SB_ECUDA;
+    kern<<<grid, sbn::kThreads, smem, st>>>(np);
+    if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
+    tl_launches += 1;
+    tl_form = SB_FORM_TILED;
+    return SB_OK;
+}
+
+// Node-weight kernel (sb_nw.cuh): fp32 forward and gradient, uniform band grids.  With a pack nothing is
+// computed here but the launch geometry; without one the z-order permutation is built in the call's
+// stream workspace first and the item geometry is computed inside the kernel.  Returns 1 when the
+// kernel does not apply.
+int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux,
+              const void *fluxerr, void *out_flux, void *out_chi2, void *out_dflux, void *out_dchi2, cudaStream_t st)
+{
+    if (!b->all_uniform || m->prm.n_cl > SB_MAX_CL || b->n_bands > sbn::kMaxBands) return 1;
+    if (m->prm.n_phase < 4 || m->prm.n_phase > 4096) return 1;
+    const int smem_max = m->smem_optin, n_sm = m->n_sm;
+    const long long n_units = (long long)bt->n_sn * bt->n_samples;
+    const double mean_obs = bt->n_sn > 0 ? (double)bt->n_obs_total / (double)bt->n_sn : 1.0;
+    const int nsl = grad ? sbn::kSlots / 2 : sbn::kSlots;
+    int cap = grad ? sbn::kCapGrad : sbn::kCapFwd;
+    while (cap >= 512 && sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl).total > (size_t)smem_max) cap -= 256;
+    if (cap < 512) return 1;
+    const size_t smem = sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl).total;
+    // groups: whole waves of n_sm groups of at most g_target units (even split of the z-ordered units),
+    // g_target = as many units as fit the item slots and the round's observation capacity
+    long long g_target = (long long)((double)cap / (mean_obs > 1.0 ? mean_obs : 1.0));
+    if (g_target > nsl) g_target = nsl;
+    if (g_target < 1) g_target = 1;
+    long long waves = (n_units + g_target * n_sm - 1) / (g_target * n_sm);
+    long long n_groups = waves * n_sm;
+    if (n_groups > n_units) n_groups = n_units;
+    if (n_groups < 1) return SB_OK;
+
+    const sb_pack *pk = bt->pack;
+    const int32_t *perm = nullptr;
+    const sbn::NItem *geom = nullptr;
+    if (pk) {
+        if (pk->model != m || pk->bands != b || pk->n_sn != bt->n_sn || pk->n_bands != b->n_bands || pk->device != m->device)
+            return SB_EINVAL;
+        perm = pk->d_perm;
+        geom = reinterpret_cast<const sbn::NItem *>(pk->d_geom);
+    } else if (bt->n_sn > 1) {
+        const ZWork zw(bt->n_sn);
+        unsigned char *ws = scratch_for(b, st, zw.bytes);
+        if (!ws) return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+        const int rc = enqueue_zorder((const float *)bt->z, bt->n_sn, ws, st, &tl_launches);
+        if (rc != SB_OK) return rc;
+        perm = reinterpret_cast<const int32_t *>(ws + zw.perm_off);
     }
-    if (rc == SB_OK) {
-        tl_launches += 1;
-        const long long n_groups = (n_units + g - 1) / g;
-        const int grid = (int)(n_groups < (long long)n_sm ? n_groups : (long long)n_sm);
-        if (tiled && grad) {
-            auto kern = sbt::sb_tiled_kernel<NCL, true>;
-            if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) rc = SB_ECUDA;
-            if (rc == SB_OK) kern<<<grid, sbt::kThreads, smem, st>>>(hp);
-        } else if (tiled) {
-            auto kern = sbt::sb_tiled_kernel<NCL, false>;
-            if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) rc = SB_ECUDA;
-            if (rc == SB_OK) kern<<<grid, sbt::kThreads, smem, st>>>(hp);
-        } else {
-            auto kern = sbh::sb_hoist_kernel<NCL, SBH_LDN>;
-            if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem))) rc = SB_ECUDA;
-            if (rc == SB_OK) kern<<<grid, sbh::kThreads, smem, st>>>(hp);
-        }
-        if (rc == SB_OK) {
-            if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
-            else { tl_launches += 1; tl_form = tiled ? SB_FORM_TILED : SB_FORM_GROUPED; }
-        }
-    }
-    if (!cuda_ok(cudaFreeAsync(ws, st)) && rc == SB_OK) rc = SB_ECUDA;
-    return rc;
+    sbn::SbNParams np;
+    memset(&np, 0, sizeof(np));
+    np.mp = m->prm;
+    np.m0 = m->m0_f32;
+    np.m1 = m->m1_f32;
+    np.n_bands = b->n_bands;
+    np.n_band_total = b->n_total;
+    np.band_off = b->d_off;
+    np.band_lam_first = b->d_lam_first;
+    np.band_zpab_inv = b->d_zpab_inv;
+    np.band_h = b->d_h;
+    np.band_dlam = b->d_dlam_f64;
+    np.band_w = b->d_w_f32;
+    np.n_sn = bt->n_sn;
+    np.n_samples = bt->n_samples;
+    np.obs_offset = bt->obs_offset;
+    np.time = (const float *)bt->time;
+    np.zp = (const float *)bt->zp;
+    np.z = (const float *)bt->z;
+    np.x0 = (const float *)bt->x0;
+    np.x1 = (const float *)bt->x1;
+    np.c = (const float *)bt->c;
+    np.t0 = (const float *)bt->t0;
+    np.band = bt->band;
+    np.flux = (const float *)flux;
+    np.fluxerr = (const float *)fluxerr;
+    np.out_flux = (float *)out_flux;
+    np.out_chi2 = (float *)out_chi2;
+    np.out_dflux = (float *)out_dflux;
+    np.out_dchi2 = (float *)out_dchi2;
+    np.perm = perm;
+    np.geom = geom;
+    np.n_groups = (int32_t)n_groups;
+    np.cap = cap;
+    const int grid = (int)(n_groups < (long long)n_sm ? n_groups : (long long)n_sm);
+    const bool small_cl = m->prm.n_cl <= 5;
+    if (grad) return small_cl ? launch_nw_inst<5, true>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, true>(m, np, smem, grid, st);
+    return small_cl ? launch_nw_inst<5, false>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, false>(m, np, smem, grid, st);
 }
 
 int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void *flux, const void *fluxerr,
@@ -503,6 +637,11 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void 
     if (bt->n_obs_total > 0 && (!bt->time || !bt->band)) return SB_EINVAL;
     if (!out_flux && !out_dflux && !out_chi2 && !out_dchi2) return SB_EINVAL;
     if ((long long)bt->n_sn * bt->n_samples >= (1LL << 31)) return SB_ELIMIT;
+    // the [.][4] gradient outputs are written as 16-byte vectors
+    if (((uintptr_t)out_dflux | (uintptr_t)out_dchi2) & (bt->dtype == SB_F32 ? 15u : 31u)) return SB_EINVAL;
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return SB_ECUDA;
+    if (dev != m->device || dev != b->device) return SB_EINVAL; // handles live on the device they were loaded on
 
     SbKParams kp;
     memset(&kp, 0, sizeof(kp));
@@ -538,29 +677,82 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void 
     const bool tiny = form == 0 && (long long)bt->n_obs_total * bt->n_samples < 4096;
     if (f32 && form != SB_FORM_DIRECT && !tiny && bt->n_obs_total > 0) {
         if (form != SB_FORM_GROUPED) {
-            const int rc = launch_grouped(true, grad, m, b, bt, flux, fluxerr, out_flux, out_chi2, out_dflux, out_dchi2, st);
+            const int rc = launch_nw(grad, m, b, bt, flux, fluxerr, out_flux, out_chi2, out_dflux, out_dchi2, st);
             if (rc != 1) return rc;
         }
         if (form != SB_FORM_TILED && !grad) {
-            const int rc = launch_grouped(false, false, m, b, bt, flux, fluxerr, out_flux, out_chi2, nullptr, nullptr, st);
+            const int rc = launch_hoist(m, b, bt, flux, fluxerr, out_flux, out_chi2, st);
             if (rc != 1) return rc;
         }
     }
     if (form == SB_FORM_GROUPED || form == SB_FORM_TILED) return SB_ELIMIT; // demanded but does not apply
     if (f32) {
-        if (grad) return launch_typed<float, true, 8>(kp, b, bt->n_obs_total, st);
-        return launch_typed<float, false, 16>(kp, b, bt->n_obs_total, st);
+        if (grad) return launch_typed<float, true, 8>(m, kp, b, bt->n_obs_total, st);
+        return launch_typed<float, false, 16>(m, kp, b, bt->n_obs_total, st);
     }
-    if (grad) return launch_typed<double, true, 8>(kp, b, bt->n_obs_total, st);
-    return launch_typed<double, false, 8>(kp, b, bt->n_obs_total, st);
+    if (grad) return launch_typed<double, true, 8>(m, kp, b, bt->n_obs_total, st);
+    return launch_typed<double, false, 8>(m, kp, b, bt->n_obs_total, st);
 }
 
 } // namespace
 
 extern "C" {
 
+int sb_pack_observations(const sb_model *m, const sb_bands *b, const sb_batch *bt, void *stream, sb_pack **out)
+{
+    NvtxRange nvtx("sb_pack_observations");
+    if (out) *out = nullptr;
+    if (!m || !b || !bt || !out) return SB_EINVAL;
+    if ((bt->dtype & 0xff) != SB_F32 || bt->n_sn < 1 || !bt->z) return SB_EINVAL;
+    if (b->n_bands > sbn::kMaxBands || !b->all_uniform) return SB_ELIMIT; // the kernels that use a pack do not apply
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return SB_ECUDA;
+    if (dev != m->device || dev != b->device) return SB_EINVAL;
+    sb_pack *h = new (std::nothrow) sb_pack();
+    if (!h) return SB_ENOMEM;
+    memset(h, 0, sizeof(*h));
+    h->n_sn = bt->n_sn;
+    h->n_bands = b->n_bands;
+    h->model = m;
+    h->bands = b;
+    h->z = bt->z;
+    h->device = dev;
+    const ZWork zw(bt->n_sn);
+    const size_t geom_bytes = sizeof(sbn::NItem) * (size_t)bt->n_sn * b->n_bands;
+    if (!cuda_ok(cudaMalloc((void **)&h->d_ws, zw.bytes)) || !cuda_ok(cudaMalloc(&h->d_geom, geom_bytes))) {
+        const int rc = tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+        sb_free_pack(h);
+        return rc;
+    }
+    h->d_perm = reinterpret_cast<int32_t *>(h->d_ws + zw.perm_off);
+    cudaStream_t st = (cudaStream_t)stream;
+    int32_t launches = 0;
+    int rc = enqueue_zorder((const float *)bt->z, bt->n_sn, h->d_ws, st, &launches);
+    if (rc == SB_OK) {
+        const long long n_items = (long long)bt->n_sn * b->n_bands;
+        const sbn::NBandsView bv{b->n_bands, b->d_off, b->d_lam_first, b->d_h, b->d_dlam_f64};
+        sbn::sb_geom_kernel<<<(unsigned)((n_items + 255) / 256), 256, 0, st>>>(m->prm, bv, (const float *)bt->z, bt->n_sn,
+                                                                             reinterpret_cast<sbn::NItem *>(h->d_geom));
+        if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;
+        else launches += 1;
+    }
+    if (rc != SB_OK) { sb_free_pack(h); return rc; }
+    tl_launches = launches;
+    *out = h;
+    return SB_OK;
+}
+
+void sb_free_pack(sb_pack *p)
+{
+    if (!p) return;
+    cudaFree(p->d_ws);
+    cudaFree(p->d_geom);
+    delete p;
+}
+
 int sb_bandflux(const sb_model *m, const sb_bands *b, const sb_batch *batch, void *out_flux, void *stream)
 {
+    NvtxRange nvtx("sb_bandflux");
     if (!out_flux && !(batch && batch->n_sn == 0)) { tl_launches = 0; return SB_EINVAL; }
     return run(m, b, batch, nullptr, nullptr, out_flux, nullptr, nullptr, nullptr, stream, false);
 }
@@ -568,6 +760,7 @@ int sb_bandflux(const sb_model *m, const sb_bands *b, const sb_batch *batch, voi
 int sb_chi2(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux, const void *fluxerr,
             void *out_chi2, void *out_flux, void *stream)
 {
+    NvtxRange nvtx("sb_chi2");
     if ((!out_chi2 || !flux || !fluxerr) && !(batch && batch->n_sn == 0)) { tl_launches = 0; return SB_EINVAL; }
     return run(m, b, batch, flux, fluxerr, out_flux, nullptr, out_chi2, nullptr, stream, false);
 }
@@ -576,6 +769,7 @@ int sb_bandflux_grad(const sb_model *m, const sb_bands *b, const sb_batch *batch
                      const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2,
                      void *stream)
 {
+    NvtxRange nvtx("sb_bandflux_grad");
     return run(m, b, batch, flux, fluxerr, out_flux, out_dflux, out_chi2, out_dchi2, stream, true);
 }
 
@@ -612,8 +806,11 @@ int run_host(const sb_model *m, const sb_bands *b, const sb_batch *hb, const voi
     if (hb->obs_offset[0] != 0 || hb->obs_offset[hb->n_sn] != hb->n_obs_total) return SB_EINVAL;
     const size_t es = base_dtype == SB_F32 ? 4 : 8;
     const long long ns = hb->n_samples;
-    const int n_sm = device_sm_count();
-    if (n_sm <= 0) return SB_ECUDA;
+    const int n_sm = m->n_sm;
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return SB_ECUDA;
+    if (dev != m->device || dev != b->device) return SB_EINVAL;
+    if (hb->pack) return SB_EINVAL; // a pack describes the whole device-resident batch, not its chunks
 
     // chunks of supernovae: about 24 MB of inputs + outputs each, at most 32 chunks, and (one sample per
     // supernova) a multiple of n_sm * 32 supernovae so that every chunk fills whole waves of groups
@@ -635,22 +832,35 @@ int run_host(const sb_model *m, const sb_bands *b, const sb_batch *hb, const voi
         if (n > max_obs) max_obs = n;
     }
 
-    keep_pool_memory();
-    // internal streams: created once per host thread and device, then reused
-    static thread_local cudaStream_t tl_streams[kHostStreams] = {};
-    static thread_local int tl_streams_dev = -1;
-    int dev = 0;
-    if (!cuda_ok(cudaGetDevice(&dev))) return SB_ECUDA;
-    if (tl_streams_dev != dev) {
-        for (int i = 0; i < kHostStreams; ++i)
-            if (!cuda_ok(cudaStreamCreateWithFlags(&tl_streams[i], cudaStreamNonBlocking))) return SB_ECUDA;
-        tl_streams_dev = dev;
+    // context of this call: three internal streams and one staging slab per stream, owned by the bands
+    // handle, taken from its pool (one context per concurrent host call) and returned before the call ends
+    SbScratch *sc = b->scratch;
+    SbScratch::HostCtx *ctx = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(sc->mu);
+        for (auto *c : sc->host)
+            if (!c->busy) { ctx = c; break; }
+        if (!ctx) {
+            ctx = new (std::nothrow) SbScratch::HostCtx();
+            if (!ctx) return SB_ENOMEM;
+            memset(ctx, 0, sizeof(*ctx));
+            sc->host.push_back(ctx);
+        }
+        ctx->busy = true;
     }
-    cudaStream_t *st = tl_streams;
-    // one stream-ordered allocation per stream, carved into the chunk's arrays (256-byte aligned)
-    ChunkBufs bufs[kHostStreams];
-    unsigned char *slab[kHostStreams] = {};
+    struct Release {
+        SbScratch *sc; SbScratch::HostCtx *c;
+        ~Release() { std::lock_guard<std::mutex> lock(sc->mu); c->busy = false; }
+    } release{sc, ctx};
     int rc = SB_OK;
+    for (int i = 0; i < kHostStreams && rc == SB_OK; ++i)
+        if (!ctx->st[i] && !cuda_ok(cudaStreamCreateWithFlags(&ctx->st[i], cudaStreamNonBlocking))) rc = SB_ECUDA;
+    if (rc != SB_OK) return rc;
+    cudaStream_t *st = ctx->st;
+    // one slab per stream, carved into the chunk's arrays (256-byte aligned); a free context has no work
+    // in flight (every call synchronises its streams before it returns), so its slabs can be regrown
+    ChunkBufs bufs[kHostStreams];
+    unsigned char **slab = ctx->slab;
     const int n_streams = kHostStreams;
     const size_t mo = (size_t)max_obs, mu = (size_t)(chunk_sn * ns);
     for (int pass = 0; pass < 2 && rc == SB_OK; ++pass) { // pass 0: size, pass 1: carve
@@ -675,10 +885,16 @@ int run_host(const sb_model *m, const sb_bands *b, const sb_batch *hb, const voi
             if (out_dchi2) carve(B.o_dchi2, 4 * es * mu);
             total = off;
         }
-        if (pass == 0) {
+        if (pass == 0 && total > ctx->slab_bytes) {
+            for (int i = 0; i < n_streams; ++i) {
+                if (slab[i]) cudaFree(slab[i]);
+                slab[i] = nullptr;
+            }
+            ctx->slab_bytes = 0;
             for (int i = 0; i < n_streams && rc == SB_OK; ++i)
-                if (!cuda_ok(cudaMallocAsync((void **)&slab[i], total ? total : 256, st[i])))
+                if (!cuda_ok(cudaMalloc((void **)&slab[i], total)))
                     rc = tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+            if (rc == SB_OK) ctx->slab_bytes = total;
         }
     }
     int32_t launches = 0, form = 0;
@@ -731,10 +947,8 @@ int run_host(const sb_model *m, const sb_bands *b, const sb_batch *hb, const voi
         if (out_chi2) d2h(out_chi2, es * (size_t)(s0 * ns), B.o_chi2, es * nun);
         if (out_dchi2) d2h(out_dchi2, 4 * es * (size_t)(s0 * ns), B.o_dchi2, 4 * es * nun);
     }
-    for (int i = 0; i < n_streams; ++i) {
-        if (slab[i]) cudaFreeAsync(slab[i], st[i]);
+    for (int i = 0; i < n_streams; ++i)
         if (!cuda_ok(cudaStreamSynchronize(st[i])) && rc == SB_OK) rc = SB_ECUDA;
-    }
     tl_launches = rc == SB_OK ? launches : 0;
     tl_form = rc == SB_OK ? form : 0;
     return rc;
@@ -747,6 +961,7 @@ extern "C" {
 int sb_chi2_host(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux, const void *fluxerr,
                  void *out_chi2, void *out_flux)
 {
+    NvtxRange nvtx("sb_chi2_host");
     if ((!out_chi2 || !flux || !fluxerr) && !(batch && batch->n_sn == 0)) { tl_launches = 0; return SB_EINVAL; }
     return run_host(m, b, batch, flux, fluxerr, out_flux, nullptr, out_chi2, nullptr, false);
 }

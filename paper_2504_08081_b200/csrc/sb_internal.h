@@ -42,7 +42,10 @@ struct sb_model {
     double *m0_f64, *m1_f64;  // [n_phase][ld]
     float2 *m01_f32;          // [n_phase][SBH_LDN] or NULL when n_wave + 34 > SBH_LDN
     int device;
+    int n_sm, smem_optin;     // of `device`, read once at load
 };
+
+struct SbScratch;             // saltband.cu: per-stream workspaces and host-call contexts of a bands handle
 
 struct sb_bands {
     int32_t n_bands, n_total, max_n;
@@ -58,6 +61,19 @@ struct sb_bands {
     float *d_w_f32;        // [n_total] folded weights
     double *d_dlam_f64;    // [n_total] lam_j - lam_first
     double *d_h;           // [n_bands] uniform step h_b
+    int device;
+    SbScratch *scratch;    // owned; the only mutable part of the handle (a cache, guarded by its mutex)
+};
+
+// Pack (sb_pack_observations): everything the node-weight kernel needs that does not depend on theta.
+struct sb_pack {
+    int32_t n_sn, n_bands;
+    int32_t *d_perm;        // [n_sn] supernova indices in redshift order (stable counting sort)
+    void *d_geom;           // [n_sn][n_bands] sbn::NItem
+    unsigned char *d_ws;    // build workspace of the z-order sort (kept: the build is stream ordered)
+    const sb_model *model;  // identity of the handles the pack was built from
+    const sb_bands *bands;
+    const void *z;          // the batch's redshift array the pack was built from (identity check only)
     int device;
 };
 
