@@ -178,7 +178,7 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
     const size_t n = (size_t)n_phase * (size_t)n_wave;
     for (size_t i = 0; i < n; ++i)
         if (!std::isfinite(m0[i]) || !std::isfinite(m1[i])) return SB_EINVAL;
-    if ((long long)n_phase * ((long long)n_wave + 20) >= (1LL << 30)) return SB_ELIMIT;
+    if ((long long)n_phase * ((long long)n_wave + SB_PAD_L + SB_PAD_R + 4) >= (1LL << 30)) return SB_ELIMIT;
 
     sb_model *h = new (std::nothrow) sb_model();
     if (!h) return SB_ENOMEM;
@@ -186,7 +186,7 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
     SbModelParams &p = h->prm;
     p.n_phase = n_phase;
     p.n_wave = n_wave;
-    p.ld = (n_wave + 16 + 3) & ~3; // SB_PAD_L zero columns left, >= 8 right (sb_internal.h)
+    p.ld = (n_wave + SB_PAD_L + SB_PAD_R + 3) & ~3; // zero columns left and right of the nodes (sb_internal.h)
     p.n_cl = n_cl;
     p.p0 = phase[0];
     p.dp = (phase[n_phase - 1] - phase[0]) / (double)(n_phase - 1);
@@ -611,6 +611,7 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     np.geom = geom;
     np.n_groups = (int32_t)n_groups;
     np.cap = cap;
+    { const char *e = getenv("SB_NW_MIX"); np.mix = e ? atoi(e) : 2; }
     const int grid = (int)(n_groups < (long long)n_sm ? n_groups : (long long)n_sm);
     const bool small_cl = m->prm.n_cl <= 5;
     if (grad) return small_cl ? launch_nw_inst<5, true>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, true>(m, np, smem, grid, st);

@@ -8,9 +8,11 @@
 
 #define SB_MAX_CL 8
 // Device model tables: node l of a phase row lives at column l + SB_PAD_L; the row is zero padded
-// on both sides (>= 8 columns on the right) so that the kernel's aligned 4-node loads of a window
-// that touches the grid edge stay inside the row.  ld = round_up(n_wave + 16, 4).
+// on both sides so that the kernels' aligned loads of a node window that starts on the grid stay inside
+// the row without bounds checks: 8 columns on the left (windows start at node >= -4), a whole 256-node
+// window plus slack on the right.  ld = round_up(n_wave + SB_PAD_L + SB_PAD_R, 4).
 #define SB_PAD_L 8
+#define SB_PAD_R 272
 
 // Physical constants (CGS, Angstrom) -- PAPER.md:41 "h and c are the Planck constant and the speed
 // of light"; AB reference flux density for the zero point (G7).

@@ -86,7 +86,7 @@ struct NUnit {           // per unit of the group (all rounds)
 };
 
 struct NSmem {
-    size_t at, ws, res, info, w, hist, wsum, bstart, segs, units, items, win, x1, misc, carry, total;
+    size_t at, ws, res, info, w, hist, wsum, bstart, segs, units, items, win, x1, slot_tab, misc, carry, total;
     __host__ __device__ NSmem(int n_band_total, int cap, bool grad, int n_items)
     {
         size_t o = 0;
@@ -105,6 +105,7 @@ struct NSmem {
         items = o; o += (size_t)n_items * sizeof(NItem);          // every (band, segment) of a round
         win = o; o += (size_t)2 * kMaxBands * sizeof(int32_t);     // [lo | end][band]: union node window
         x1 = o; o += (size_t)kSlots * sizeof(float2);             // [item slot] {x1, x1}
+        slot_tab = o; o += (size_t)kSlots * sizeof(int32_t);       // [item slot] band-in-stage | segment << 8
         misc = o; o += 64;
         o = (o + 15) & ~(size_t)15;
         carry = o; o += 8 * sizeof(double);                        // chi^2 [, d chi^2] of a unit split over rounds
@@ -131,10 +132,44 @@ struct SbNParams {
     const NItem *geom;                // [n_sn][n_bands] item geometry of the pack, or NULL (computed here)
     int32_t n_groups;                 // groups: unit range of group i = [i n_units / n_groups, (i+1) n_units / n_groups)
     int32_t cap;                      // observations per round
+    int32_t mix;                      // which warps start a super-step with phase A (experiment knob)
 };
 
-__device__ __forceinline__ float4 lds128(const float *p) { return *reinterpret_cast<const float4 *>(p); }
-__device__ __forceinline__ float2 lds64(const float *p) { return *reinterpret_cast<const float2 *>(p); }
+// Shared-memory accesses of the hot loops go through 32-bit shared-state-space addresses (one cvta at
+// kernel start) instead of generic pointers: no 64-bit address arithmetic and no per-access window-base
+// computation (S2UR + ULEA, each a scoreboard stall).  An array is accessed either only through these
+// or only through C++ pointers between two CTA barriers.
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ float4 lds128(uint32_t a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ float2 lds64(uint32_t a)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ float lds32(uint32_t a)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds32u(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v)); }
+
+struct NShared { // shared-state-space addresses of the arrays phase B reads
+    uint32_t info, ws, wd, x1, res;
+    int32_t cap;
+};
 
 // ---- geometry of one item (redshift z, band b): one thread.  The in-range sample range [j_lo, j_hi) is
 // decided in fp64 (reading G9), then the window of model cells and the colour-law mode.
@@ -216,8 +251,8 @@ __device__ __forceinline__ void item_geometry(const SbModelParams &mp, const NBa
 // moments, weighted by CL, gives the node weights of d/dc (at_slot + kSlotW).
 template <int NCL, int CM, bool GRAD>
 __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NSeg &S, const NItem &I, int w_lo,
-                                               int q_start, int q_a, int q_b, int q_lo,
-                                               const float *__restrict__ s_w, float *__restrict__ at_slot, int lane)
+                                               int q_start, int q_a, int q_b, int q_lo, uint32_t a_w,
+                                               uint32_t at_slot, int lane)
 {
     constexpr unsigned FULL = 0xffffffffu;
     const float cs = S.cs; // c log2(e)
@@ -243,8 +278,8 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
     float pc0 = 0.f, pc1 = 0.f, pc2 = 0.f; // GRAD: carries of the d/dc weights
     int gq = w_lo + 32 * q_start + lane + 1 - I.g_first; // this lane's cell (first pass) relative to g_first
     int carry = jstart(gq);                                // lane 0: start of its cell
-    const float *wbase = s_w + I.wbase;
-    float *outp = at_slot + (q_start - q_lo) * 32 + lane;
+    const uint32_t wbase = a_w + (uint32_t)I.wbase * 4u;
+    uint32_t outp = at_slot + (uint32_t)((q_start - q_lo) * 32 + lane) * 4u;
     auto from_left = [&](float cur, float prev, int d) {
         const float a = __shfl_up_sync(FULL, cur, d);
         const float b = __shfl_sync(FULL, prev, (lane - d) & 31);
@@ -284,7 +319,7 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
         const int cntA = jeA - jsA, cntB = jeB - jsB;
         const float fA = (float)jsA, fB = (float)jsB;
         const float2 f2 = make_float2(fA, fB);
-        const float *wpA = wbase + jsA, *wpB = wbase + jsB;
+        uint32_t wpA = wbase + (uint32_t)jsA * 4u, wpB = wbase + (uint32_t)jsB * 4u;
         const int km = __reduce_max_sync(FULL, max(cntA, cntB));
         float2 m0 = make_float2(0.f, 0.f), m1 = m0, m2 = m0, m3 = m0;
         float2 n0 = m0, n1 = m0, n2 = m0, n3 = m0; // GRAD: weighted by CL
@@ -297,8 +332,10 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
 #pragma unroll 1
         for (int k = 0; k < km; ++k) { // one sample of each of the two cells per trip
             float2 w = make_float2(0.f, 0.f);
-            if (k < cntA) w.x = wpA[k];
-            if (k < cntB) w.y = wpB[k];
+            if (k < cntA) w.x = lds32(wpA);
+            if (k < cntB) w.y = lds32(wpB);
+            wpA += 4u;
+            wpB += 4u;
             const float2 cl = col.template arg2<CM>(r2v);
             const float2 ar = GRAD ? __fmul2_rn(cl, cc2) : cl;
             const float2 e = __fmul2_rn(make_float2(sb::exp_scaled(ar.x), sb::exp_scaled(ar.y)), w);
@@ -320,14 +357,14 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
         }
         const bool stA = q >= q_a, stB = q + 1 >= q_a && q + 1 < q_b;
         const float2 at = node_weights(I.g_first + gq, m0, m1, m2, m3, pa0, pa1, pa2);
-        if (stA) outp[0] = at.x;
-        if (stB) outp[32] = at.y;
+        if (stA) sts32(outp, at.x);
+        if (stB) sts32(outp + 128u, at.y);
         if (GRAD) {
             const float2 ac = node_weights(I.g_first + gq, n0, n1, n2, n3, pc0, pc1, pc2);
-            if (stA) outp[kSlotW] = ac.x;
-            if (stB) outp[kSlotW + 32] = ac.y;
+            if (stA) sts32(outp + kSlotW * 4u, ac.x);
+            if (stB) sts32(outp + kSlotW * 4u + 128u, ac.y);
         }
-        outp += 64;
+        outp += 256u;
         gq += 64;
     }
 }
@@ -336,8 +373,7 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
 // slot is zero filled up to a whole 64-node block (phase B reads it in 64-node blocks).
 template <int NCL, bool GRAD>
 __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const NSeg &S, const NItem &I, int w_lo,
-                                             int q_lo, int q_hi, const float *__restrict__ s_w,
-                                             float *__restrict__ at_slot, int lane)
+                                             int q_lo, int q_hi, uint32_t a_w, uint32_t at_slot, int lane)
 {
     int q_a = q_hi, q_b = q_hi, qa = 0;
     if (I.n_in > 0) {
@@ -346,23 +382,24 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const NSeg
         q_a = min(max(qa, q_lo), q_hi);
         q_b = max(min(qb + 1, q_hi), q_a);
     }
-    const int q_fill = q_lo + (((q_hi - q_lo) + 1) & ~1);
+    // zero fill up to what phase B reads: whole 64-node blocks, and (forward) at least 128 nodes
+    const int q_fill = q_lo + ((!GRAD && q_hi - q_lo <= 2) ? 4 : (((q_hi - q_lo) + 1) & ~1));
     for (int q = q_lo; q < q_a; ++q) {
-        at_slot[(q - q_lo) * 32 + lane] = 0.f;
-        if (GRAD) at_slot[kSlotW + (q - q_lo) * 32 + lane] = 0.f;
+        sts32(at_slot + (uint32_t)((q - q_lo) * 32 + lane) * 4u, 0.f);
+        if (GRAD) sts32(at_slot + (uint32_t)(kSlotW + (q - q_lo) * 32 + lane) * 4u, 0.f);
     }
     for (int q = q_b; q < q_fill; ++q) {
-        at_slot[(q - q_lo) * 32 + lane] = 0.f;
-        if (GRAD) at_slot[kSlotW + (q - q_lo) * 32 + lane] = 0.f;
+        sts32(at_slot + (uint32_t)((q - q_lo) * 32 + lane) * 4u, 0.f);
+        if (GRAD) sts32(at_slot + (uint32_t)(kSlotW + (q - q_lo) * 32 + lane) * 4u, 0.f);
     }
     if (q_a >= q_b) return;
     const int q_start = q_a > qa ? q_a - 1 : q_a;
     if (I.cmode == sb::CM_INSIDE)
-        phase_a_passes<NCL, sb::CM_INSIDE, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+        phase_a_passes<NCL, sb::CM_INSIDE, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
     else if (I.cmode == sb::CM_LINEAR)
-        phase_a_passes<NCL, sb::CM_LINEAR, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+        phase_a_passes<NCL, sb::CM_LINEAR, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
     else
-        phase_a_passes<NCL, sb::CM_GENERIC, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, s_w, at_slot, lane);
+        phase_a_passes<NCL, sb::CM_GENERIC, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
 }
 
 // ---- phase B: observations [i_lo, i_hi) of the sorted list (all of one band) on one warp ----------
@@ -373,13 +410,11 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const NSeg
 // Per node pair and row: t = M0 + x1 M1 (FFMA2), D_s += At t (FFMA2); GRAD adds E_s += At M1 (d/dx1) and
 // C_s += Atc t (d/dc).  Every element of a pair sees the scalar sequence of fused multiply-adds.
 template <int N128, bool T64, bool GRAD>
-__device__ __forceinline__ void phase_b_window(const SbNParams &P, int n0, const float *__restrict__ s_at,
-                                               const float2 *__restrict__ s_x1, const float4 *__restrict__ s_ws,
-                                               const float4 *__restrict__ s_wd, const uint32_t *__restrict__ s_info,
-                                               float *__restrict__ res, int cap, int i_lo, int i_hi, int lane)
+__device__ __forceinline__ void phase_b_window(const SbNParams &P, int n0, uint32_t a_at, const NShared &SA, bool first,
+                                               int i_lo, int i_hi, int lane)
 {
     constexpr int NQ = 2 * N128 + (T64 ? 1 : 0); // packed node pairs per lane
-    constexpr int ATS = GRAD ? 2 * kSlotW : kSlotW;
+    constexpr uint32_t ATS = (GRAD ? 2 * kSlotW : kSlotW) * 4u; // bytes per item slot
     constexpr int NV = GRAD ? 4 : 1;
     const int ld = P.mp.ld;
     float2 M0[4][NQ], M1[4][NQ]; // [slot = row mod 4][node pair]
@@ -387,79 +422,68 @@ __device__ __forceinline__ void phase_b_window(const SbNParams &P, int n0, const
     for (int s = 0; s < 4; ++s)
 #pragma unroll
         for (int q = 0; q < NQ; ++q) { M0[s][q] = make_float2(0.f, 0.f); M1[s][q] = make_float2(0.f, 0.f); }
-    const int col4 = n0 + SB_PAD_L + 4 * lane;              // column of the lane's first node of block 0
-    const int colt = n0 + SB_PAD_L + 128 * N128 + 2 * lane; // column of the lane's tail pair
-    bool ok[N128 > 0 ? N128 : 1];
-#pragma unroll
-    for (int h = 0; h < N128; ++h) ok[h] = col4 + 128 * h >= 0 && col4 + 128 * h + 4 <= ld;
-    const bool okt = T64 && colt >= 0 && colt + 2 <= ld;
-    const float *p0 = P.m0, *p1 = P.m1;
+    // the table rows are zero padded on the right by a whole window (saltband.cu: ld), so every load of a
+    // window that starts at a node of the grid stays inside its row: no bounds predicates
+    const float *p0 = P.m0 + (n0 + SB_PAD_L + 4 * lane), *p1 = P.m1 + (n0 + SB_PAD_L + 4 * lane);
+    const int toff = 128 * N128 - 2 * lane; // tail pair: column n0 + PAD + 128 N128 + 2 lane
     int rb_held = -64; // rows rb_held .. rb_held + 3 are in the registers
+    const uint32_t a_lane = a_at + (uint32_t)lane * 16u, a_tail = a_at + 512u * N128 + (uint32_t)lane * 8u;
 
     auto load_slot = [&](auto s_tag, int row) {
         constexpr int s = decltype(s_tag)::value;
         const ptrdiff_t ro = (ptrdiff_t)row * ld;
 #pragma unroll
         for (int h = 0; h < N128; ++h) {
-            float4 a = make_float4(0.f, 0.f, 0.f, 0.f), c = a;
-            if (ok[h]) {
-                a = __ldg(reinterpret_cast<const float4 *>(p0 + ro + col4 + 128 * h));
-                c = __ldg(reinterpret_cast<const float4 *>(p1 + ro + col4 + 128 * h));
-            }
+            const float4 a = __ldg(reinterpret_cast<const float4 *>(p0 + ro + 128 * h));
+            const float4 c = __ldg(reinterpret_cast<const float4 *>(p1 + ro + 128 * h));
             M0[s][2 * h] = make_float2(a.x, a.y); M0[s][2 * h + 1] = make_float2(a.z, a.w);
             M1[s][2 * h] = make_float2(c.x, c.y); M1[s][2 * h + 1] = make_float2(c.z, c.w);
         }
         if constexpr (T64) {
-            float2 a = make_float2(0.f, 0.f), c = a;
-            if (okt) {
-                a = __ldg(reinterpret_cast<const float2 *>(p0 + ro + colt));
-                c = __ldg(reinterpret_cast<const float2 *>(p1 + ro + colt));
-            }
-            M0[s][2 * N128] = a;
-            M1[s][2 * N128] = c;
-        }
-    };
-    auto load_row = [&](int row) { // warp-uniform row -> its register slot
-        switch (row & 3) {
-        case 0: load_slot(std::integral_constant<int, 0>{}, row); break;
-        case 1: load_slot(std::integral_constant<int, 1>{}, row); break;
-        case 2: load_slot(std::integral_constant<int, 2>{}, row); break;
-        default: load_slot(std::integral_constant<int, 3>{}, row); break;
+            M0[s][2 * N128] = __ldg(reinterpret_cast<const float2 *>(p0 + ro + toff));
+            M1[s][2 * N128] = __ldg(reinterpret_cast<const float2 *>(p1 + ro + toff));
         }
     };
     auto rows = [&](int rb) { // make rows rb .. rb+3 resident; the sorted order makes rb grow slowly
-        if (rb == rb_held) return;
         const int d = rb - rb_held;
-        if (d > 0 && d < 4) {
-            for (int r = rb_held + 4; r < rb + 4; ++r) load_row(r);
-        } else {
-            for (int r = rb; r < rb + 4; ++r) load_row(r);
-        }
+        int r = (d > 0 && d < 4) ? rb_held + 4 : rb; // first row that is not in the registers yet
         rb_held = rb;
+#pragma unroll 1
+        for (; r < rb + 4; ++r) { // warp-uniform row -> its register slot
+            switch (r & 3) {
+            case 0: load_slot(std::integral_constant<int, 0>{}, r); break;
+            case 1: load_slot(std::integral_constant<int, 1>{}, r); break;
+            case 2: load_slot(std::integral_constant<int, 2>{}, r); break;
+            default: load_slot(std::integral_constant<int, 3>{}, r); break;
+            }
+        }
     };
 
-    auto one = [&](int i, float *out) { // out[0..NV): value [, d/dx1, d/dc, d/dt0] shares of observation i
-        const uint32_t info = s_info[i];
-        const int slot = (int)(info & 31u);
-        rows((int)((info >> 5) & 4095u));
-        const float4 w4 = s_ws[i];
-        const float2 xx = s_x1[slot];
-        const float *ap = s_at + slot * ATS;
+    struct Vals { float v[NV]; };
+    auto one = [&](int i) { // value [, d/dx1, d/dc, d/dt0] shares of observation i
+        Vals out;
+        const uint32_t info = lds32u(SA.info + (uint32_t)i * 4u);
+        const uint32_t slot = info & 31u;
+        const int rb = (int)((info >> 5) & 4095u);
+        if (rb != rb_held) rows(rb);
+        const float4 w4 = lds128(SA.ws + (uint32_t)i * 16u);
+        const float2 xx = lds64(SA.x1 + slot * 8u);
+        const uint32_t so = slot * ATS;
         float2 at[NQ], ac[GRAD ? NQ : 1];
 #pragma unroll
         for (int h = 0; h < N128; ++h) {
-            const float4 t = lds128(ap + 128 * h + 4 * lane);
+            const float4 t = lds128(a_lane + so + 512u * h);
             at[2 * h] = make_float2(t.x, t.y);
             at[2 * h + 1] = make_float2(t.z, t.w);
             if constexpr (GRAD) {
-                const float4 u = lds128(ap + kSlotW + 128 * h + 4 * lane);
+                const float4 u = lds128(a_lane + so + kSlotW * 4u + 512u * h);
                 ac[2 * h] = make_float2(u.x, u.y);
                 ac[2 * h + 1] = make_float2(u.z, u.w);
             }
         }
         if constexpr (T64) {
-            at[2 * N128] = lds64(ap + 128 * N128 + 2 * lane);
-            if constexpr (GRAD) ac[2 * N128] = lds64(ap + kSlotW + 128 * N128 + 2 * lane);
+            at[2 * N128] = lds64(a_tail + so);
+            if constexpr (GRAD) ac[2 * N128] = lds64(a_tail + so + kSlotW * 4u);
         }
         float2 D[4], E[GRAD ? 4 : 1], C[GRAD ? 4 : 1];
 #pragma unroll
@@ -483,35 +507,46 @@ __device__ __forceinline__ void phase_b_window(const SbNParams &P, int n0, const
             }
         }
         const float d0 = D[0].x + D[0].y, d1 = D[1].x + D[1].y, d2 = D[2].x + D[2].y, d3 = D[3].x + D[3].y;
-        out[0] = __fmaf_rn(w4.w, d3, __fmaf_rn(w4.z, d2, __fmaf_rn(w4.y, d1, w4.x * d0)));
+        out.v[0] = __fmaf_rn(w4.w, d3, __fmaf_rn(w4.z, d2, __fmaf_rn(w4.y, d1, w4.x * d0)));
         if constexpr (GRAD) {
-            const float4 v4 = s_wd[i];
+            const float4 v4 = lds128(SA.wd + (uint32_t)i * 16u);
             const float e0 = E[0].x + E[0].y, e1 = E[1].x + E[1].y, e2 = E[2].x + E[2].y, e3 = E[3].x + E[3].y;
             const float c0 = C[0].x + C[0].y, c1 = C[1].x + C[1].y, c2 = C[2].x + C[2].y, c3 = C[3].x + C[3].y;
-            out[1] = __fmaf_rn(w4.w, e3, __fmaf_rn(w4.z, e2, __fmaf_rn(w4.y, e1, w4.x * e0)));
-            out[2] = __fmaf_rn(w4.w, c3, __fmaf_rn(w4.z, c2, __fmaf_rn(w4.y, c1, w4.x * c0)));
-            out[3] = __fmaf_rn(v4.w, d3, __fmaf_rn(v4.z, d2, __fmaf_rn(v4.y, d1, v4.x * d0)));
+            out.v[1] = __fmaf_rn(w4.w, e3, __fmaf_rn(w4.z, e2, __fmaf_rn(w4.y, e1, w4.x * e0)));
+            out.v[2] = __fmaf_rn(w4.w, c3, __fmaf_rn(w4.z, c2, __fmaf_rn(w4.y, c1, w4.x * c0)));
+            out.v[3] = __fmaf_rn(v4.w, d3, __fmaf_rn(v4.z, d2, __fmaf_rn(v4.y, d1, v4.x * d0)));
         }
+        return out;
     };
 
-    for (int i = i_lo; i < i_hi; i += 4) {
-        float acc[4 * NV];
+    // NOBS observations share one transposed warp reduction (forward: eight, so that the chain of dependent
+    // shuffles is paid once per eight; gradient: four, 16 values): NH passes of a four-times unrolled body
+    constexpr int NH = GRAD ? 1 : 2, NOBS = 4 * NH;
+    for (int i = i_lo; i < i_hi; i += NOBS) {
+        float acc[NOBS * NV];
+#pragma unroll 1
+        for (int half = 0; half < NH; ++half) {
+            float q4[4 * NV];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            if (i + j < i_hi) {
-                one(i + j, acc + NV * j);
-            } else {
+            for (int j = 0; j < 4; ++j) { // past the end of the chunk: the last observation again (not stored)
+                const Vals r = one(min(i + 4 * half + j, i_hi - 1));
 #pragma unroll
-                for (int v = 0; v < NV; ++v) acc[NV * j + v] = 0.f;
+                for (int v = 0; v < NV; ++v) q4[NV * j + v] = r.v[v];
+            }
+#pragma unroll
+            for (int k = 0; k < 4 * NV; ++k) {
+                if (NH == 1 || half == 0) acc[k] = q4[k];
+                else acc[(NH - 1) * 4 * NV + k] = q4[k];
             }
         }
-        if constexpr (GRAD) { // lane L ends with value (L >> 1) = 4 * observation + component
-            const float v = sbh::warp_reduce_transpose<16>(acc, lane);
-            const int vi = lane >> 1, j = vi >> 2, comp = vi & 3;
-            if ((lane & 1) == 0 && i + j < i_hi) res[comp * cap + (int)(s_info[i + j] >> 17)] += v;
-        } else {      // lane L ends with the total of observation i + (L >> 3)
-            const float v = sbh::warp_reduce_transpose<4>(acc, lane);
-            if ((lane & 7) == 0 && i + (lane >> 3) < i_hi) res[s_info[i + (lane >> 3)] >> 17] += v;
+        // lane L ends with value (L >> SH): observation (L >> SH) / NV, component (L >> SH) % NV
+        constexpr int SH = GRAD ? 1 : 2;
+        const float v = sbh::warp_reduce_transpose<NOBS * NV>(acc, lane);
+        const int vi = lane >> SH, j = vi / NV, comp = vi % NV;
+        if ((lane & ((1 << SH) - 1)) == 0 && i + j < i_hi) {
+            const uint32_t e = lds32u(SA.info + (uint32_t)(i + j) * 4u) >> 17;
+            const uint32_t ra = SA.res + (uint32_t)(comp * SA.cap) * 4u + e * 4u;
+            sts32(ra, first ? v : v + lds32(ra));
         }
     }
     __syncwarp();
@@ -576,7 +611,9 @@ __global__ void __launch_bounds__(kThreads, 1) sb_nw_kernel(const __grid_constan
     float2 *s_x1 = reinterpret_cast<float2 *>(smem_raw + L.x1);         // [item slot]
     int *misc = reinterpret_cast<int *>(smem_raw + L.misc);             // [1] n_seg, [2] n_ev, [3] next unit, [4] next offset
     double *carry = reinterpret_cast<double *>(smem_raw + L.carry);
-    const float4 *s_wd = s_ws + CAP;                                    // GRAD: d/dt0 phase weights
+    int *slot_tab = reinterpret_cast<int *>(smem_raw + L.slot_tab);     // [item slot] band-in-stage | segment << 8
+    const uint32_t a_at = smem_addr(s_at), a_w = smem_addr(s_w);
+    const NShared SA{smem_addr(s_info), smem_addr(s_ws), smem_addr(s_ws + CAP), smem_addr(s_x1), smem_addr(res), CAP};
 
     for (int i = tid; i < P.n_band_total; i += kThreads) s_w[i] = __ldg(P.band_w + i);
     const long long n_units = (long long)P.n_sn * P.n_samples;
@@ -796,87 +833,96 @@ __global__ void __launch_bounds__(kThreads, 1) sb_nw_kernel(const __grid_constan
                     atomicMax(&win_all[kMaxBands + b], I.n_end);
                 }
             }
-            if (tid < NSL) { const float x = segs[tid % n_seg].x1; s_x1[tid] = make_float2(x, x); }
+            if (tid < NSL) {
+                const int bl = tid / n_seg, sg = tid - bl * n_seg;
+                const float x = segs[sg].x1;
+                s_x1[tid] = make_float2(x, x);
+                slot_tab[tid] = bl | (sg << 8);
+            }
             __syncthreads(); // sorted records, items and band windows are visible
 
             // ---- stages: bps bands x one 256-node window segment; phase A of stage s+1 and phase B of
             // stage s share a super-step (double-buffered node weights), one CTA barrier per stage
             const int n_bst = (n_bands + bps - 1) / bps;
+            auto win_len = [&](int b) { // nodes of band b's union window (0: none)
+                const int lo = win_all[b], hi = win_all[kMaxBands + b];
+                return hi > lo ? hi - lo : 0;
+            };
             auto n_wseg_of = [&](int st) { // window segments of band stage st (the widest band decides)
                 const int b0 = st * bps, nbs = min(bps, n_bands - b0);
                 int n = 0;
                 for (int bl = 0; bl < nbs; ++bl) {
-                    const int len = win_all[kMaxBands + b0 + bl] - win_all[b0 + bl];
+                    const int len = win_len(b0 + bl);
                     if (len > 0) n = max(n, (len + kSlotW - 1) / kSlotW);
                 }
                 return n;
             };
-            auto phase_a = [&](int st, int wseg, float *at_buf) {
-                const int b0 = st * bps, nbs = min(bps, n_bands - b0), n_items = nbs * n_seg;
-                for (int it = warp; it < n_items; it += kWarps) {
-                    const int bl = it / n_seg, sg = it - bl * n_seg;
-                    const int w_lo = win_all[b0 + bl], len = win_all[kMaxBands + b0 + bl] - w_lo;
-                    if (len <= 0) continue;
-                    const int np_b = (len + 31) >> 5;
-                    const int q_lo = wseg * kPassSeg, q_hi = min(q_lo + kPassSeg, np_b);
-                    if (q_lo >= q_hi) continue;
-                    phase_a_item<NCL, GRAD>(mp, segs[sg], items_all[b0 * n_seg + it], w_lo, q_lo, q_hi, s_w,
-                                            at_buf + (size_t)it * ATS, lane);
-                }
-            };
-            auto phase_b = [&](int st, int wseg, const float *at_buf) {
-                const int b0 = st * bps, nbs = min(bps, n_bands - b0);
-                for (int bl = 0; bl < nbs; ++bl) {
-                    const int w_lo = win_all[b0 + bl], len = win_all[kMaxBands + b0 + bl] - w_lo;
-                    if (len <= 0) continue;
-                    const int width = min(kSlotW, len - wseg * kSlotW);
-                    if (width <= 0) continue;
-                    const int lo = bstart[b0 + bl], n = bstart[b0 + bl + 1] - lo;
-                    const int per = (((n + kWarps - 1) / kWarps) + 3) & ~3;
-                    const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
-                    if (i_lo >= i_hi) continue;
-                    const int n0 = w_lo + wseg * kSlotW;
-                    const int nb64 = (width + 63) >> 6;
-                    // slot numbers in s_info are (b % bps) * n_seg + sg = bl * n_seg + sg
-                    if constexpr (GRAD) {
-                        for (int h0 = 0; h0 < nb64; h0 += 2) {
-                            if (h0 + 1 < nb64)
-                                phase_b_window<1, false, true>(P, n0 + 64 * h0, at_buf + 64 * h0, s_x1, s_ws, s_wd, s_info, res, CAP, i_lo, i_hi, lane);
-                            else
-                                phase_b_window<0, true, true>(P, n0 + 64 * h0, at_buf + 64 * h0, s_x1, s_ws, s_wd, s_info, res, CAP, i_lo, i_hi, lane);
+            // stage cursors (band stage, window segment), identical in every thread: `nxt` is the stage whose
+            // node weights are built (into buffer `buf`), `cur` the one whose observations are contracted
+            int st_n = 0, ws_n = 0, nws_n = 0, st_c = n_bst, ws_c = 0;
+            while (st_n < n_bst && (nws_n = n_wseg_of(st_n)) == 0) ++st_n;
+            int buf = 0;
+            // which warps start a super-step with phase A: 0 all, 1 the warps of two schedulers, 2 two warps of every scheduler
+            const bool a_first = P.mix == 0 ? true : P.mix == 1 ? (warp & 2) == 0 : ((warp >> 2) & 1) == 0;
+            while (st_n < n_bst || st_c < n_bst) {
+#pragma unroll 1
+                for (int ph = 0; ph < 2; ++ph) {
+                    if ((ph == 0) == a_first) {
+                        // ---- phase A of stage (st_n, ws_n): node weights of its items -> buffer buf
+                        if (st_n >= n_bst) continue;
+                        const uint32_t at_buf = a_at + (uint32_t)(buf * BUF) * 4u;
+                        const int b0 = st_n * bps, nbs = min(bps, n_bands - b0), n_items = nbs * n_seg;
+                        for (int it = warp; it < n_items; it += kWarps) {
+                            const int tb = slot_tab[it];
+                            const int bl = tb & 255, sg = tb >> 8;
+                            const int w_lo = win_all[b0 + bl], len = win_len(b0 + bl);
+                            if (len <= 0) continue;
+                            const int np_b = (len + 31) >> 5;
+                            const int q_lo = ws_n * kPassSeg, q_hi = min(q_lo + kPassSeg, np_b);
+                            if (q_lo >= q_hi) continue;
+                            phase_a_item<NCL, GRAD>(mp, segs[sg], items_all[b0 * n_seg + it], w_lo, q_lo, q_hi, a_w,
+                                                    at_buf + (uint32_t)(it * ATS) * 4u, lane);
                         }
                     } else {
-                        if (nb64 == 4) phase_b_window<2, false, false>(P, n0, at_buf, s_x1, s_ws, s_wd, s_info, res, CAP, i_lo, i_hi, lane);
-                        else if (nb64 == 3) phase_b_window<1, true, false>(P, n0, at_buf, s_x1, s_ws, s_wd, s_info, res, CAP, i_lo, i_hi, lane);
-                        else if (nb64 == 2) phase_b_window<1, false, false>(P, n0, at_buf, s_x1, s_ws, s_wd, s_info, res, CAP, i_lo, i_hi, lane);
-                        else phase_b_window<0, true, false>(P, n0, at_buf, s_x1, s_ws, s_wd, s_info, res, CAP, i_lo, i_hi, lane);
+                        // ---- phase B of stage (st_c, ws_c): its observations x buffer buf ^ 1
+                        if (st_c >= n_bst) continue;
+                        const uint32_t at_buf = a_at + (uint32_t)((buf ^ 1) * BUF) * 4u;
+                        const int b0 = st_c * bps, nbs = min(bps, n_bands - b0);
+                        for (int bl = 0; bl < nbs; ++bl) {
+                            const int w_lo = win_all[b0 + bl], len = win_len(b0 + bl);
+                            if (len <= 0) continue;
+                            const int width = min(kSlotW, len - ws_c * kSlotW);
+                            if (width <= 0) continue;
+                            const int lo = bstart[b0 + bl], n = bstart[b0 + bl + 1] - lo;
+                            const int per = (((n + kWarps - 1) / kWarps) + (GRAD ? 3 : 7)) & (GRAD ? ~3 : ~7);
+                            const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
+                            if (i_lo >= i_hi) continue;
+                            const int n0 = w_lo + ws_c * kSlotW;
+                            const int nb64 = (width + 63) >> 6;
+                            const bool first = ws_c == 0; // first sweep of these observations: results are stored, not added
+                            // slot numbers in the records are (b % bps) * n_seg + sg = bl * n_seg + sg
+                            if constexpr (GRAD) {
+                                for (int h0 = 0; h0 < nb64; h0 += 2) {
+                                    if (h0 + 1 < nb64)
+                                        phase_b_window<1, false, true>(P, n0 + 64 * h0, at_buf + 256u * h0, SA, first && h0 == 0, i_lo, i_hi, lane);
+                                    else
+                                        phase_b_window<0, true, true>(P, n0 + 64 * h0, at_buf + 256u * h0, SA, first && h0 == 0, i_lo, i_hi, lane);
+                                }
+                            } else {
+                                if (nb64 == 4) phase_b_window<2, false, false>(P, n0, at_buf, SA, first, i_lo, i_hi, lane);
+                                else if (nb64 == 3) phase_b_window<1, true, false>(P, n0, at_buf, SA, first, i_lo, i_hi, lane);
+                                else phase_b_window<1, false, false>(P, n0, at_buf, SA, first, i_lo, i_hi, lane);
+                            }
+                        }
                     }
                 }
-            };
-            // stage cursor (band stage, window segment), identical in every thread
-            int st = 0, wseg = 0, nws = 0;
-            while (st < n_bst && (nws = n_wseg_of(st)) == 0) ++st;
-            int buf = 0;
-            const bool a_first = ((warp >> 2) & 1) == 0; // two warps of every scheduler start with phase A
-            if (st < n_bst) phase_a(st, wseg, s_at);
-            __syncthreads();
-            while (st < n_bst) {
-                int st2 = st, wseg2 = wseg + 1, nws2 = nws;
-                if (wseg2 >= nws) {
-                    wseg2 = 0;
-                    ++st2;
-                    while (st2 < n_bst && (nws2 = n_wseg_of(st2)) == 0) ++st2;
-                }
-                const bool more = st2 < n_bst;
-                if (a_first) {
-                    if (more) phase_a(st2, wseg2, s_at + (buf ^ 1) * BUF);
-                    phase_b(st, wseg, s_at + buf * BUF);
-                } else {
-                    phase_b(st, wseg, s_at + buf * BUF);
-                    if (more) phase_a(st2, wseg2, s_at + (buf ^ 1) * BUF);
-                }
                 __syncthreads();
-                st = st2; wseg = wseg2; nws = nws2; buf ^= 1;
+                st_c = st_n; ws_c = ws_n; buf ^= 1;
+                if (st_n < n_bst && ++ws_n >= nws_n) { // advance the build cursor
+                    ws_n = 0;
+                    ++st_n;
+                    while (st_n < n_bst && (nws_n = n_wseg_of(st_n)) == 0) ++st_n;
+                }
             }
 
             // ---- epilogue: one warp per segment; a6 zero point (fp64), flux [, gradient] out (coalesced),
