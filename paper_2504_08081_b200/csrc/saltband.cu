@@ -113,6 +113,7 @@ bool allow_max_smem(const void *kern, int device, int smem_optin)
     if (!cuda_ok(cudaFuncGetAttributes(&fa, kern))) return false;
     const int dyn = smem_optin - (int)fa.sharedSizeBytes; // static + dynamic <= the opt-in limit
     if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn))) return false;
+    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     done.emplace_back(kern, device);
     return true;
 }
@@ -522,12 +523,12 @@ int launch_hoist(const sb_model *m, const sb_bands *b, const sb_batch *bt, const
     return SB_OK;
 }
 
-template <int NCL, bool GRAD>
+template <int NCL, bool GRAD, int NW>
 int launch_nw_inst(const sb_model *m, const sbn::SbNParams &np, size_t smem, int grid, cudaStream_t st)
 {
-    auto kern = sbn::sb_nw_kernel<NCL, GRAD>;
+    auto kern = sbn::sb_nw_kernel<NCL, GRAD, NW>;
     if (!allow_max_smem((const void *)kern, m->device, m->smem_optin)) return SB_ECUDA;
-    kern<<<grid, sbn::kThreads, smem, st>>>(np);
+    kern<<<grid, NW * 32, smem, st>>>(np);
     if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
     tl_launches += 1;
     tl_form = SB_FORM_TILED;
@@ -546,18 +547,29 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     const int smem_max = m->smem_optin, n_sm = m->n_sm;
     const long long n_units = (long long)bt->n_sn * bt->n_samples;
     const double mean_obs = bt->n_sn > 0 ? (double)bt->n_obs_total / (double)bt->n_sn : 1.0;
-    const int nsl = grad ? sbn::kSlots / 2 : sbn::kSlots;
-    int cap = grad ? sbn::kCapGrad : sbn::kCapFwd;
-    while (cap >= 512 && sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl).total > (size_t)smem_max) cap -= 256;
-    if (cap < 512) return 1;
-    const size_t smem = sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl).total;
+    // CTA shape: two CTAs of 8 warps per SM when their shared memory fits twice (1 KB per CTA is reserved)
+    static const int want_two = [] { const char *e = getenv("SB_NW_CTAS"); return e ? atoi(e) : 1; }();
+    int nw = want_two == 2 ? 8 : 16;
+    int nsl = 0, cap = 0;
+    for (;;) {
+        nsl = grad ? nw : 2 * nw;
+        cap = nw == 16 ? (grad ? sbn::Cfg<16>::kCapGrad : sbn::Cfg<16>::kCapFwd) : (grad ? sbn::Cfg<8>::kCapGrad : sbn::Cfg<8>::kCapFwd);
+        const size_t limit = nw == 16 ? (size_t)smem_max : (size_t)(smem_max + 1024) / 2 - 1024;
+        const int cap_min = nw == 16 ? 512 : (grad ? 384 : 768);
+        while (cap >= cap_min && sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl, nw).total > limit) cap -= 128;
+        if (cap >= cap_min) break;
+        if (nw == 8) { nw = 16; continue; } // does not fit twice: one CTA per SM
+        return 1;
+    }
+    const size_t smem = sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl, nw).total;
+    const int n_cta = nw == 16 ? n_sm : 2 * n_sm; // resident CTAs
     // groups: whole waves of n_sm groups of at most g_target units (even split of the z-ordered units),
     // g_target = as many units as fit the item slots and the round's observation capacity
     long long g_target = (long long)((double)cap / (mean_obs > 1.0 ? mean_obs : 1.0));
     if (g_target > nsl) g_target = nsl;
     if (g_target < 1) g_target = 1;
-    long long waves = (n_units + g_target * n_sm - 1) / (g_target * n_sm);
-    long long n_groups = waves * n_sm;
+    long long waves = (n_units + g_target * n_cta - 1) / (g_target * n_cta);
+    long long n_groups = waves * n_cta;
     if (n_groups > n_units) n_groups = n_units;
     if (n_groups < 1) return SB_OK;
 
@@ -612,10 +624,14 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     np.n_groups = (int32_t)n_groups;
     np.cap = cap;
     { const char *e = getenv("SB_NW_MIX"); np.mix = e ? atoi(e) : 2; }
-    const int grid = (int)(n_groups < (long long)n_sm ? n_groups : (long long)n_sm);
+    const int grid = (int)(n_groups < (long long)n_cta ? n_groups : (long long)n_cta);
     const bool small_cl = m->prm.n_cl <= 5;
-    if (grad) return small_cl ? launch_nw_inst<5, true>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, true>(m, np, smem, grid, st);
-    return small_cl ? launch_nw_inst<5, false>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, false>(m, np, smem, grid, st);
+    if (nw == 16) {
+        if (grad) return small_cl ? launch_nw_inst<5, true, 16>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, true, 16>(m, np, smem, grid, st);
+        return small_cl ? launch_nw_inst<5, false, 16>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, false, 16>(m, np, smem, grid, st);
+    }
+    if (grad) return small_cl ? launch_nw_inst<5, true, 8>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, true, 8>(m, np, smem, grid, st);
+    return small_cl ? launch_nw_inst<5, false, 8>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, false, 8>(m, np, smem, grid, st);
 }
 
 int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void *flux, const void *fluxerr,

@@ -41,15 +41,22 @@ namespace sbn {
 
 using sbh::HColour;
 
-constexpr int kWarps = 16;
-constexpr int kThreads = kWarps * 32;
 constexpr int kSlotW = 256;           // node weights per item slot (one window segment)
-constexpr int kSlots = 32;            // item slots per buffer (forward); gradient: half (two weight sets)
 constexpr int kPassSeg = kSlotW / 32; // phase-A passes per window segment
-constexpr int kBins = 2048;           // bins of the (band, phase row) counting sort
 constexpr int kMaxBands = 64;
-constexpr int kMaxSeg = 32;           // segments (units) per round
-constexpr int kCapFwd = 3072, kCapGrad = 1536; // observations per round (multiples of kThreads)
+
+// CTA shape.  NW = 16: one CTA of 16 warps per SM; NW = 8: two CTAs of 8 warps per SM (half the shared
+// memory each), so that the barriers, prologue and epilogue of one CTA overlap the other's stages.  The
+// work per warp (items per stage, observations per chunk) is the same in both.
+template <int NW> struct Cfg {
+    static constexpr int kWarps = NW;
+    static constexpr int kThreads = NW * 32;
+    static constexpr int kSlots = 2 * NW;                  // item slots per buffer (forward); gradient: half
+    static constexpr int kBins = NW == 16 ? 2048 : 1024;   // bins of the (band, phase row) counting sort
+    static constexpr int kMaxSeg = kSlots;                 // segments (units) per round
+    static constexpr int kCapFwd = NW == 16 ? 3072 : 1280; // observations per round
+    static constexpr int kCapGrad = NW == 16 ? 1536 : 640;
+};
 
 // Geometry of one item (supernova, band): depends on z and the band only (never on theta), so the pack
 // (sb_pack.cuh) can hold it.  64 bytes, loaded as four 16-byte words.
@@ -87,8 +94,9 @@ struct NUnit {           // per unit of the group (all rounds)
 
 struct NSmem {
     size_t at, ws, res, info, w, hist, wsum, bstart, segs, units, items, win, x1, slot_tab, misc, carry, total;
-    __host__ __device__ NSmem(int n_band_total, int cap, bool grad, int n_items)
+    __host__ __device__ NSmem(int n_band_total, int cap, bool grad, int n_items, int nw)
     {
+        const int kSlots = 2 * nw, kWarps = nw, kMaxSeg = 2 * nw, kBins = nw == 16 ? 2048 : 1024;
         size_t o = 0;
         at = o; o += (size_t)2 * kSlots * kSlotW * sizeof(float);
         ws = o; o += (size_t)cap * sizeof(float4) * (grad ? 2 : 1);
@@ -583,19 +591,21 @@ __device__ __forceinline__ bool obs_phase(const SbModelParams &mp, const NSeg &S
 }
 
 // ---- the kernel ---------------------------------------------------------------------------------
-template <int NCL, bool GRAD>
-__global__ void __launch_bounds__(kThreads, 1) sb_nw_kernel(const __grid_constant__ SbNParams P)
+template <int NCL, bool GRAD, int NW>
+__global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const __grid_constant__ SbNParams P)
 {
+    constexpr int kWarps = Cfg<NW>::kWarps, kThreads = Cfg<NW>::kThreads, kSlots = Cfg<NW>::kSlots;
+    constexpr int kBins = Cfg<NW>::kBins, kCapFwd = Cfg<NW>::kCapFwd, kCapGrad = Cfg<NW>::kCapGrad;
     constexpr int NSL = GRAD ? kSlots / 2 : kSlots;     // item slots per buffer
     constexpr int ATS = GRAD ? 2 * kSlotW : kSlotW;     // floats per item slot
     constexpr int BUF = kSlots * kSlotW;                // floats per buffer
-    constexpr int KPT = (GRAD ? kCapGrad : kCapFwd) / kThreads; // observations per thread in the prologue
+    constexpr int KPT = ((GRAD ? kCapGrad : kCapFwd) + kThreads - 1) / kThreads; // observations per thread in the prologue
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr unsigned FULL = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const SbModelParams &mp = P.mp;
     const int n_bands = P.n_bands, CAP = P.cap;
-    const NSmem L(P.n_band_total, CAP, GRAD, n_bands * NSL);
+    const NSmem L(P.n_band_total, CAP, GRAD, n_bands * NSL, NW);
     float *s_at = reinterpret_cast<float *>(smem_raw + L.at);
     float4 *s_ws = reinterpret_cast<float4 *>(smem_raw + L.ws);
     float *s_w = reinterpret_cast<float *>(smem_raw + L.w);
