@@ -179,6 +179,27 @@ struct NShared { // shared-state-space addresses of the arrays phase B reads
     int32_t cap;
 };
 
+// Colour-law modes of an item beyond sb::CM_*: the item's samples cross only ONE end of [cl_lo, cl_hi]
+// (one clamp and one fixed slope instead of two clamps and a slope select per sample).
+enum { CM_CROSS_HI = 3, CM_CROSS_LO = 4 };
+
+// Exponent argument of the colour factor for two wavelengths at once (packed FP32 pairs).
+template <int NCL, int CM> __device__ __forceinline__ float2 colour_arg2(const HColour<NCL> &col, float2 r)
+{
+    if constexpr (CM == CM_CROSS_HI || CM == CM_CROSS_LO) {
+        constexpr bool HI = CM == CM_CROSS_HI;
+        const float lim = HI ? col.r_hi : col.r_lo, sl = HI ? col.s_hi : col.s_lo;
+        const float2 rc = HI ? make_float2(fminf(r.x, lim), fminf(r.y, lim)) : make_float2(fmaxf(r.x, lim), fmaxf(r.y, lim));
+        const float2 d = __fadd2_rn(r, make_float2(-rc.x, -rc.y));
+        float2 p = make_float2(col.a[NCL - 1], col.a[NCL - 1]);
+#pragma unroll
+        for (int q = NCL - 2; q >= 0; --q) p = __ffma2_rn(p, rc, make_float2(col.a[q], col.a[q]));
+        return __ffma2_rn(make_float2(sl, sl), d, p);
+    } else {
+        return col.template arg2<CM>(r);
+    }
+}
+
 // ---- geometry of one item (redshift z, band b): one thread.  The in-range sample range [j_lo, j_hi) is
 // decided in fp64 (reading G9), then the window of model cells and the colour-law mode.
 struct NBandsView {
@@ -232,6 +253,8 @@ __device__ __forceinline__ void item_geometry(const SbModelParams &mp, const NBa
     const double r_min = fmin(r_a, r_b), r_max = fmax(r_a, r_b);
     const double margin = 1e-4;
     int cmode = sb::CM_GENERIC;
+    if (r_min >= mp.r_lo + margin) cmode = CM_CROSS_HI; // never below the range: only the upper continuation
+    if (r_max <= mp.r_hi - margin) cmode = CM_CROSS_LO; // never above the range
     if (r_min >= mp.r_lo + margin && r_max <= mp.r_hi - margin) {
         cmode = sb::CM_INSIDE;
     } else if (r_min >= mp.r_hi + margin) { // CL = p_hi + s_hi (r - r_hi)
@@ -276,8 +299,9 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
     const int nW = mp.n_wave;
     const float c0 = I.c0, inv_ha = I.inv_ha, ha_hi = I.ha_hi, ha_lo = I.ha_lo, hal = I.hal, r_first = I.r_first;
     const int n_in = I.n_in, ncell = I.ncell;
+    const float nc0 = -c0 * inv_ha;
     auto jstart = [&](int x) { // first band sample (relative to the first in-range one) of cell x
-        int j = (int)ceilf(((float)x - c0) * inv_ha);
+        int j = (int)ceilf(__fmaf_rn((float)x, inv_ha, nc0));
         j = min(max(j, 0), n_in); // x <= 0 gives j <= 0 because c0 >= 0
         if (x >= ncell) j = n_in;
         return j;
@@ -288,35 +312,39 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
     int carry = jstart(gq);                                // lane 0: start of its cell
     const uint32_t wbase = a_w + (uint32_t)I.wbase * 4u;
     uint32_t outp = at_slot + (uint32_t)((q_start - q_lo) * 32 + lane) * 4u;
-    auto from_left = [&](float cur, float prev, int d) {
-        const float a = __shfl_up_sync(FULL, cur, d);
-        const float b = __shfl_sync(FULL, prev, (lane - d) & 31);
-        return lane >= d ? a : b;
+    // value of lane - d: of `cur` for lanes >= d, of `prev` (the previous pass) for lanes < d -- one select
+    // and one indexed shuffle: the lanes 32 - d .. 31, which nobody reads `cur` from, offer `prev`
+    const int src1 = (lane - 1) & 31, src2 = (lane - 2) & 31, src3 = (lane - 3) & 31;
+    auto from_left = [&](float cur, float prev, int d, int src) {
+        return __shfl_sync(FULL, lane >= 32 - d ? prev : cur, src);
     };
     // moments of the lane's two cells (.x: cell g, .y: cell g + 32) -> weights on their four nodes (Keys
     // a = -1/2; linear in border cells, G2), packed; the lane's node of each pass takes its cell's w_-1
     // and w_0, w_1, w_2 of the three cells to the left
-    auto node_weights = [&](int g, float2 m0, float2 m1, float2 m2, float2 m3, float &p0, float &p1, float &p2) {
+    auto node_weights = [&](int g, bool border, float2 m0, float2 m1, float2 m2, float2 m3, float &p0, float &p1, float &p2) {
         const float2 half = make_float2(0.5f, 0.5f);
         float2 am = __fmul2_rn(half, __fadd2_rn(__ffma2_rn(make_float2(2.0f, 2.0f), m2, make_float2(-m3.x, -m3.y)),
                                                  make_float2(-m1.x, -m1.y)));
         float2 a0 = __ffma2_rn(make_float2(1.5f, 1.5f), m3, __ffma2_rn(make_float2(-2.5f, -2.5f), m2, m0));
         float2 a1 = __fmul2_rn(half, __ffma2_rn(make_float2(-3.0f, -3.0f), m3, __ffma2_rn(make_float2(4.0f, 4.0f), m2, m1)));
         float2 a2 = __fmul2_rn(half, __fadd2_rn(m3, make_float2(-m2.x, -m2.y)));
-        if (g <= 0 || g >= nW - 2) {
-            am.x = 0.f; a0.x = m0.x - m1.x; a1.x = m1.x; a2.x = 0.f;
+        if (border) { // some cell of these two passes is a border cell of the model grid (warp uniform, rare)
+            if (g <= 0 || g >= nW - 2) {
+                am.x = 0.f; a0.x = m0.x - m1.x; a1.x = m1.x; a2.x = 0.f;
+            }
+            if (g + 32 <= 0 || g + 32 >= nW - 2) {
+                am.y = 0.f; a0.y = m0.y - m1.y; a1.y = m1.y; a2.y = 0.f;
+            }
         }
-        if (g + 32 <= 0 || g + 32 >= nW - 2) {
-            am.y = 0.f; a0.y = m0.y - m1.y; a1.y = m1.y; a2.y = 0.f;
-        }
-        const float2 l0 = make_float2(from_left(a0.x, p0, 1), from_left(a0.y, a0.x, 1));
-        const float2 l1 = make_float2(from_left(a1.x, p1, 2), from_left(a1.y, a1.x, 2));
-        const float2 l2 = make_float2(from_left(a2.x, p2, 3), from_left(a2.y, a2.x, 3));
+        const float2 l0 = make_float2(from_left(a0.x, p0, 1, src1), from_left(a0.y, a0.x, 1, src1));
+        const float2 l1 = make_float2(from_left(a1.x, p1, 2, src2), from_left(a1.y, a1.x, 2, src2));
+        const float2 l2 = make_float2(from_left(a2.x, p2, 3, src3), from_left(a2.y, a2.x, 3, src3));
         p0 = a0.y;
         p1 = a1.y;
         p2 = a2.y;
         return __fadd2_rn(__fadd2_rn(__fadd2_rn(am, l0), l1), l2);
     };
+    const float2 hh = make_float2(ha_hi, ha_hi), ll = make_float2(hal, hal), cc2 = make_float2(cs, cs);
 #pragma unroll 1
     for (int q = q_start; q < q_b; q += 2) {
         const int jeA = jstart(gq + 1), jeB = jstart(gq + 33);
@@ -331,20 +359,18 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
         const int km = __reduce_max_sync(FULL, max(cntA, cntB));
         float2 m0 = make_float2(0.f, 0.f), m1 = m0, m2 = m0, m3 = m0;
         float2 n0 = m0, n1 = m0, n2 = m0, n3 = m0; // GRAD: weighted by CL
-        const float2 hh = make_float2(ha_hi, ha_hi), ll = make_float2(hal, hal), cc2 = make_float2(cs, cs);
         // u_js - cell, and the reduced wavelength of the first sample, of both cells
         float2 t2v = __fadd2_rn(__ffma2_rn(f2, make_float2(ha_lo, ha_lo),
                                            __ffma2_rn(f2, hh, make_float2(-(float)gq, -(float)(gq + 32)))),
                                 make_float2(c0, c0));
         float2 r2v = __ffma2_rn(f2, ll, make_float2(r_first, r_first));
-#pragma unroll 1
-        for (int k = 0; k < km; ++k) { // one sample of each of the two cells per trip
+        auto trip = [&](int k) { // sample k of each of the lane's two cells
             float2 w = make_float2(0.f, 0.f);
             if (k < cntA) w.x = lds32(wpA);
             if (k < cntB) w.y = lds32(wpB);
             wpA += 4u;
             wpB += 4u;
-            const float2 cl = col.template arg2<CM>(r2v);
+            const float2 cl = colour_arg2<NCL, CM>(col, r2v);
             const float2 ar = GRAD ? __fmul2_rn(cl, cc2) : cl;
             const float2 e = __fmul2_rn(make_float2(sb::exp_scaled(ar.x), sb::exp_scaled(ar.y)), w);
             const float2 tt = __fmul2_rn(t2v, t2v);
@@ -362,13 +388,22 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
             }
             t2v = __fadd2_rn(t2v, hh);
             r2v = __fadd2_rn(r2v, ll);
+        };
+        int k = 0;
+#pragma unroll 1
+        for (; k + 2 <= km; k += 2) { // two trips per iteration: their colour-law / ex2 chains overlap
+            trip(k);
+            trip(k + 1);
         }
+        if (k < km) trip(k);
+        const int g = I.g_first + gq, g0 = g - lane; // g0: cell of lane 0 in the first of the two passes
+        const bool border = g0 <= 0 || g0 + 63 >= nW - 2;
         const bool stA = q >= q_a, stB = q + 1 >= q_a && q + 1 < q_b;
-        const float2 at = node_weights(I.g_first + gq, m0, m1, m2, m3, pa0, pa1, pa2);
+        const float2 at = node_weights(g, border, m0, m1, m2, m3, pa0, pa1, pa2);
         if (stA) sts32(outp, at.x);
         if (stB) sts32(outp + 128u, at.y);
         if (GRAD) {
-            const float2 ac = node_weights(I.g_first + gq, n0, n1, n2, n3, pc0, pc1, pc2);
+            const float2 ac = node_weights(g, border, n0, n1, n2, n3, pc0, pc1, pc2);
             if (stA) sts32(outp + kSlotW * 4u, ac.x);
             if (stB) sts32(outp + kSlotW * 4u + 128u, ac.y);
         }
@@ -406,6 +441,10 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const NSeg
         phase_a_passes<NCL, sb::CM_INSIDE, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
     else if (I.cmode == sb::CM_LINEAR)
         phase_a_passes<NCL, sb::CM_LINEAR, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
+    else if (I.cmode == CM_CROSS_HI)
+        phase_a_passes<NCL, CM_CROSS_HI, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
+    else if (I.cmode == CM_CROSS_LO)
+        phase_a_passes<NCL, CM_CROSS_LO, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
     else
         phase_a_passes<NCL, sb::CM_GENERIC, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
 }
