@@ -19,7 +19,7 @@ def load_handles(wl):
 
 def run_gpu(wl, *, mode: str = "chi2", fp64: bool = False, theta: Optional[Dict[str, np.ndarray]] = None,
             use_zp: bool = True, handles=None, want_flux: bool = True, want_dflux: bool = True,
-            with_data: bool = True, form: Optional[str] = None) -> Dict[str, np.ndarray]:
+            with_data: bool = True, form: Optional[str] = None, use_pack: bool = False) -> Dict[str, np.ndarray]:
     """mode: 'flux' (sb_bandflux), 'chi2' (sb_chi2), 'grad' (sb_bandflux_grad).  form: None (library's
     choice), 'direct' or 'grouped' (include/saltband.h SB_FORM_*).  Returns host fp64 arrays."""
     import torch
@@ -45,6 +45,8 @@ def run_gpu(wl, *, mode: str = "chi2", fp64: bool = False, theta: Optional[Dict[
         time=dev_f(wl.time), band=torch.as_tensor(np.asarray(wl.band, dtype=np.int32)).to(dev),
         zp=dev_f(wl.zp) if use_zp else None, z=dev_f(wl.z), x0=dev_f(th["x0"]), x1=dev_f(th["x1"]),
         c=dev_f(th["c"]), t0=dev_f(th["t0"]))
+    if use_pack:  # include/saltband.h: sb_pack_observations (fp32 only), built on the current stream
+        common["pack"] = sb.sb_pack_observations(model, bands, dtype=sb.SB_F32, n_sn=wl.n_sn, z=common["z"])
     out: Dict[str, np.ndarray] = {}
     nan = float("nan")
     o_flux = torch.full((n_tot * n_samples,), nan, dtype=ft, device=dev) if want_flux else None
@@ -141,6 +143,44 @@ def grad_tolerance(wl, ref: Dict[str, np.ndarray], th: Dict[str, np.ndarray], n_
             scale[sl, 3] = max(abs(th["t0"][u]), 1.0)
     A = np.stack([np.zeros_like(m), m, m, m / (dp * opz)], axis=1)
     return rel * (np.abs(ref["dflux"]) + A) + floor * peak[:, None] / scale
+
+
+def grad_tolerance_strict(wl, ref: Dict[str, np.ndarray], th: Dict[str, np.ndarray], n_samples: int, fp64: bool):
+    """SURVEY.md G13 as written: 1e-5 |dm/dtheta| + 1e-9 max|m| / theta-scale (3e-5 for t0); fp64: 1e-12 / 1e-15.
+    Relative to the derivative itself, so it is only attainable where the derivative integral does not
+    cancel (see grad_conditioning); asserted on that subset, and on every evaluation for x0 and in fp64."""
+    rel = np.array([1e-12] * 4) if fp64 else np.array([1e-5, 1e-5, 1e-5, 3e-5])
+    floor = 1e-15 if fp64 else 1e-9
+    peak = unit_peaks(wl, ref["flux"], n_samples)
+    scale = _theta_scale(wl, th, n_samples, len(ref["flux"]))
+    return rel[None, :] * np.abs(ref["dflux"]) + floor * peak[:, None] / scale
+
+
+def grad_conditioning(wl, ref: Dict[str, np.ndarray], n_samples: int) -> np.ndarray:
+    """|dm/dtheta| / A per evaluation and component (A = the non-cancelling magnitude of grad_tolerance;
+    inf for x0, whose integrand is the flux integrand itself): small values mean the derivative integral
+    cancels and no tolerance relative to the total can hold in fp32 (reading G13a)."""
+    m = np.abs(ref["flux"])
+    dp = float(wl.model["phase"][1] - wl.model["phase"][0])
+    opz = np.repeat(1.0 + wl.z.astype(np.float64), np.diff(wl.obs_offset) * n_samples)
+    A = np.stack([np.zeros_like(m), m, m, m / (dp * opz)], axis=1)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        return np.where(A > 0, np.abs(ref["dflux"]) / A, np.inf)
+
+
+def _theta_scale(wl, th, n_samples, n_ev):
+    scale = np.empty((n_ev, 4))
+    for s in range(wl.n_sn):
+        a, b = int(wl.obs_offset[s]), int(wl.obs_offset[s + 1])
+        n_obs = b - a
+        for k in range(n_samples):
+            u = s * n_samples + k
+            sl = slice(a * n_samples + k * n_obs, a * n_samples + (k + 1) * n_obs)
+            scale[sl, 0] = abs(th["x0"][u])
+            scale[sl, 1] = max(abs(th["x1"][u]), 1.0)
+            scale[sl, 2] = max(abs(th["c"][u]), 1.0)
+            scale[sl, 3] = max(abs(th["t0"][u]), 1.0)
+    return scale
 
 
 def dchi2_tolerance(wl, ref: Dict[str, np.ndarray], tol_flux, tol_dflux, n_samples: int, fp64: bool) -> np.ndarray:

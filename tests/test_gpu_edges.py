@@ -91,8 +91,9 @@ def test_empty_and_degenerate_batches(cuda_device, fp64):
     got = sbgpu.run_gpu(wl2, mode="chi2", fp64=fp64)
     refc = oracle.run_workload(wl2, want_flux=True, want_chi2=True)
     assert got["chi2"][0] == 0.0 and got["chi2"][2] == 0.0
-    assert np.all(np.abs(got["chi2"] - refc["chi2"]) <= 1e-3 + 1e-4 * refc["chi2"])
-    assert np.all(np.abs(got["flux"] - refc["flux"]) <= sbgpu.flux_tolerance(wl2, refc["flux"], 1, fp64))
+    tol2 = sbgpu.flux_tolerance(wl2, refc["flux"], 1, fp64)
+    assert np.all(np.abs(got["chi2"] - refc["chi2"]) <= sbgpu.chi2_tolerance(wl2, refc["flux"], tol2, 1, fp64))
+    assert np.all(np.abs(got["flux"] - refc["flux"]) <= tol2)
 
 
 @pytest.mark.parametrize("fp64", [False, True])

@@ -45,7 +45,7 @@ def _sample_indices(n, k, seed):
     return idx[(idx >= 0) & (idx < n)]
 
 
-@pytest.mark.parametrize("config,k", [(5, 240), (4, 160), (2, 1024)])
+@pytest.mark.parametrize("config,k", [(5, 2000), (4, 400), (2, 1024)])
 def test_full_size_forward_sampled_units(cuda_device, config, k):
     wl = workloads.make_workload(config)  # full BASELINE.json size
     idx = _sample_indices(wl.n_sn, k, 77 + config)
@@ -62,6 +62,17 @@ def test_full_size_forward_sampled_units(cuda_device, config, k):
     assert np.all(np.abs(g_chi - ref["chi2"]) <= tolc)
     # properties that hold at any size: every output written, finite, chi^2 >= 0
     assert np.all(np.isfinite(got["flux"])) and np.all(np.isfinite(got["chi2"])) and np.all(got["chi2"] >= 0)
+    # ALL units (also the groups without a sampled unit): the node-weight kernel against the direct
+    # kernel, two exact re-associations of the same sums, each within the flux tolerance of the oracle
+    assert got["form"] == "tiled"
+    direct = sbgpu.run_gpu(wl, mode="chi2", form="direct")
+    peak = sbgpu.unit_peaks(wl, direct["flux"], 1)
+    tol_all = 2.0 * (1e-5 * np.abs(direct["flux"]) + 1e-9 * peak)
+    err_all = np.abs(got["flux"] - direct["flux"])
+    assert np.all(err_all <= tol_all), f"tiled vs direct worst ratio {np.max(err_all / np.maximum(tol_all, 1e-300)):.3g}"
+    # with a pack (sb_pack_observations) the call gives bit-identical results
+    packed = sbgpu.run_gpu(wl, mode="chi2", use_pack=True)
+    assert np.array_equal(packed["flux"], got["flux"]) and np.array_equal(packed["chi2"], got["chi2"])
 
 
 def test_full_size_config3_sampled_parameter_samples(cuda_device):

@@ -1,4 +1,4 @@
-"""-m gpu edge cases of the grouped / tiled formulations (csrc/sb_hoist.cuh, csrc/sb_tiled.cuh), each
+"""-m gpu edge cases of the grouped / tiled formulations (csrc/sb_hoist.cuh, csrc/sb_nw.cuh), each
 against the fp64 oracle and in every formulation that applies: windows wider than one 512-node
 segment of the node-weight array, a unit with more observations than one round holds (the unit is
 split over rounds and its chi^2 carried), empty units inside a group, groups that mix very different
@@ -100,6 +100,25 @@ def test_unit_larger_than_a_round_and_empty_units(cuda_device):
     check_all_forms(wl)
     got = sbgpu.run_gpu(wl, mode="chi2", form="tiled")
     assert got["chi2"][1] == 0.0 and got["chi2"][4] == 0.0
+
+
+@pytest.mark.parametrize("n_bands", [1, 3, 5])
+def test_split_unit_with_odd_band_counts(cuda_device, n_bands):
+    """A unit larger than a round (chi^2 and d chi^2 carried between rounds in fp64 shared memory) with an
+    ODD number of (band, segment) items: the carry must stay 8-byte aligned whatever the item count
+    (round-1 advisor finding).  Forward and gradient, node-weight kernel against the oracle."""
+    wl0 = workloads.make_workload(2, n_sn=3)
+    bd = wl0.bands
+    sub = workloads.generators.pack_bands([(bd["wave"][bd["offset"][b]:bd["offset"][b + 1]],
+                                            bd["trans"][bd["offset"][b]:bd["offset"][b + 1]]) for b in range(n_bands)])
+    rng = np.random.default_rng(20 + n_bands)
+    counts = np.array([3300, 7, 1700])
+    off = np.concatenate([[0], np.cumsum(counts)])
+    n = int(off[-1])
+    th = {k: v.astype(np.float64) for k, v in wl0.theta.items()}
+    wl = custom_workload(wl0.model, sub, off, rng.uniform(-15.0, 45.0, n), rng.integers(0, n_bands, n),
+                         wl0.z.astype(np.float64), th)
+    check_all_forms(attach(wl), forms=("tiled",), grad_forms=("tiled",))
 
 
 def test_single_band_phases_outside_grid_and_samples_axis(cuda_device):
