@@ -191,6 +191,55 @@ int sb_bandflux_grad_host(const sb_model *m, const sb_bands *b, const sb_batch *
                           const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2,
                           void *out_dchi2);
 
+/* sb_fit_lbfgs -- device-resident batched fit of (x0, x1, c, t0): every unit (supernova, parameter sample)
+ * is one optimiser LANE that minimises its own chi^2 ("fmin_bfgs.py ... optimisation via
+ * L-BFGS-B" is one of the paper's two workloads; the paper gives no algorithmic detail, the algorithm is
+ * reading G16 of DESIGN.md).  Limited-memory BFGS (two-loop recursion, `memory` curvature pairs) with a
+ * backtracking Armijo line search (c1 = 1e-4, step halved on rejection, at most 30 halvings) and an
+ * optional box (trial points are projected on it).  Lanes work in scaled variables u = theta / s,
+ * s = (x0 of the start point, 1, 1, 1).  One STEP = one batched evaluation of chi^2 and its gradient at
+ * every running lane's trial point (the kernels of sb_bandflux_grad, through batch->pack when given)
+ * plus one lane-update kernel; the call enqueues exactly max_eval steps on `stream` and returns: there
+ * is NO host synchronisation and no device-to-host copy.  Stopped lanes are skipped by the evaluation
+ * kernels, and steps after the last lane has stopped return at once.
+ *   batch          as for sb_bandflux_grad; x0, x1, c, t0 are the START point of every lane (not modified)
+ *   flux, fluxerr  DEVICE [n_obs_total], required
+ *   opts           see sb_fit_opts; all fields must be set (sb_fit_default_opts fills the defaults)
+ *   result         DEVICE outputs, written when a lane stops (all lanes have stopped when the call's work
+ *                  is complete): theta [n_units][4] = (x0, x1, c, t0) of the last accepted point and chi2
+ *                  [n_units], both of the batch's element type; optional int32 status (0 running -- never
+ *                  seen after completion, 1 converged, 2 line search stalled, 3 budget exhausted), n_iter
+ *                  (accepted steps), n_eval (evaluations) [n_units]; optional trace [trace_len][n_units]
+ *                  fp64: chi^2 after i accepted steps (row 0: start point; NaN where not reached).
+ * A lane converges when an accepted step lowers chi^2 by <= ftol * max(|chi2_old|, |chi2_new|, 1) or
+ * when max_k |d chi^2 / d u_k| <= gtol.  In SB_F32 batches every trial point is rounded to fp32 (the
+ * kernels take fp32 parameters); lane state and all optimiser arithmetic are fp64.  Lane state lives in a
+ * workspace owned by the sb_bands handle (one per stream, as for the compute calls; ~0.7 KB per lane).
+ * Errors as for the compute calls; SB_EINVAL for out-of-range options. */
+typedef struct {
+    int32_t memory;    /* curvature pairs kept per lane, 1..8 (default 8) */
+    int32_t max_eval;  /* evaluations per lane = steps enqueued, >= 1 (default 60) */
+    int32_t max_iter;  /* accepted steps per lane, >= 1 (default 1000) */
+    int32_t trace_len; /* rows of result->trace (0: no trace) */
+    double ftol, gtol; /* >= 0 (defaults 1e-12, 0) */
+    const double *lo, *hi; /* HOST [4] box on (x0, x1, c, t0) in theta units, or NULL: no bound on that side */
+} sb_fit_opts;
+
+typedef struct {
+    void *theta, *chi2;                /* [n_units][4], [n_units], element type of the batch; required */
+    int32_t *status, *n_iter, *n_eval; /* [n_units] each, or NULL */
+    double *trace;                     /* [trace_len][n_units] or NULL (required iff trace_len > 0) */
+} sb_fit_result;
+
+void sb_fit_default_opts(sb_fit_opts *opts);
+int sb_fit_lbfgs(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+                 const void *fluxerr, const sb_fit_opts *opts, const sb_fit_result *result, void *stream);
+/* The same fit for data in HOST memory (every pointer of batch, flux, fluxerr and result is a HOST
+ * pointer): copies the batch to a device buffer owned by the sb_bands handle, builds a pack, runs the
+ * fit, copies the results back and returns when they are complete.  batch->pack must be NULL. */
+int sb_fit_lbfgs_host(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+                      const void *fluxerr, const sb_fit_opts *opts, const sb_fit_result *result);
+
 /* Introspection (host side, cheap). */
 int32_t sb_bands_count(const sb_bands *b);
 /* ZPAB_b as computed at load (fp64), or NaN for a bad index. */

@@ -11,6 +11,10 @@ from .api import (  # noqa: F401
     SB_FORM_DIRECT,
     SB_FORM_GROUPED,
     SB_FORM_TILED,
+    FIT_CONVERGED,
+    FIT_EXHAUSTED,
+    FIT_RUNNING,
+    FIT_STALLED,
     Bands,
     Model,
     Pack,
@@ -23,6 +27,8 @@ from .api import (  # noqa: F401
     sb_bandflux_grad_host,
     sb_chi2,
     sb_chi2_host,
+    sb_fit_lbfgs,
+    sb_fit_lbfgs_host,
     sb_load_bandpasses,
     sb_load_model,
     sb_pack_observations,

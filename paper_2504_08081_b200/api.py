@@ -31,6 +31,18 @@ class _Batch(C.Structure):
     ]
 
 
+class _FitOpts(C.Structure):
+    _fields_ = [("memory", C.c_int32), ("max_eval", C.c_int32), ("max_iter", C.c_int32), ("trace_len", C.c_int32),
+                ("ftol", C.c_double), ("gtol", C.c_double), ("lo", C.POINTER(C.c_double)), ("hi", C.POINTER(C.c_double))]
+
+
+class _FitResult(C.Structure):
+    _fields_ = [("theta", C.c_void_p), ("chi2", C.c_void_p), ("status", C.c_void_p), ("n_iter", C.c_void_p),
+                ("n_eval", C.c_void_p), ("trace", C.c_void_p)]
+
+
+FIT_RUNNING, FIT_CONVERGED, FIT_STALLED, FIT_EXHAUSTED = 0, 1, 2, 3  # sb_fit_result.status
+
 _lib = None
 
 
@@ -71,6 +83,12 @@ def _load():
     L.sb_chi2_host.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp]
     L.sb_bandflux_grad_host.restype = C.c_int
     L.sb_bandflux_grad_host.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp, vp, vp]
+    L.sb_fit_default_opts.restype = None
+    L.sb_fit_default_opts.argtypes = [C.POINTER(_FitOpts)]
+    L.sb_fit_lbfgs.restype = C.c_int
+    L.sb_fit_lbfgs.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, C.POINTER(_FitOpts), C.POINTER(_FitResult), vp]
+    L.sb_fit_lbfgs_host.restype = C.c_int
+    L.sb_fit_lbfgs_host.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, C.POINTER(_FitOpts), C.POINTER(_FitResult)]
     L.sb_bands_count.restype = C.c_int32
     L.sb_bands_count.argtypes = [vp]
     L.sb_bands_zpab.restype = C.c_double
@@ -338,3 +356,69 @@ def sb_bandflux_grad_host(model: Model, bands: Bands, *, dtype: int, n_sn: int, 
         _hptr(out_chi2, ft, n_units, "out_chi2", allow_none=True),
         _hptr(out_dchi2, ft, n_units * 4, "out_dchi2", allow_none=True))
     _check(rc, "sb_bandflux_grad_host")
+
+
+# ---------------------------------------------------------------- batched L-BFGS fit
+def _fit_opts(memory, max_eval, max_iter, trace_len, ftol, gtol, lo, hi):
+    """sb_fit_opts with the library's defaults (sb_fit_default_opts) for every argument left None."""
+    o = _FitOpts()
+    _load().sb_fit_default_opts(C.byref(o))
+    keep = []
+    for name, v in (("memory", memory), ("max_eval", max_eval), ("max_iter", max_iter), ("trace_len", trace_len),
+                    ("ftol", ftol), ("gtol", gtol)):
+        if v is not None:
+            setattr(o, name, v)
+    for name, v in (("lo", lo), ("hi", hi)):
+        if v is not None:
+            arr = _f64(v)
+            if arr.shape != (4,):
+                raise ValueError(f"{name} must have 4 elements (x0, x1, c, t0)")
+            keep.append(arr)
+            setattr(o, name, _dptr(arr))
+    return o, keep
+
+
+def sb_fit_lbfgs(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,
+                 obs_offset, time, band, zp, z, x0, x1, c, t0, flux, fluxerr, out_theta, out_chi2, out_status=None,
+                 out_n_iter=None, out_n_eval=None, out_trace=None, pack=None, memory=None, max_eval=None,
+                 max_iter=None, ftol=None, gtol=None, lo=None, hi=None) -> None:
+    """include/saltband.h: sb_fit_lbfgs.  x0, x1, c, t0 are the start point; every array is a CUDA tensor; the
+    fit is enqueued on the current stream (no synchronisation).  out_trace: [trace_len, n_units] fp64."""
+    import torch
+
+    ft = torch.float32 if (dtype & 0xFF) == SB_F32 else torch.float64
+    n_units = n_sn * n_samples
+    bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total, pack)
+    trace_len = 0 if out_trace is None else out_trace.shape[0]
+    opts, keep = _fit_opts(memory, max_eval, max_iter, trace_len, ftol, gtol, lo, hi)
+    res = _FitResult(_ptr(out_theta, ft, 4 * n_units, "out_theta"), _ptr(out_chi2, ft, n_units, "out_chi2"),
+                     _ptr(out_status, torch.int32, n_units, "out_status", allow_none=True),
+                     _ptr(out_n_iter, torch.int32, n_units, "out_n_iter", allow_none=True),
+                     _ptr(out_n_eval, torch.int32, n_units, "out_n_eval", allow_none=True),
+                     _ptr(out_trace, torch.float64, trace_len * n_units, "out_trace", allow_none=True))
+    rc = _load().sb_fit_lbfgs(model._h, bands._h, C.byref(bt), _ptr(flux, ft, n_obs_total, "flux"),
+                              _ptr(fluxerr, ft, n_obs_total, "fluxerr"), C.byref(opts), C.byref(res), _stream())
+    del keep
+    _check(rc, "sb_fit_lbfgs")
+
+
+def sb_fit_lbfgs_host(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,
+                      obs_offset, time, band, zp, z, x0, x1, c, t0, flux, fluxerr, out_theta, out_chi2,
+                      out_status=None, out_n_iter=None, out_n_eval=None, out_trace=None, memory=None, max_eval=None,
+                      max_iter=None, ftol=None, gtol=None, lo=None, hi=None) -> None:
+    """include/saltband.h: sb_fit_lbfgs_host.  Every array is a CPU tensor; returns when the results are complete."""
+    import torch
+
+    ft, bt = _host_batch(dtype, n_sn, n_samples, n_obs_total, obs_offset, time, band, zp, z, x0, x1, c, t0)
+    n_units = n_sn * n_samples
+    trace_len = 0 if out_trace is None else out_trace.shape[0]
+    opts, keep = _fit_opts(memory, max_eval, max_iter, trace_len, ftol, gtol, lo, hi)
+    res = _FitResult(_hptr(out_theta, ft, 4 * n_units, "out_theta"), _hptr(out_chi2, ft, n_units, "out_chi2"),
+                     _hptr(out_status, torch.int32, n_units, "out_status", allow_none=True),
+                     _hptr(out_n_iter, torch.int32, n_units, "out_n_iter", allow_none=True),
+                     _hptr(out_n_eval, torch.int32, n_units, "out_n_eval", allow_none=True),
+                     _hptr(out_trace, torch.float64, trace_len * n_units, "out_trace", allow_none=True))
+    rc = _load().sb_fit_lbfgs_host(model._h, bands._h, C.byref(bt), _hptr(flux, ft, n_obs_total, "flux"),
+                                   _hptr(fluxerr, ft, n_obs_total, "fluxerr"), C.byref(opts), C.byref(res))
+    del keep
+    _check(rc, "sb_fit_lbfgs_host")

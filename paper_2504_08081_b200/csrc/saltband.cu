@@ -15,6 +15,7 @@
 #include "sb_kernels.cuh"
 #include "sb_hoist.cuh"
 #include "sb_nw.cuh"
+#include "sb_fit.cuh"
 
 // Per-stream workspaces and host-call contexts of a bands handle.  This is the only mutable state
 // behind the handles: a cache, guarded by `mu`.  A compute call without a pack needs a few hundred KB
@@ -23,11 +24,13 @@
 // keeps until sb_free_bands.  Calls on distinct streams never share a slot; calls on the same stream
 // are ordered by the stream.  Replaced buffers are retired, not freed: earlier work may still use them.
 struct SbScratch {
-    struct Slot { cudaStream_t stream; unsigned char *buf; size_t bytes; };
+    struct Slot { cudaStream_t stream; int kind; unsigned char *buf; size_t bytes; };
     struct HostCtx { // one per concurrent host-buffer call: three streams and their staging slabs
         cudaStream_t st[3];
         unsigned char *slab[3];
         size_t slab_bytes;
+        unsigned char *fit_slab; // sb_fit_lbfgs_host: the whole batch, resident for the duration of the fit
+        size_t fit_bytes;
         bool busy;
     };
     std::mutex mu;
@@ -120,12 +123,13 @@ bool allow_max_smem(const void *kern, int device, int smem_optin)
 
 // Workspace of at least `bytes` for calls on `stream` (see SbScratch).  Allocates only when the stream
 // has no slot yet or its slot is too small.
-unsigned char *scratch_for(const sb_bands *b, cudaStream_t stream, size_t bytes)
+enum { kScratchSort = 0, kScratchFit = 1 }; // what a slot is for: calls of different kinds may nest
+unsigned char *scratch_for(const sb_bands *b, cudaStream_t stream, size_t bytes, int kind = kScratchSort)
 {
     SbScratch *sc = b->scratch;
     std::lock_guard<std::mutex> lock(sc->mu);
     for (auto &s : sc->slots)
-        if (s.stream == stream) {
+        if (s.stream == stream && s.kind == kind) {
             if (s.bytes >= bytes) return s.buf;
             unsigned char *nb = nullptr;
             const size_t want = bytes + bytes / 2;
@@ -137,7 +141,7 @@ unsigned char *scratch_for(const sb_bands *b, cudaStream_t stream, size_t bytes)
         }
     unsigned char *nb = nullptr;
     if (!cuda_ok(cudaMalloc((void **)&nb, bytes))) return nullptr;
-    sc->slots.push_back({stream, nb, bytes});
+    sc->slots.push_back({stream, kind, nb, bytes});
     return nb;
 }
 
@@ -342,6 +346,7 @@ void sb_free_bands(sb_bands *b)
                 if (c->slab[i]) cudaFree(c->slab[i]);
                 if (c->st[i]) cudaStreamDestroy(c->st[i]);
             }
+            if (c->fit_slab) cudaFree(c->fit_slab);
             delete c;
         }
         delete b->scratch;
@@ -523,6 +528,11 @@ int launch_hoist(const sb_model *m, const sb_bands *b, const sb_batch *bt, const
     return SB_OK;
 }
 
+// Fit driver only: per-unit "live" flags and their count, written by the lane kernels (sb_fit.cuh) and
+// read by the evaluation kernels, which skip the units of stopped lanes and return at once when no lane
+// is left.
+struct RunLive { const int32_t *live = nullptr, *n_live = nullptr; };
+
 template <int NCL, bool GRAD, int NW>
 int launch_nw_inst(const sb_model *m, const sbn::SbNParams &np, size_t smem, int grid, cudaStream_t st)
 {
@@ -540,7 +550,8 @@ int launch_nw_inst(const sb_model *m, const sbn::SbNParams &np, size_t smem, int
 // stream workspace first and the item geometry is computed inside the kernel.  Returns 1 when the
 // kernel does not apply.
 int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *bt, const void *flux,
-              const void *fluxerr, void *out_flux, void *out_chi2, void *out_dflux, void *out_dchi2, cudaStream_t st)
+              const void *fluxerr, void *out_flux, void *out_chi2, void *out_dflux, void *out_dchi2, cudaStream_t st,
+              const RunLive &lv)
 {
     if (!b->all_uniform || m->prm.n_cl > SB_MAX_CL || b->n_bands > sbn::kMaxBands) return 1;
     if (m->prm.n_phase < 4 || m->prm.n_phase > 4096) return 1;
@@ -621,6 +632,8 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     np.out_dchi2 = (float *)out_dchi2;
     np.perm = perm;
     np.geom = geom;
+    np.live = lv.live;
+    np.n_live = lv.n_live;
     np.n_groups = (int32_t)n_groups;
     np.cap = cap;
     { const char *e = getenv("SB_NW_MIX"); np.mix = e ? atoi(e) : 2; }
@@ -635,7 +648,8 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
 }
 
 int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void *flux, const void *fluxerr,
-        void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2, void *stream, bool grad)
+        void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2, void *stream, bool grad,
+        const RunLive &lv = RunLive())
 {
     tl_launches = 0;
     tl_form = 0;
@@ -689,12 +703,13 @@ int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void 
     kp.out_dflux = out_dflux;
     kp.out_chi2 = out_chi2;
     kp.out_dchi2 = out_dchi2;
+    kp.n_live = lv.n_live;
     cudaStream_t st = (cudaStream_t)stream;
     // automatic choice: calls too small to fill the warps of one CTA per SM go to the direct kernel
     const bool tiny = form == 0 && (long long)bt->n_obs_total * bt->n_samples < 4096;
     if (f32 && form != SB_FORM_DIRECT && !tiny && bt->n_obs_total > 0) {
         if (form != SB_FORM_GROUPED) {
-            const int rc = launch_nw(grad, m, b, bt, flux, fluxerr, out_flux, out_chi2, out_dflux, out_dchi2, st);
+            const int rc = launch_nw(grad, m, b, bt, flux, fluxerr, out_flux, out_chi2, out_dflux, out_dchi2, st, lv);
             if (rc != 1) return rc;
         }
         if (form != SB_FORM_TILED && !grad) {
@@ -987,6 +1002,237 @@ int sb_bandflux_grad_host(const sb_model *m, const sb_bands *b, const sb_batch *
                           const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2)
 {
     return run_host(m, b, batch, flux, fluxerr, out_flux, out_dflux, out_chi2, out_dchi2, true);
+}
+
+} // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// Device-resident batched L-BFGS fit (sb_fit.cuh): one lane per unit, no host synchronisation
+// ------------------------------------------------------------------------------------------
+namespace {
+
+struct FitLayout { // carve-up of the fit workspace (kScratchFit slot of the call's stream)
+    size_t theta[4], chi2, dchi2, u, g, d, ut, f, alpha, scale, S, Y, ints[7], n_live, bytes;
+    FitLayout(size_t n, size_t es, int memory)
+    {
+        size_t o = 0;
+        auto take = [&](size_t b) { const size_t at = o; o += (b + 255) & ~(size_t)255; return at; };
+        for (int k = 0; k < 4; ++k) theta[k] = take(es * n);
+        chi2 = take(es * n);
+        dchi2 = take(4 * es * n);
+        u = take(32 * n); g = take(32 * n); d = take(32 * n); ut = take(32 * n);
+        f = take(8 * n); alpha = take(8 * n); scale = take(8 * n);
+        S = take((size_t)memory * 32 * n); Y = take((size_t)memory * 32 * n);
+        for (int k = 0; k < 7; ++k) ints[k] = take(4 * n);
+        n_live = take(256);
+        bytes = o;
+    }
+};
+
+int fit_check_opts(const sb_fit_opts *o)
+{
+    if (!o) return SB_EINVAL;
+    if (o->memory < 1 || o->memory > sbf::kMaxMemory || o->max_eval < 1 || o->max_iter < 1 || o->trace_len < 0) return SB_EINVAL;
+    if (!(o->ftol >= 0.0) || !(o->gtol >= 0.0)) return SB_EINVAL;
+    if (o->lo && o->hi)
+        for (int k = 0; k < 4; ++k)
+            if (!(o->lo[k] <= o->hi[k])) return SB_EINVAL;
+    return SB_OK;
+}
+
+int fit_device(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void *flux, const void *fluxerr,
+               const sb_fit_opts *opts, const sb_fit_result *res, cudaStream_t st)
+{
+    tl_launches = 0;
+    tl_form = 0;
+    if (!m || !b || !bt_in || !flux || !fluxerr || !res) return SB_EINVAL;
+    int rc = fit_check_opts(opts);
+    if (rc != SB_OK) return rc;
+    const int32_t base = bt_in->dtype & 0xff;
+    if (base != SB_F32 && base != SB_F64) return SB_EINVAL;
+    if (bt_in->n_sn < 0 || bt_in->n_samples < 1 || bt_in->n_obs_total < 0) return SB_EINVAL;
+    if (bt_in->n_sn == 0) return SB_OK;
+    if (!res->theta || !res->chi2) return SB_EINVAL;
+    if (opts->trace_len > 0 && !res->trace) return SB_EINVAL;
+    if (!bt_in->x0 || !bt_in->x1 || !bt_in->c || !bt_in->t0) return SB_EINVAL;
+    const long long n_units = (long long)bt_in->n_sn * bt_in->n_samples;
+    if (n_units >= (1LL << 31)) return SB_ELIMIT;
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return SB_ECUDA;
+    if (dev != m->device || dev != b->device) return SB_EINVAL;
+    const size_t es = base == SB_F32 ? 4 : 8, n = (size_t)n_units;
+    const FitLayout L(n, es, opts->memory);
+    unsigned char *ws = scratch_for(b, st, L.bytes, kScratchFit);
+    if (!ws) return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+
+    sbf::FitParams F;
+    memset(&F, 0, sizeof(F));
+    F.st.u = (double *)(ws + L.u); F.st.g = (double *)(ws + L.g); F.st.d = (double *)(ws + L.d); F.st.ut = (double *)(ws + L.ut);
+    F.st.f = (double *)(ws + L.f); F.st.alpha = (double *)(ws + L.alpha); F.st.scale = (double *)(ws + L.scale);
+    F.st.S = (double *)(ws + L.S); F.st.Y = (double *)(ws + L.Y);
+    F.st.n_hist = (int32_t *)(ws + L.ints[0]); F.st.head = (int32_t *)(ws + L.ints[1]); F.st.n_eval = (int32_t *)(ws + L.ints[2]);
+    F.st.n_iter = (int32_t *)(ws + L.ints[3]); F.st.n_back = (int32_t *)(ws + L.ints[4]); F.st.status = (int32_t *)(ws + L.ints[5]);
+    F.st.live = (int32_t *)(ws + L.ints[6]);
+    F.st.n_live = (int32_t *)(ws + L.n_live);
+    F.n = (int32_t)n_units;
+    F.memory = opts->memory; F.max_eval = opts->max_eval; F.max_iter = opts->max_iter; F.trace_len = opts->trace_len;
+    F.ftol = opts->ftol; F.gtol = opts->gtol;
+    F.has_box = (opts->lo || opts->hi) ? 1 : 0;
+    for (int k = 0; k < 4; ++k) {
+        F.lo[k] = opts->lo ? opts->lo[k] : -INFINITY;
+        F.hi[k] = opts->hi ? opts->hi[k] : INFINITY;
+    }
+    F.x0 = ws + L.theta[0]; F.x1 = ws + L.theta[1]; F.c = ws + L.theta[2]; F.t0 = ws + L.theta[3];
+    F.chi2 = ws + L.chi2; F.dchi2 = ws + L.dchi2;
+    F.theta_out = res->theta; F.chi2_out = res->chi2;
+    F.status_out = res->status; F.n_iter_out = res->n_iter; F.n_eval_out = res->n_eval;
+    F.trace_out = res->trace;
+
+    const unsigned blocks_i = (unsigned)((n + 255) / 256), blocks_u = (unsigned)((n + 127) / 128);
+    int32_t launches = 0, form = 0;
+    if (base == SB_F32)
+        sbf::sb_fit_init_kernel<float><<<blocks_i, 256, 0, st>>>(F, (const float *)bt_in->x0, (const float *)bt_in->x1,
+                                                                  (const float *)bt_in->c, (const float *)bt_in->t0);
+    else
+        sbf::sb_fit_init_kernel<double><<<blocks_i, 256, 0, st>>>(F, (const double *)bt_in->x0, (const double *)bt_in->x1,
+                                                                   (const double *)bt_in->c, (const double *)bt_in->t0);
+    if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
+    launches += 1;
+    sb_batch eb = *bt_in; // the evaluation batch: the caller's observations at the lanes' trial parameters
+    eb.x0 = F.x0; eb.x1 = F.x1; eb.c = F.c; eb.t0 = F.t0;
+    const RunLive lv{F.st.live, F.st.n_live};
+    for (int e = 0; e < opts->max_eval; ++e) {
+        rc = run(m, b, &eb, flux, fluxerr, nullptr, nullptr, ws + L.chi2, ws + L.dchi2, (void *)st, true, lv);
+        if (rc != SB_OK) return rc;
+        launches += tl_launches;
+        form = tl_form;
+        if (base == SB_F32) sbf::sb_fit_update_kernel<float><<<blocks_u, 128, 0, st>>>(F);
+        else sbf::sb_fit_update_kernel<double><<<blocks_u, 128, 0, st>>>(F);
+        if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
+        launches += 1;
+    }
+    tl_launches = launches;
+    tl_form = form;
+    return SB_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+void sb_fit_default_opts(sb_fit_opts *o)
+{
+    if (!o) return;
+    o->memory = 8;
+    o->max_eval = 60;
+    o->max_iter = 1000;
+    o->trace_len = 0;
+    o->ftol = 1e-12;
+    o->gtol = 0.0;
+    o->lo = nullptr;
+    o->hi = nullptr;
+}
+
+int sb_fit_lbfgs(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux, const void *fluxerr,
+                 const sb_fit_opts *opts, const sb_fit_result *result, void *stream)
+{
+    NvtxRange nvtx("sb_fit_lbfgs");
+    return fit_device(m, b, batch, flux, fluxerr, opts, result, (cudaStream_t)stream);
+}
+
+int sb_fit_lbfgs_host(const sb_model *m, const sb_bands *b, const sb_batch *hb, const void *flux, const void *fluxerr,
+                      const sb_fit_opts *opts, const sb_fit_result *hres)
+{
+    NvtxRange nvtx("sb_fit_lbfgs_host");
+    tl_launches = 0;
+    tl_form = 0;
+    if (!m || !b || !hb || !flux || !fluxerr || !hres) return SB_EINVAL;
+    int rc = fit_check_opts(opts);
+    if (rc != SB_OK) return rc;
+    const int32_t base = hb->dtype & 0xff;
+    if (base != SB_F32 && base != SB_F64) return SB_EINVAL;
+    if (hb->n_sn < 0 || hb->n_samples < 1 || hb->n_obs_total < 0 || hb->pack) return SB_EINVAL;
+    if (hb->n_sn == 0) return SB_OK;
+    if (!hb->obs_offset || !hb->z || !hb->x0 || !hb->x1 || !hb->c || !hb->t0 || !hres->theta || !hres->chi2) return SB_EINVAL;
+    if (hb->n_obs_total > 0 && (!hb->time || !hb->band)) return SB_EINVAL;
+    if (hb->obs_offset[0] != 0 || hb->obs_offset[hb->n_sn] != hb->n_obs_total) return SB_EINVAL;
+    if (opts->trace_len > 0 && !hres->trace) return SB_EINVAL;
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return SB_ECUDA;
+    if (dev != m->device || dev != b->device) return SB_EINVAL;
+    const size_t es = base == SB_F32 ? 4 : 8;
+    const size_t nsn = (size_t)hb->n_sn, nob = (size_t)hb->n_obs_total, nun = nsn * (size_t)hb->n_samples;
+
+    // the whole batch stays resident for the fit: one staging slab of a host-call context of the handle
+    SbScratch *sc = b->scratch;
+    SbScratch::HostCtx *ctx = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(sc->mu);
+        for (auto *c : sc->host)
+            if (!c->busy) { ctx = c; break; }
+        if (!ctx) {
+            ctx = new (std::nothrow) SbScratch::HostCtx();
+            if (!ctx) return SB_ENOMEM;
+            memset(ctx, 0, sizeof(*ctx));
+            sc->host.push_back(ctx);
+        }
+        ctx->busy = true;
+    }
+    struct Release {
+        SbScratch *sc; SbScratch::HostCtx *c;
+        ~Release() { std::lock_guard<std::mutex> lock(sc->mu); c->busy = false; }
+    } release{sc, ctx};
+    if (!ctx->st[0] && !cuda_ok(cudaStreamCreateWithFlags(&ctx->st[0], cudaStreamNonBlocking))) return SB_ECUDA;
+    cudaStream_t st = ctx->st[0];
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t at = off; off += (bytes + 255) & ~(size_t)255; return at; };
+    const size_t o_off = take(4 * (nsn + 1)), o_band = take(4 * nob), o_time = take(es * nob), o_zp = take(hb->zp ? es * nob : 0),
+                 o_flux = take(es * nob), o_err = take(es * nob), o_z = take(es * nsn), o_x0 = take(es * nun), o_x1 = take(es * nun),
+                 o_c = take(es * nun), o_t0 = take(es * nun), r_theta = take(4 * es * nun), r_chi2 = take(es * nun),
+                 r_status = take(4 * nun), r_iter = take(4 * nun), r_eval = take(4 * nun),
+                 r_trace = take(8 * (size_t)opts->trace_len * nun);
+    if (off > ctx->fit_bytes) { // a free context has no work in flight: its slab can be regrown
+        if (ctx->fit_slab) cudaFree(ctx->fit_slab);
+        ctx->fit_slab = nullptr;
+        ctx->fit_bytes = 0;
+        if (!cuda_ok(cudaMalloc((void **)&ctx->fit_slab, off)))
+            return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+        ctx->fit_bytes = off;
+    }
+    unsigned char *D = ctx->fit_slab;
+    rc = SB_OK;
+    auto h2d = [&](size_t at, const void *src, size_t bytes) {
+        if (rc == SB_OK && bytes && !cuda_ok(cudaMemcpyAsync(D + at, src, bytes, cudaMemcpyHostToDevice, st))) rc = SB_ECUDA;
+    };
+    auto d2h = [&](void *dst, size_t at, size_t bytes) {
+        if (rc == SB_OK && dst && bytes && !cuda_ok(cudaMemcpyAsync(dst, D + at, bytes, cudaMemcpyDeviceToHost, st))) rc = SB_ECUDA;
+    };
+    h2d(o_off, hb->obs_offset, 4 * (nsn + 1)); h2d(o_band, hb->band, 4 * nob); h2d(o_time, hb->time, es * nob);
+    if (hb->zp) h2d(o_zp, hb->zp, es * nob);
+    h2d(o_flux, flux, es * nob); h2d(o_err, fluxerr, es * nob); h2d(o_z, hb->z, es * nsn);
+    h2d(o_x0, hb->x0, es * nun); h2d(o_x1, hb->x1, es * nun); h2d(o_c, hb->c, es * nun); h2d(o_t0, hb->t0, es * nun);
+    if (rc != SB_OK) return rc;
+    sb_batch db = *hb;
+    db.obs_offset = (const int32_t *)(D + o_off); db.band = (const int32_t *)(D + o_band); db.time = D + o_time;
+    db.zp = hb->zp ? D + o_zp : nullptr; db.z = D + o_z; db.x0 = D + o_x0; db.x1 = D + o_x1; db.c = D + o_c; db.t0 = D + o_t0;
+    sb_pack *pack = nullptr; // observations and redshifts are fixed over the fit: precompute once (fp32 fast path)
+    int32_t launches = 0;
+    if (base == SB_F32 && sb_pack_observations(m, b, &db, (void *)st, &pack) == SB_OK) { db.pack = pack; launches += tl_launches; }
+    sb_fit_result dres;
+    dres.theta = D + r_theta; dres.chi2 = D + r_chi2;
+    dres.status = (int32_t *)(D + r_status); dres.n_iter = (int32_t *)(D + r_iter); dres.n_eval = (int32_t *)(D + r_eval);
+    dres.trace = opts->trace_len > 0 ? (double *)(D + r_trace) : nullptr;
+    rc = fit_device(m, b, &db, D + o_flux, D + o_err, opts, &dres, st);
+    launches += tl_launches;
+    const int32_t form = tl_form;
+    d2h(hres->theta, r_theta, 4 * es * nun); d2h(hres->chi2, r_chi2, es * nun);
+    d2h(hres->status, r_status, 4 * nun); d2h(hres->n_iter, r_iter, 4 * nun); d2h(hres->n_eval, r_eval, 4 * nun);
+    if (opts->trace_len > 0) d2h(hres->trace, r_trace, 8 * (size_t)opts->trace_len * nun);
+    if (!cuda_ok(cudaStreamSynchronize(st)) && rc == SB_OK) rc = SB_ECUDA;
+    sb_free_pack(pack);
+    tl_launches = rc == SB_OK ? launches : 0;
+    tl_form = rc == SB_OK ? form : 0;
+    return rc;
 }
 
 } // extern "C"

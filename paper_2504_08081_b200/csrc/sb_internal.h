@@ -96,6 +96,7 @@ struct SbKParams {
     int32_t tile_cells;               // coefficient-row entries per warp buffer (multiple of 8)
     int32_t chunk_cap;                // evaluation records per chunk
     int32_t group_units;              // units per CTA group (<= 16)
+    const int32_t *n_live;            // fit driver: [1] 0 = nothing to do (or NULL)
 };
 
 // Kernel parameter block of the band-grouped kernel (sb_hoist.cuh), fp32 forward.

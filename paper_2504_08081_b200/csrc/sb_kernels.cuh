@@ -601,6 +601,7 @@ __global__ void __launch_bounds__(NWARPS * kWarpSize, 1) sb_fused_kernel(const _
     constexpr int NT = NWARPS * kWarpSize;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
+    if (P.n_live != nullptr && __ldg(P.n_live) == 0) return; // fit driver: every lane has stopped
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const SbModelParams &mp = P.mp;
     const int TC = P.tile_cells, CAP = P.chunk_cap, G = P.group_units;

@@ -138,6 +138,7 @@ struct SbNParams {
     float *out_dflux, *out_dchi2;     // gradient kernel only; may be NULL
     const int32_t *perm;              // z-ordered supernova indices (pack or workspace), or NULL
     const NItem *geom;                // [n_sn][n_bands] item geometry of the pack, or NULL (computed here)
+    const int32_t *live, *n_live;     // fit driver: [n_units] 0 = skip the unit; [1] 0 = nothing to do (or NULL)
     int32_t n_groups;                 // groups: unit range of group i = [i n_units / n_groups, (i+1) n_units / n_groups)
     int32_t cap;                      // observations per round
     int32_t mix;                      // which warps start a super-step with phase A (experiment knob)
@@ -664,6 +665,7 @@ __global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const 
     const uint32_t a_at = smem_addr(s_at), a_w = smem_addr(s_w);
     const NShared SA{smem_addr(s_info), smem_addr(s_ws), smem_addr(s_ws + CAP), smem_addr(s_x1), smem_addr(res), CAP};
 
+    if (P.n_live != nullptr && __ldg(P.n_live) == 0) return; // fit driver: every lane has stopped
     for (int i = tid; i < P.n_band_total; i += kThreads) s_w[i] = __ldg(P.band_w + i);
     const long long n_units = (long long)P.n_sn * P.n_samples;
     const long long n_groups = P.n_groups;
@@ -688,6 +690,7 @@ __global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const 
             t.unit = sn * P.n_samples + ks;
             t.o_lo = __ldg(P.obs_offset + sn);
             t.n = __ldg(P.obs_offset + sn + 1) - t.o_lo;
+            if (P.live != nullptr && __ldg(P.live + t.unit) == 0) t.n = 0; // stopped lane: nothing to evaluate
             t.z = __ldg(P.z + sn);
             t.x0 = __ldg(P.x0 + t.unit);
             t.x1 = __ldg(P.x1 + t.unit);
