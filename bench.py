@@ -131,7 +131,7 @@ def flops_per_call(wl, grad: bool, form: str = "direct"):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 20 ms while the timed region runs."""
 
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
@@ -143,7 +143,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -275,13 +275,157 @@ def run_reference(args):
     return 0
 
 
+def run_fit(args):
+    """--mode fit: the batched device-resident L-BFGS fit (sb_fit_lbfgs; PAPER.md:17 fmin_bfgs.py) on
+    BASELINE.json configs[3] (4096 supernovae x 100 observations, perturbed start).  A step = one whole fit of
+    every supernova: --fit-evals batched chi^2 + gradient evaluations and lane updates, no host sync.
+    e2e = sb_fit_lbfgs_host on pinned host buffers; the oracle optimiser (oracle/lbfgs.py) is timed beside it
+    on a bounded sample."""
+    import torch
+
+    import paper_2504_08081_b200 as sb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+    config = 4 if args.config == 5 else args.config
+    steps, warmup = max(min(args.steps, 50), 1), max(min(args.warmup, 5), 3)
+    wl = workloads.make_workload(config, seed_offset=rank)
+    md, bd = wl.model, wl.bands
+    model = sb.sb_load_model(md["phase"], md["wave"], md["m0"], md["m1"], md["cl_coef"], md["cl_wave_b"],
+                             md["cl_wave_v"], md["cl_lo"], md["cl_hi"])
+    bands = sb.sb_load_bandpasses(bd["offset"], bd["wave"], bd["trans"])
+    ft = torch.float32
+    n, n_tot = wl.n_sn, wl.n_obs_total
+
+    def pin(a, dtype):
+        return torch.as_tensor(np.ascontiguousarray(a)).to(dtype).pin_memory()
+
+    h = {"obs_offset": pin(wl.obs_offset, torch.int32), "time": pin(wl.time, ft), "band": pin(wl.band, torch.int32),
+         "zp": pin(wl.zp, ft), "z": pin(wl.z, ft)}
+    for k in ("x0", "x1", "c", "t0"):
+        h[k] = pin(wl.theta[k], ft)
+    d = {k: v.to(dev) for k, v in h.items()}
+    tt = {k: torch.as_tensor(wl.theta_true[k]).to(dev) for k in ("x0", "x1", "c", "t0")}
+    true_flux = torch.empty(n_tot, dtype=ft, device=dev)
+    sb.sb_bandflux(model, bands, dtype=sb.SB_F32, n_sn=n, n_samples=1, n_obs_total=n_tot, obs_offset=d["obs_offset"],
+                   time=d["time"], band=d["band"], zp=d["zp"], z=d["z"], out_flux=true_flux, **tt)
+    torch.cuda.synchronize()
+    workloads.attach_data(wl, true_flux.double().cpu().numpy())
+    h["flux"], h["fluxerr"] = pin(wl.flux, ft), pin(wl.fluxerr, ft)
+    d["flux"], d["fluxerr"] = h["flux"].to(dev), h["fluxerr"].to(dev)
+    pack = sb.sb_pack_observations(model, bands, dtype=sb.SB_F32, n_sn=n, z=d["z"])
+    opts = dict(max_eval=args.fit_evals, ftol=1e-7)
+    common = dict(dtype=sb.SB_F32, n_sn=n, n_samples=1, n_obs_total=n_tot)
+    o = dict(out_theta=torch.empty((n, 4), dtype=ft, device=dev), out_chi2=torch.empty(n, dtype=ft, device=dev),
+             out_status=torch.empty(n, dtype=torch.int32, device=dev), out_n_iter=torch.empty(n, dtype=torch.int32, device=dev),
+             out_n_eval=torch.empty(n, dtype=torch.int32, device=dev))
+    ho = {k: torch.empty_like(v, device="cpu").pin_memory() for k, v in o.items()}
+    launches = [0]
+
+    def step():
+        sb.sb_fit_lbfgs(model, bands, **d, **o, pack=pack, **common, **opts)
+        launches[0] = sb.last_launch_count()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        a.record()
+        step()
+        b.record()
+    barrier()
+    clocks = sampler.stop()
+    total_ms = float(sum(a.elapsed_time(b) for a, b in ev))
+    if dist is not None:
+        tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        total_ms = float(tmax.item())
+    ms_per_step = total_ms / steps
+    n_eval = o["out_n_eval"].cpu().numpy().astype(np.int64)
+    status = o["out_status"].cpu().numpy()
+    chi2 = o["out_chi2"].double().cpu().numpy()
+    e2e_steps = min(steps, 10)
+    for _ in range(2):
+        sb.sb_fit_lbfgs_host(model, bands, **h, **ho, **common, **opts)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sb.sb_fit_lbfgs_host(model, bands, **h, **ho, **common, **opts)
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    if dist is not None:
+        tmax = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        e2e_ms = float(tmax.item())
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        from oracle import lbfgs
+
+        k = 24  # bounded sample: the first 24 supernovae, one lane at a time on one host core
+        sub = oracle_sample(wl, k)
+        true = oracle.run_workload(sub, theta={k_: v.copy() for k_, v in sub.theta_true.items()})["flux"]
+        workloads.attach_data(sub, true)
+        t0 = time.perf_counter()
+        ref = lbfgs.fit_workload(sub, round_theta_to=np.float32, **opts)
+        sec = time.perf_counter() - t0
+        cpu = {"value": k / sec, "unit": "fits/s", "cores": 1, "kind": "oracle (oracle/lbfgs.py over the fp64 oracle)",
+               "sample": f"first {k} of {wl.n_sn} supernovae of {wl.name}", "seconds": sec,
+               "evaluations_per_sec": float(ref["n_eval"].sum()) / sec, "mean_n_eval": float(ref["n_eval"].mean())}
+    in_bytes = sum(v.numel() * v.element_size() for v in h.values())
+    out_bytes = sum(v.numel() * v.element_size() for v in ho.values())
+    line = {
+        "metric": "lbfgs_fits_per_sec", "value": n * world / (ms_per_step * 1e-3), "unit": "fits/s", "n_gpus": world,
+        "steps": steps, "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32 evaluations, f64 optimiser state", "data": "synthetic",
+        "config": {"workload": wl.name, "n_sn": n, "n_obs_total": n_tot, "mode": "fit", "max_eval": args.fit_evals,
+                   "ftol": opts["ftol"], "memory": 8, "pack": True,
+                   "evaluations_per_sec": float(n_eval.sum()) * world / (ms_per_step * 1e-3),
+                   "bandflux_grad_evals_per_sec": float((n_eval * np.diff(wl.obs_offset)).sum()) * world / (ms_per_step * 1e-3),
+                   "mean_n_eval": float(n_eval.mean()), "converged_frac": float(np.mean(status == 1)),
+                   "median_chi2": float(np.median(chi2)), "parallelism": f"dp{world} (independent shards)"},
+        "e2e": {"value": n * world / (e2e_ms * 1e-3), "unit": "fits/s", "h2d_bytes_per_step": in_bytes,
+                "d2h_bytes_per_step": out_bytes, "ms_per_step": e2e_ms, "steps": e2e_steps, "call": "sb_fit_lbfgs_host"},
+        "gpu_launches": launches[0] * steps, "clocks": clocks, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
-    ap.add_argument("--mode", default="chi2", choices=["chi2", "grad"])
+    ap.add_argument("--mode", default="chi2", choices=["chi2", "grad", "fit"],
+                    help="chi2: sb_chi2 (default); grad: sb_bandflux_grad; fit: sb_fit_lbfgs (batched L-BFGS, config 4 shape)")
+    ap.add_argument("--pack", action="store_true",
+                    help="time the calls with an sb_pack_observations pack (built once, outside the timed region)")
+    ap.add_argument("--fit-evals", type=int, default=40, help="--mode fit: evaluations (steps) per lane")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--form", default="auto", choices=["auto", "direct", "grouped", "tiled"],
                     help="formulation (include/saltband.h SB_FORM_*): auto = the library's choice")
@@ -291,6 +435,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.mode == "fit":
+        return run_fit(args)
 
     import torch
 
@@ -342,6 +488,11 @@ def main():
     h["flux"], h["fluxerr"] = pin(wl.flux, ft), pin(wl.fluxerr, ft)
     d["flux"], d["fluxerr"] = h["flux"].to(dev), h["fluxerr"].to(dev)
 
+    # optional pack (include/saltband.h: sb_pack_observations): z order and item geometry, built once
+    pack = sb.sb_pack_observations(model, bands, dtype=sb.SB_F32, n_sn=wl.n_sn, z=d["z"])
+    torch.cuda.synchronize()
+    use_pack = [bool(args.pack)]
+
     o_flux = torch.empty(n_ev, dtype=ft, device=dev)
     o_chi = torch.empty(n_units, dtype=ft, device=dev)
     o_dflux = torch.empty(n_ev * 4, dtype=ft, device=dev) if grad else None
@@ -350,15 +501,16 @@ def main():
     form_ran = [""]
 
     def step(t):
+        pk = pack if use_pack[0] else None
         if grad:
             sb.sb_bandflux_grad(model, bands, obs_offset=t["obs_offset"], time=t["time"], band=t["band"], zp=t["zp"],
                                 z=t["z"], x0=t["x0"], x1=t["x1"], c=t["c"], t0=t["t0"], flux=t["flux"],
                                 fluxerr=t["fluxerr"], out_flux=o_flux, out_dflux=o_dflux, out_chi2=o_chi,
-                                out_dchi2=o_dchi, **common)
+                                out_dchi2=o_dchi, pack=pk, **common)
         else:
             sb.sb_chi2(model, bands, obs_offset=t["obs_offset"], time=t["time"], band=t["band"], zp=t["zp"], z=t["z"],
                        x0=t["x0"], x1=t["x1"], c=t["c"], t0=t["t0"], flux=t["flux"], fluxerr=t["fluxerr"],
-                       out_chi2=o_chi, out_flux=o_flux, **common)
+                       out_chi2=o_chi, out_flux=o_flux, pack=pk, **common)
         launches_per_step[0] = sb.last_launch_count()
         form_ran[0] = sb.last_form()
 
@@ -398,6 +550,28 @@ def main():
         total_ms = float(tmax.item())
     ms_per_step = total_ms / steps
     value = n_ev * world * steps / (total_ms * 1e-3)
+    launches_timed = launches_per_step[0]
+
+    # ---- the same call with a pack (or without, if --pack): observations and redshifts are static over the
+    # thousands of calls of a fit or a sampling run, so the theta-independent work can be
+    # done once; reported beside the headline value, which times everything a bare call launches
+    use_pack[0] = not use_pack[0]
+    alt_steps = min(steps, 50)
+    for _ in range(3):
+        step(d)
+    barrier()
+    ev2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(alt_steps)]
+    for a, b in ev2:
+        if need_flush:
+            flush_buf.fill_(1)
+        a.record()
+        step(d)
+        b.record()
+    barrier()
+    alt_ms = float(np.mean([a.elapsed_time(b) for a, b in ev2]))
+    alt = {"pack": use_pack[0], "ms_per_step": alt_ms, "value": n_ev / (alt_ms * 1e-3), "steps": alt_steps,
+           "gpu_launches_per_step": launches_per_step[0], "note": "this rank only"}
+    use_pack[0] = not use_pack[0]
 
     # ---- end to end: the host-buffer C-ABI call (sb_chi2_host / sb_bandflux_grad_host) on pinned host
     # inputs and outputs: every step copies all inputs host -> device and all results device -> host
@@ -451,12 +625,22 @@ def main():
         peak_src = "measured: FFMA-chain microbenchmark (csrc/sb_probe.cu) in this run"
     except Exception as exc:  # pragma: no cover
         peak_tf, peak_src = 148 * 128 * 2 * 1.965e9 * 1e-12, f"nominal 148 SM x 128 lanes x 2 x 1.965 GHz ({exc})"
-    achieved = flops_ours / (kernel_ms * 1e-3) * 1e-12
+    model_tf = flops_ours / (kernel_ms * 1e-3) * 1e-12
     algo_bytes = in_bytes + out_bytes
+    # fraction = min(A, B) / peak, A = executed-model flops (above), B = FP32 flops
+    # counted by ncu for one launch of this kernel on this workload (SASS opcode table of the committed
+    # `ncu --set full` capture, profiles/traffic.json; packed FFMA2/FMUL2/FADD2 count twice) over the time
+    # measured here.  B guards against an inflated model, A against counting padded or repeated work.
+    cap = _ncu_capture(form_run, grad, wl.name)
+    counted = cap.get("counted_fp32_flop")
+    counted_tf = counted / (kernel_ms * 1e-3) * 1e-12 if counted else None
+    achieved = min(model_tf, counted_tf) if counted_tf else model_tf
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
-        "traffic": _ncu_traffic(form_run, grad, wl.name),
-        "kernel": {"grouped": "sb_hoist_kernel<fwd>", "tiled": "sb_tiled_kernel<%s>" % ("grad" if grad else "fwd")}.get(
+        "model": model_tf, "counted": counted_tf, "counted_flop_per_launch": counted,
+        "counted_source": cap.get("source"),
+        "traffic": cap.get("dram_bytes"),
+        "kernel": {"grouped": "sb_hoist_kernel<fwd>", "tiled": "sb_nw_kernel<%s>" % ("grad" if grad else "fwd")}.get(
             form_run, "sb_fused_kernel<float,%s>" % ("grad" if grad else "fwd")),
         "form": form_run,
         "kernel_ms": kernel_ms, "flops_per_eval": flops_ours / n_ev, "peak_source": peak_src,
@@ -466,8 +650,9 @@ def main():
                                 "observations per (unit, band)"}.get(
             form_run, "executed formulation (DESIGN.md): G_geom = G_col = 1"),
         "survey_direct_model": {"flops_per_eval": flops_survey / n_ev,
-                                "achieved": flops_survey / (kernel_ms * 1e-3) * 1e-12,
-                                "frac": flops_survey / (kernel_ms * 1e-3) * 1e-12 / peak_tf},
+                                "evals_per_sec_at_half_peak": 0.5 * peak_tf * 1e12 / (flops_survey / n_ev),
+                                "note": "SURVEY.md 8(d) G = 1 model: a rate target for context (BASELINE.md section 3), "
+                                        "not work this kernel executes"},
         "mean_in_range_samples": mean_in, "mean_cells": mean_cell,
         "hbm": {"algorithmic_bytes": algo_bytes, "achieved_gbs": algo_bytes / (kernel_ms * 1e-3) * 1e-9,
                 "peak_gbs": _measured_peaks().get("hbm_gbs"),
@@ -484,14 +669,14 @@ def main():
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": wl.name, "n_sn": wl.n_sn, "n_samples": ns, "n_obs_total": n_tot, "n_evals": n_ev,
-                   "mode": args.mode, "form": form_run, "chi2_evals_per_sec": n_units * world * steps / (total_ms * 1e-3),
+                   "mode": args.mode, "form": form_run, "pack": bool(args.pack), "chi2_evals_per_sec": n_units * world * steps / (total_ms * 1e-3),
                    "l2": "inputs+outputs %.0f MB > 126 MB L2, no flush" % ((in_bytes + out_bytes) / 1e6) if not need_flush
                    else "L2 flushed (256 MB write) between timed steps", "parallelism": f"dp{world} (independent shards)"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps,
                 "call": "sb_bandflux_grad_host" if grad else "sb_chi2_host"},
-        "gpu_launches": launches_per_step[0] * steps, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-        "wall_s_timed_region": wall,
+        "gpu_launches": launches_timed * steps, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+        "with_pack" if not args.pack else "without_pack": alt, "wall_s_timed_region": wall,
     }
     print(json.dumps(line))
     if dist is not None:
@@ -499,17 +684,18 @@ def main():
     return 0
 
 
-def _ncu_traffic(form: str, grad: bool, workload: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the step's main kernel, copied from
-    the `ncu --set full` capture summarised under profiles/ (profiles/traffic.json); None if this
-    (formulation, mode, workload) has not been captured."""
+def _ncu_capture(form: str, grad: bool, workload: str) -> dict:
+    """Per-launch figures of the step's main kernel copied from the `ncu --set full` capture summarised
+    under profiles/ (profiles/traffic.json): dram_bytes = dram__bytes_read.sum + dram__bytes_write.sum,
+    counted_fp32_flop = FP32 flops from the SASS opcode table.  {} if this (formulation, mode, workload)
+    has not been captured."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
             tab = json.load(fh)
     except (OSError, ValueError):
-        return None
+        return {}
     ent = tab.get(f"{form}:{'grad' if grad else 'fwd'}:{workload}")
-    return ent.get("dram_bytes") if isinstance(ent, dict) else None
+    return ent if isinstance(ent, dict) else {}
 
 
 def _measured_peaks():
