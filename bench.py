@@ -425,6 +425,8 @@ def main():
                     help="chi2: sb_chi2 (default); grad: sb_bandflux_grad; fit: sb_fit_lbfgs (batched L-BFGS, config 4 shape)")
     ap.add_argument("--pack", action="store_true",
                     help="time the calls with an sb_pack_observations pack (built once, outside the timed region)")
+    ap.add_argument("--band-jitter", type=float, default=0.0,
+                    help="non-uniform band grids: interior grid points moved by U(-j, j) x step (workloads.jitter_band_grids)")
     ap.add_argument("--fit-evals", type=int, default=40, help="--mode fit: evaluations (steps) per lane")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--form", default="auto", choices=["auto", "direct", "grouped", "tiled"],
@@ -458,7 +460,7 @@ def main():
     grad = args.mode == "grad"
 
     # ---- workload shard of this rank (weak scaling: one full config per GPU)
-    wl = workloads.make_workload(args.config, seed_offset=rank)
+    wl = workloads.make_workload(args.config, seed_offset=rank, band_jitter=args.band_jitter)
     md, bd = wl.model, wl.bands
     model = sb.sb_load_model(md["phase"], md["wave"], md["m0"], md["m1"], md["cl_coef"], md["cl_wave_b"],
                              md["cl_wave_v"], md["cl_lo"], md["cl_hi"])
@@ -669,7 +671,7 @@ def main():
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": wl.name, "n_sn": wl.n_sn, "n_samples": ns, "n_obs_total": n_tot, "n_evals": n_ev,
-                   "mode": args.mode, "form": form_run, "pack": bool(args.pack), "chi2_evals_per_sec": n_units * world * steps / (total_ms * 1e-3),
+                   "mode": args.mode, "form": form_run, "pack": bool(args.pack), "band_jitter": args.band_jitter, "chi2_evals_per_sec": n_units * world * steps / (total_ms * 1e-3),
                    "l2": "inputs+outputs %.0f MB > 126 MB L2, no flush" % ((in_bytes + out_bytes) / 1e6) if not need_flush
                    else "L2 flushed (256 MB write) between timed steps", "parallelism": f"dp{world} (independent shards)"},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": d2h,

@@ -15,7 +15,8 @@ SB_F32, SB_F64 = 0, 1
 SB_FORM_DIRECT, SB_FORM_GROUPED, SB_FORM_TILED = 0x100, 0x200, 0x400  # optional formulation bits OR-ed into dtype
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_PKG, "libsaltband.so")
+# SALTBAND_LIB=checked loads the bounds-checked build of the same sources (build.py --checked)
+_LIB_PATH = os.path.join(_PKG, "libsaltband_checked.so" if os.environ.get("SALTBAND_LIB") == "checked" else "libsaltband.so")
 
 
 class SaltbandError(RuntimeError):

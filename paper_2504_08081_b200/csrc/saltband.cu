@@ -309,16 +309,19 @@ int sb_load_bandpasses(int32_t n_bands, const int64_t *offset, const double *wav
         for (int64_t j = 0; j < n; ++j)
             if (std::fabs(lam[j] - (lam[0] + (double)j * hstep[b])) > 1e-9 * lam[j]) h->all_uniform = 0;
     }
-    std::vector<float2> tab_f((size_t)total);
+    std::vector<float2> tab_f((size_t)total), wd_f((size_t)total);
     std::vector<double2> tab_d((size_t)total);
     for (int64_t i = 0; i < total; ++i) {
         tab_d[i] = make_double2(dlam[i], w[i]);
         tab_f[i] = make_float2((float)dlam[i], (float)w[i]);
     }
+    for (int b = 0; b < n_bands; ++b) // offset of every sample from the band's mean-step grid (0 on uniform grids)
+        for (int64_t i = offset[b]; i < offset[b + 1]; ++i)
+            wd_f[i] = make_float2((float)w[i], (float)(dlam[i] - (double)(i - offset[b]) * hstep[b]));
     cudaGetDevice(&h->device);
     if (!upload(&h->d_off, off) || !upload(&h->d_lam_first, lam_first) || !upload(&h->d_zpab_inv, zpab_inv) ||
         !upload(&h->d_tab_f64, tab_d) || !upload(&h->d_tab_f32, tab_f) || !upload(&h->d_w_f32, w_f) ||
-        !upload(&h->d_dlam_f64, dlam) || !upload(&h->d_h, hstep)) {
+        !upload(&h->d_dlam_f64, dlam) || !upload(&h->d_h, hstep) || !upload(&h->d_wd_f32, wd_f)) {
         sb_free_bands(h);
         return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
     }
@@ -335,6 +338,7 @@ void sb_free_bands(sb_bands *b)
     cudaFree(b->d_tab_f32);
     cudaFree(b->d_tab_f64);
     cudaFree(b->d_w_f32);
+    cudaFree(b->d_wd_f32);
     cudaFree(b->d_dlam_f64);
     cudaFree(b->d_h);
     free(b->h_zpab);
@@ -533,12 +537,12 @@ int launch_hoist(const sb_model *m, const sb_bands *b, const sb_batch *bt, const
 // is left.
 struct RunLive { const int32_t *live = nullptr, *n_live = nullptr; };
 
-template <int NCL, bool GRAD, int NW>
+template <int NCL, bool GRAD, bool NU>
 int launch_nw_inst(const sb_model *m, const sbn::SbNParams &np, size_t smem, int grid, cudaStream_t st)
 {
-    auto kern = sbn::sb_nw_kernel<NCL, GRAD, NW>;
+    auto kern = sbn::sb_nw_kernel<NCL, GRAD, NU>;
     if (!allow_max_smem((const void *)kern, m->device, m->smem_optin)) return SB_ECUDA;
-    kern<<<grid, NW * 32, smem, st>>>(np);
+    kern<<<grid, 16 * 32, smem, st>>>(np);
     if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
     tl_launches += 1;
     tl_form = SB_FORM_TILED;
@@ -553,27 +557,20 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
               const void *fluxerr, void *out_flux, void *out_chi2, void *out_dflux, void *out_dchi2, cudaStream_t st,
               const RunLive &lv)
 {
-    if (!b->all_uniform || m->prm.n_cl > SB_MAX_CL || b->n_bands > sbn::kMaxBands) return 1;
+    if (m->prm.n_cl > SB_MAX_CL || b->n_bands > sbn::kMaxBands) return 1;
     if (m->prm.n_phase < 4 || m->prm.n_phase > 4096) return 1;
     const int smem_max = m->smem_optin, n_sm = m->n_sm;
     const long long n_units = (long long)bt->n_sn * bt->n_samples;
     const double mean_obs = bt->n_sn > 0 ? (double)bt->n_obs_total / (double)bt->n_sn : 1.0;
-    // CTA shape: two CTAs of 8 warps per SM when their shared memory fits twice (1 KB per CTA is reserved)
-    static const int want_two = [] { const char *e = getenv("SB_NW_CTAS"); return e ? atoi(e) : 1; }();
-    int nw = want_two == 2 ? 8 : 16;
-    int nsl = 0, cap = 0;
-    for (;;) {
-        nsl = grad ? nw : 2 * nw;
-        cap = nw == 16 ? (grad ? sbn::Cfg<16>::kCapGrad : sbn::Cfg<16>::kCapFwd) : (grad ? sbn::Cfg<8>::kCapGrad : sbn::Cfg<8>::kCapFwd);
-        const size_t limit = nw == 16 ? (size_t)smem_max : (size_t)(smem_max + 1024) / 2 - 1024;
-        const int cap_min = nw == 16 ? 512 : (grad ? 384 : 768);
-        while (cap >= cap_min && sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl, nw).total > limit) cap -= 128;
-        if (cap >= cap_min) break;
-        if (nw == 8) { nw = 16; continue; } // does not fit twice: one CTA per SM
-        return 1;
-    }
-    const size_t smem = sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl, nw).total;
-    const int n_cta = nw == 16 ? n_sm : 2 * n_sm; // resident CTAs
+    const bool nu = !b->all_uniform; // non-uniform band grids: the kernel variant that reads {W_j, delta_j}
+    // one CTA of 16 warps per SM; observations per round: as many as fit beside the band tables
+    constexpr int nw = 16;
+    const int nsl = grad ? nw : 2 * nw;
+    int cap = grad ? sbn::Cfg<16>::kCapGrad : sbn::Cfg<16>::kCapFwd;
+    while (cap >= 512 && sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl, nw, nu).total > (size_t)smem_max) cap -= 128;
+    if (cap < 512) return 1;
+    const size_t smem = sbn::NSmem(b->n_total, cap, grad, b->n_bands * nsl, nw, nu).total;
+    const int n_cta = n_sm; // resident CTAs
     // groups: whole waves of n_sm groups of at most g_target units (even split of the z-ordered units),
     // g_target = as many units as fit the item slots and the round's observation capacity
     long long g_target = (long long)((double)cap / (mean_obs > 1.0 ? mean_obs : 1.0));
@@ -613,6 +610,7 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     np.band_h = b->d_h;
     np.band_dlam = b->d_dlam_f64;
     np.band_w = b->d_w_f32;
+    np.band_wd = b->d_wd_f32;
     np.n_sn = bt->n_sn;
     np.n_samples = bt->n_samples;
     np.obs_offset = bt->obs_offset;
@@ -639,12 +637,12 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     { const char *e = getenv("SB_NW_MIX"); np.mix = e ? atoi(e) : 2; }
     const int grid = (int)(n_groups < (long long)n_cta ? n_groups : (long long)n_cta);
     const bool small_cl = m->prm.n_cl <= 5;
-    if (nw == 16) {
-        if (grad) return small_cl ? launch_nw_inst<5, true, 16>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, true, 16>(m, np, smem, grid, st);
-        return small_cl ? launch_nw_inst<5, false, 16>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, false, 16>(m, np, smem, grid, st);
+    if (nu) {
+        if (grad) return small_cl ? launch_nw_inst<5, true, true>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, true, true>(m, np, smem, grid, st);
+        return small_cl ? launch_nw_inst<5, false, true>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, false, true>(m, np, smem, grid, st);
     }
-    if (grad) return small_cl ? launch_nw_inst<5, true, 8>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, true, 8>(m, np, smem, grid, st);
-    return small_cl ? launch_nw_inst<5, false, 8>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, false, 8>(m, np, smem, grid, st);
+    if (grad) return small_cl ? launch_nw_inst<5, true, false>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, true, false>(m, np, smem, grid, st);
+    return small_cl ? launch_nw_inst<5, false, false>(m, np, smem, grid, st) : launch_nw_inst<SB_MAX_CL, false, false>(m, np, smem, grid, st);
 }
 
 int run(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, const void *flux, const void *fluxerr,
@@ -736,7 +734,7 @@ int sb_pack_observations(const sb_model *m, const sb_bands *b, const sb_batch *b
     if (out) *out = nullptr;
     if (!m || !b || !bt || !out) return SB_EINVAL;
     if ((bt->dtype & 0xff) != SB_F32 || bt->n_sn < 1 || !bt->z) return SB_EINVAL;
-    if (b->n_bands > sbn::kMaxBands || !b->all_uniform) return SB_ELIMIT; // the kernels that use a pack do not apply
+    if (b->n_bands > sbn::kMaxBands) return SB_ELIMIT; // the kernel that uses a pack does not apply
     int dev = -1;
     if (!cuda_ok(cudaGetDevice(&dev))) return SB_ECUDA;
     if (dev != m->device || dev != b->device) return SB_EINVAL;
@@ -762,7 +760,7 @@ int sb_pack_observations(const sb_model *m, const sb_bands *b, const sb_batch *b
     int rc = enqueue_zorder((const float *)bt->z, bt->n_sn, h->d_ws, st, &launches);
     if (rc == SB_OK) {
         const long long n_items = (long long)bt->n_sn * b->n_bands;
-        const sbn::NBandsView bv{b->n_bands, b->d_off, b->d_lam_first, b->d_h, b->d_dlam_f64};
+        const sbn::NBandsView bv{b->n_bands, b->all_uniform, b->d_off, b->d_lam_first, b->d_h, b->d_dlam_f64};
         sbn::sb_geom_kernel<<<(unsigned)((n_items + 255) / 256), 256, 0, st>>>(m->prm, bv, (const float *)bt->z, bt->n_sn,
                                                                              reinterpret_cast<sbn::NItem *>(h->d_geom));
         if (!cuda_ok(cudaGetLastError())) rc = SB_ECUDA;

@@ -61,8 +61,9 @@ struct sb_bands {
     // band-grouped kernel (sb_hoist.cuh): only when every band grid is uniform
     int32_t all_uniform;   // 1 when |lam_j - (lam_first + j h_b)| <= 1e-9 lam_j for every band
     float *d_w_f32;        // [n_total] folded weights
+    float2 *d_wd_f32;      // [n_total] {folded weight, lam_j - (lam_first + j h_b)}: node-weight kernel, non-uniform grids
     double *d_dlam_f64;    // [n_total] lam_j - lam_first
-    double *d_h;           // [n_bands] uniform step h_b
+    double *d_h;           // [n_bands] mean step h_b = (lam_last - lam_first)/(n - 1) (the step, when the grid is uniform)
     int device;
     SbScratch *scratch;    // owned; the only mutable part of the handle (a cache, guarded by its mutex)
 };

@@ -30,12 +30,26 @@
 //   epilogue  per unit in fp64: zero point, coalesced stores, chi^2 (and d chi^2) in a fixed order.
 // The gradient variant (GRAD) adds CL-weighted node weights (d/dc), the M1-only sums (d/dx1) and the
 // phase-derivative row weights (d/dt0).
-// Requirements (checked by the host, otherwise sb_kernels.cuh runs): fp32, uniform band grids, n_phase in
-// [4, 4096], n_cl <= NCL, n_bands <= 64.
+// Band grids need not be uniform (tabulated filters): the NU variant of the kernel reads, beside
+// the folded weight W_j of a band sample, its offset delta_j = lambda_j - (lambda_first + j h) from the band's
+// mean-step grid, so that the position inside the model cell and the colour-law argument are those of the true
+// wavelength; which samples belong to a model cell is found by a local search from the uniform-grid guess.
+// Requirements (checked by the host, otherwise sb_kernels.cuh runs): fp32, n_phase in [4, 4096], n_cl <= NCL,
+// n_bands <= 64.
 #pragma once
 #include "sb_internal.h"
 #include "sb_kernels.cuh"
 #include "sb_hoist.cuh"
+
+// Checked build (python -m paper_2504_08081_b200.build --checked, -DSB_CHECKED): every shared-memory index
+// computed below is compared with the bound of its array and the kernel traps on a violation (the next
+// CUDA call then fails: SB_ECUDA).  Stands in for compute-sanitizer, which this GPU pool does not allow
+// (profiles/r2_sanitizer.md).  Compiles to nothing in the product build.
+#ifdef SB_CHECKED
+#define SB_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define SB_CHECK(cond) do { } while (0)
+#endif
 
 namespace sbn {
 
@@ -69,8 +83,8 @@ struct __align__(16) NItem {
     int32_t n_lo;    // first node that carries a weight (g_first - 1, >= -1)
     int32_t n_end;   // one past the last node that carries a weight (g_last + 3)
     int32_t pad_;
-    float c0, ha_hi, ha_lo, inv_ha; // u of the first sample minus g_first; cells per band sample (split), inverse
-    float hal, r_first;             // reduced-wavelength step per sample, value at the first sample
+    float c0, ha_hi, ha_lo, inv_ha; // u of the first sample ON THE MEAN-STEP GRID minus g_first; cells per (mean) band step (split), inverse
+    float hal, r_first;             // reduced-wavelength step per (mean) band step, value at the first sample of the mean-step grid
     float lin_a, lin_b;             // CM_LINEAR: CL = lin_a + lin_b r (unscaled)
 };
 static_assert(sizeof(NItem) == 64, "NItem is loaded as four float4");
@@ -94,7 +108,7 @@ struct NUnit {           // per unit of the group (all rounds)
 
 struct NSmem {
     size_t at, ws, res, info, w, hist, wsum, bstart, segs, units, items, win, x1, slot_tab, misc, carry, total;
-    __host__ __device__ NSmem(int n_band_total, int cap, bool grad, int n_items, int nw)
+    __host__ __device__ NSmem(int n_band_total, int cap, bool grad, int n_items, int nw, bool nu)
     {
         const int kSlots = 2 * nw, kWarps = nw, kMaxSeg = 2 * nw, kBins = nw == 16 ? 2048 : 1024;
         size_t o = 0;
@@ -102,7 +116,7 @@ struct NSmem {
         ws = o; o += (size_t)cap * sizeof(float4) * (grad ? 2 : 1);
         res = o; o += (size_t)cap * sizeof(float) * (grad ? 4 : 1);
         info = o; o += (size_t)cap * sizeof(uint32_t);
-        w = o; o += (size_t)((n_band_total + 3) & ~3) * sizeof(float);
+        w = o; o += (size_t)((n_band_total + 3) & ~3) * (nu ? sizeof(float2) : sizeof(float)); // W_j or {W_j, delta_j}
         hist = o; o += (size_t)kBins * sizeof(int32_t);
         wsum = o; o += (size_t)kWarps * sizeof(int32_t);
         bstart = o; o += (size_t)(kMaxBands + 4) * sizeof(int32_t);
@@ -128,7 +142,8 @@ struct SbNParams {
     int32_t n_bands, n_band_total;
     const int32_t *band_off;
     const double *band_lam_first, *band_zpab_inv, *band_h, *band_dlam;
-    const float *band_w;
+    const float *band_w;              // [n_band_total] folded weights W_j
+    const float2 *band_wd;            // [n_band_total] {W_j, delta_j} (NU kernels)
     int32_t n_sn, n_samples;
     const int32_t *obs_offset;
     const float *time, *zp, *z, *x0, *x1, *c, *t0;
@@ -178,6 +193,7 @@ __device__ __forceinline__ void sts32(uint32_t a, float v) { asm volatile("st.sh
 struct NShared { // shared-state-space addresses of the arrays phase B reads
     uint32_t info, ws, wd, x1, res;
     int32_t cap;
+    int32_t n_slots; // item slots per node-weight buffer (checked build)
 };
 
 // Colour-law modes of an item beyond sb::CM_*: the item's samples cross only ONE end of [cl_lo, cl_hi]
@@ -204,7 +220,7 @@ template <int NCL, int CM> __device__ __forceinline__ float2 colour_arg2(const H
 // ---- geometry of one item (redshift z, band b): one thread.  The in-range sample range [j_lo, j_hi) is
 // decided in fp64 (reading G9), then the window of model cells and the colour-law mode.
 struct NBandsView {
-    int32_t n_bands;
+    int32_t n_bands, all_uniform;
     const int32_t *band_off;
     const double *band_lam_first, *band_h, *band_dlam;
 };
@@ -233,24 +249,26 @@ __device__ __forceinline__ void item_geometry(const SbModelParams &mp, const NBa
     const double a_d = inv_opz / mp.dl;                      // cells per observer-frame Angstrom
     const double ub = (lam_first * inv_opz - mp.l0) / mp.dl; // u of dlam = 0
     const double ha = h * a_d;                               // cells per band sample
-    const double u_lo = (double)j_lo * ha + ub;
-    const double u_hi = (double)(j_hi - 1) * ha + ub;
+    // first and last in-range sample at their true wavelengths (the mean-step grid differs on non-uniform grids)
+    const double u_lo = __ldg(dlam + j_lo) * a_d + ub;
+    const double u_hi = __ldg(dlam + j_hi - 1) * a_d + ub;
     const int g_first = min(max((int)floor(u_lo), 0), nW - 2);
     const int g_last = min(max((int)floor(u_hi), 0), nW - 2);
     I.n_in = j_hi - j_lo;
     I.g_first = g_first;
     I.ncell = g_last - g_first + 1;
     I.wbase = boff + j_lo;
-    I.c0 = (float)(u_lo - (double)g_first);
+    I.c0 = (float)((double)j_lo * ha + ub - (double)g_first);
+    if (B.all_uniform) I.c0 = fmaxf(I.c0, 0.f); // uniform grid: the mean-step grid IS the grid (up to rounding of the table)
     I.ha_hi = (float)ha;
     I.ha_lo = (float)(ha - (double)I.ha_hi);
     I.inv_ha = (float)(1.0 / ha);
     const double al_d = inv_opz * mp.cl_inv_span;
     const double be_d = (lam_first * inv_opz - mp.cl_b) * mp.cl_inv_span;
     const double hal = h * al_d;
-    const double r_a = (double)j_lo * hal + be_d, r_b = (double)(j_hi - 1) * hal + be_d;
+    const double r_a = __ldg(dlam + j_lo) * al_d + be_d, r_b = __ldg(dlam + j_hi - 1) * al_d + be_d;
     I.hal = (float)hal;
-    I.r_first = (float)r_a;
+    I.r_first = (float)((double)j_lo * hal + be_d);
     const double r_min = fmin(r_a, r_b), r_max = fmax(r_a, r_b);
     const double margin = 1e-4;
     int cmode = sb::CM_GENERIC;
@@ -281,7 +299,7 @@ __device__ __forceinline__ void item_geometry(const SbModelParams &mp, const NBa
 // The loop walks TWO passes (cells gq and gq + 32 of the lane) per iteration as packed FP32 pairs.
 // GRAD: the colour law is evaluated unscaled (CL itself; exponent = CL * c log2(e)) and a second set of
 // moments, weighted by CL, gives the node weights of d/dc (at_slot + kSlotW).
-template <int NCL, int CM, bool GRAD>
+template <int NCL, int CM, bool GRAD, bool NU>
 __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NSeg &S, const NItem &I, int w_lo,
                                                int q_start, int q_a, int q_b, int q_lo, uint32_t a_w,
                                                uint32_t at_slot, int lane)
@@ -301,17 +319,32 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
     const float c0 = I.c0, inv_ha = I.inv_ha, ha_hi = I.ha_hi, ha_lo = I.ha_lo, hal = I.hal, r_first = I.r_first;
     const int n_in = I.n_in, ncell = I.ncell;
     const float nc0 = -c0 * inv_ha;
+    constexpr uint32_t WS = NU ? 8u : 4u; // bytes per entry of the staged band table: W_j or {W_j, delta_j}
+    const uint32_t wbase = a_w + (uint32_t)I.wbase * WS;
+    // NU: cells and reduced wavelength per Angstrom (observer frame) of this unit
+    const float acell = NU ? (float)(S.inv_opz / mp.dl) : 0.f, alr = NU ? (float)(S.inv_opz * mp.cl_inv_span) : 0.f;
     auto jstart = [&](int x) { // first band sample (relative to the first in-range one) of cell x
         int j = (int)ceilf(__fmaf_rn((float)x, inv_ha, nc0));
-        j = min(max(j, 0), n_in); // x <= 0 gives j <= 0 because c0 >= 0
+        j = min(max(j, 0), n_in); // uniform grids: x <= 0 gives j <= 0 because c0 >= 0
         if (x >= ncell) j = n_in;
+        if constexpr (NU) { // local search from the mean-step guess: u_k = c0 + k ha + delta_k acell against x
+            if (x <= 0) j = 0;
+            if (x > 0 && x < ncell) {
+                const float xf = (float)x - c0;
+                auto uk = [&](int k) {
+                    const float kf = (float)k;
+                    return __fmaf_rn(kf, ha_hi, __fmaf_rn(kf, ha_lo, lds64(wbase + (uint32_t)k * 8u).y * acell));
+                };
+                while (j > 0 && uk(j - 1) >= xf) --j;
+                while (j < n_in && uk(j) < xf) ++j;
+            }
+        }
         return j;
     };
     float pa0 = 0.f, pa1 = 0.f, pa2 = 0.f;
     float pc0 = 0.f, pc1 = 0.f, pc2 = 0.f; // GRAD: carries of the d/dc weights
     int gq = w_lo + 32 * q_start + lane + 1 - I.g_first; // this lane's cell (first pass) relative to g_first
     int carry = jstart(gq);                                // lane 0: start of its cell
-    const uint32_t wbase = a_w + (uint32_t)I.wbase * 4u;
     uint32_t outp = at_slot + (uint32_t)((q_start - q_lo) * 32 + lane) * 4u;
     // value of lane - d: of `cur` for lanes >= d, of `prev` (the previous pass) for lanes < d -- one select
     // and one indexed shuffle: the lanes 32 - d .. 31, which nobody reads `cur` from, offer `prev`
@@ -356,7 +389,7 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
         const int cntA = jeA - jsA, cntB = jeB - jsB;
         const float fA = (float)jsA, fB = (float)jsB;
         const float2 f2 = make_float2(fA, fB);
-        uint32_t wpA = wbase + (uint32_t)jsA * 4u, wpB = wbase + (uint32_t)jsB * 4u;
+        uint32_t wpA = wbase + (uint32_t)jsA * WS, wpB = wbase + (uint32_t)jsB * WS;
         const int km = __reduce_max_sync(FULL, max(cntA, cntB));
         float2 m0 = make_float2(0.f, 0.f), m1 = m0, m2 = m0, m3 = m0;
         float2 n0 = m0, n1 = m0, n2 = m0, n3 = m0; // GRAD: weighted by CL
@@ -367,23 +400,34 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
         float2 r2v = __ffma2_rn(f2, ll, make_float2(r_first, r_first));
         auto trip = [&](int k) { // sample k of each of the lane's two cells
             float2 w = make_float2(0.f, 0.f);
-            if (k < cntA) w.x = lds32(wpA);
-            if (k < cntB) w.y = lds32(wpB);
-            wpA += 4u;
-            wpB += 4u;
-            const float2 cl = colour_arg2<NCL, CM>(col, r2v);
+            SB_CHECK(k >= cntA || (wpA >= wbase && wpA < wbase + (uint32_t)n_in * WS));
+            SB_CHECK(k >= cntB || (wpB >= wbase && wpB < wbase + (uint32_t)n_in * WS));
+            float2 tq = t2v, rq = r2v; // position in the cell and reduced wavelength of this sample
+            if constexpr (NU) {
+                float2 dd = make_float2(0.f, 0.f);
+                if (k < cntA) { const float2 v = lds64(wpA); w.x = v.x; dd.x = v.y; }
+                if (k < cntB) { const float2 v = lds64(wpB); w.y = v.x; dd.y = v.y; }
+                tq = __ffma2_rn(dd, make_float2(acell, acell), t2v);
+                rq = __ffma2_rn(dd, make_float2(alr, alr), r2v);
+            } else {
+                if (k < cntA) w.x = lds32(wpA);
+                if (k < cntB) w.y = lds32(wpB);
+            }
+            wpA += WS;
+            wpB += WS;
+            const float2 cl = colour_arg2<NCL, CM>(col, rq);
             const float2 ar = GRAD ? __fmul2_rn(cl, cc2) : cl;
             const float2 e = __fmul2_rn(make_float2(sb::exp_scaled(ar.x), sb::exp_scaled(ar.y)), w);
-            const float2 tt = __fmul2_rn(t2v, t2v);
-            const float2 ttt = __fmul2_rn(tt, t2v);
+            const float2 tt = __fmul2_rn(tq, tq);
+            const float2 ttt = __fmul2_rn(tt, tq);
             m0 = __fadd2_rn(m0, e);
-            m1 = __ffma2_rn(e, t2v, m1);
+            m1 = __ffma2_rn(e, tq, m1);
             m2 = __ffma2_rn(e, tt, m2);
             m3 = __ffma2_rn(e, ttt, m3);
             if (GRAD) {
                 const float2 g = __fmul2_rn(e, cl);
                 n0 = __fadd2_rn(n0, g);
-                n1 = __ffma2_rn(g, t2v, n1);
+                n1 = __ffma2_rn(g, tq, n1);
                 n2 = __ffma2_rn(g, tt, n2);
                 n3 = __ffma2_rn(g, ttt, n3);
             }
@@ -401,6 +445,8 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
         const bool border = g0 <= 0 || g0 + 63 >= nW - 2;
         const bool stA = q >= q_a, stB = q + 1 >= q_a && q + 1 < q_b;
         const float2 at = node_weights(g, border, m0, m1, m2, m3, pa0, pa1, pa2);
+        SB_CHECK(!stA || (outp >= at_slot && outp < at_slot + kSlotW * 4u));
+        SB_CHECK(!stB || (outp + 128u >= at_slot && outp + 128u < at_slot + kSlotW * 4u));
         if (stA) sts32(outp, at.x);
         if (stB) sts32(outp + 128u, at.y);
         if (GRAD) {
@@ -415,7 +461,7 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
 
 // One item, window segment passes [q_lo, q_hi) of the band's node grid (q_hi - q_lo <= kPassSeg); the
 // slot is zero filled up to a whole 64-node block (phase B reads it in 64-node blocks).
-template <int NCL, bool GRAD>
+template <int NCL, bool GRAD, bool NU>
 __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const NSeg &S, const NItem &I, int w_lo,
                                              int q_lo, int q_hi, uint32_t a_w, uint32_t at_slot, int lane)
 {
@@ -428,6 +474,7 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const NSeg
     }
     // zero fill up to what phase B reads: whole 64-node blocks, and (forward) at least 128 nodes
     const int q_fill = q_lo + ((!GRAD && q_hi - q_lo <= 2) ? 4 : (((q_hi - q_lo) + 1) & ~1));
+    SB_CHECK(q_hi - q_lo >= 1 && q_hi - q_lo <= kPassSeg && q_fill - q_lo <= kPassSeg);
     for (int q = q_lo; q < q_a; ++q) {
         sts32(at_slot + (uint32_t)((q - q_lo) * 32 + lane) * 4u, 0.f);
         if (GRAD) sts32(at_slot + (uint32_t)(kSlotW + (q - q_lo) * 32 + lane) * 4u, 0.f);
@@ -439,15 +486,15 @@ __device__ __forceinline__ void phase_a_item(const SbModelParams &mp, const NSeg
     if (q_a >= q_b) return;
     const int q_start = q_a > qa ? q_a - 1 : q_a;
     if (I.cmode == sb::CM_INSIDE)
-        phase_a_passes<NCL, sb::CM_INSIDE, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
+        phase_a_passes<NCL, sb::CM_INSIDE, GRAD, NU>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
     else if (I.cmode == sb::CM_LINEAR)
-        phase_a_passes<NCL, sb::CM_LINEAR, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
+        phase_a_passes<NCL, sb::CM_LINEAR, GRAD, NU>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
     else if (I.cmode == CM_CROSS_HI)
-        phase_a_passes<NCL, CM_CROSS_HI, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
+        phase_a_passes<NCL, CM_CROSS_HI, GRAD, NU>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
     else if (I.cmode == CM_CROSS_LO)
-        phase_a_passes<NCL, CM_CROSS_LO, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
+        phase_a_passes<NCL, CM_CROSS_LO, GRAD, NU>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
     else
-        phase_a_passes<NCL, sb::CM_GENERIC, GRAD>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
+        phase_a_passes<NCL, sb::CM_GENERIC, GRAD, NU>(mp, S, I, w_lo, q_start, q_a, q_b, q_lo, a_w, at_slot, lane);
 }
 
 // ---- phase B: observations [i_lo, i_hi) of the sorted list (all of one band) on one warp ----------
@@ -510,8 +557,10 @@ __device__ __forceinline__ void phase_b_window(const SbNParams &P, int n0, uint3
     struct Vals { float v[NV]; };
     auto one = [&](int i) { // value [, d/dx1, d/dc, d/dt0] shares of observation i
         Vals out;
+        SB_CHECK(i >= 0 && i < SA.cap);
         const uint32_t info = lds32u(SA.info + (uint32_t)i * 4u);
         const uint32_t slot = info & 31u;
+        SB_CHECK(slot < (uint32_t)SA.n_slots && (int)(info >> 17) < SA.cap);
         const int rb = (int)((info >> 5) & 4095u);
         if (rb != rb_held) rows(rb);
         const float4 w4 = lds128(SA.ws + (uint32_t)i * 16u);
@@ -631,9 +680,10 @@ __device__ __forceinline__ bool obs_phase(const SbModelParams &mp, const NSeg &S
 }
 
 // ---- the kernel ---------------------------------------------------------------------------------
-template <int NCL, bool GRAD, int NW>
-__global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const __grid_constant__ SbNParams P)
+template <int NCL, bool GRAD, bool NU>
+__global__ void __launch_bounds__(16 * 32, 1) sb_nw_kernel(const __grid_constant__ SbNParams P)
 {
+    constexpr int NW = 16; // one CTA of 16 warps per SM (two CTAs of 8 warps were measured slower: DESIGN.md section 9)
     constexpr int kWarps = Cfg<NW>::kWarps, kThreads = Cfg<NW>::kThreads, kSlots = Cfg<NW>::kSlots;
     constexpr int kBins = Cfg<NW>::kBins, kCapFwd = Cfg<NW>::kCapFwd, kCapGrad = Cfg<NW>::kCapGrad;
     constexpr int NSL = GRAD ? kSlots / 2 : kSlots;     // item slots per buffer
@@ -645,7 +695,7 @@ __global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const SbModelParams &mp = P.mp;
     const int n_bands = P.n_bands, CAP = P.cap;
-    const NSmem L(P.n_band_total, CAP, GRAD, n_bands * NSL, NW);
+    const NSmem L(P.n_band_total, CAP, GRAD, n_bands * NSL, NW, NU);
     float *s_at = reinterpret_cast<float *>(smem_raw + L.at);
     float4 *s_ws = reinterpret_cast<float4 *>(smem_raw + L.ws);
     float *s_w = reinterpret_cast<float *>(smem_raw + L.w);
@@ -663,16 +713,21 @@ __global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const 
     double *carry = reinterpret_cast<double *>(smem_raw + L.carry);
     int *slot_tab = reinterpret_cast<int *>(smem_raw + L.slot_tab);     // [item slot] band-in-stage | segment << 8
     const uint32_t a_at = smem_addr(s_at), a_w = smem_addr(s_w);
-    const NShared SA{smem_addr(s_info), smem_addr(s_ws), smem_addr(s_ws + CAP), smem_addr(s_x1), smem_addr(res), CAP};
+    const NShared SA{smem_addr(s_info), smem_addr(s_ws), smem_addr(s_ws + CAP), smem_addr(s_x1), smem_addr(res), CAP, NSL};
 
     if (P.n_live != nullptr && __ldg(P.n_live) == 0) return; // fit driver: every lane has stopped
-    for (int i = tid; i < P.n_band_total; i += kThreads) s_w[i] = __ldg(P.band_w + i);
+    if constexpr (NU) {
+        float2 *s_wd = reinterpret_cast<float2 *>(smem_raw + L.w);
+        for (int i = tid; i < P.n_band_total; i += kThreads) s_wd[i] = __ldg(P.band_wd + i);
+    } else {
+        for (int i = tid; i < P.n_band_total; i += kThreads) s_w[i] = __ldg(P.band_w + i);
+    }
     const long long n_units = (long long)P.n_sn * P.n_samples;
     const long long n_groups = P.n_groups;
     const bool want_chi = P.out_chi2 != nullptr || (GRAD && P.out_dchi2 != nullptr);
     const int nP = mp.n_phase;
     const int nq = max(1, min(nP - 3, kBins / n_bands)); // phase-row bins per band
-    const NBandsView BV{n_bands, P.band_off, P.band_lam_first, P.band_h, P.band_dlam};
+    const NBandsView BV{n_bands, NU ? 0 : 1, P.band_off, P.band_lam_first, P.band_h, P.band_dlam};
     auto unit_lo = [&](long long g) { return (g * n_units) / n_groups; };
     auto pf = [](const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); };
 
@@ -750,6 +805,7 @@ __global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const 
             if (tid < kMaxBands) { win_all[tid] = 0x7fffffff; win_all[kMaxBands + tid] = -0x7fffffff; }
             __syncthreads();
             const int n_seg = misc[1], n_ev = misc[2];
+            SB_CHECK(n_seg >= 0 && n_seg <= NSL && n_ev >= 0 && n_ev <= CAP && n_bands * n_seg <= n_bands * NSL);
             if (tid < n_seg) { // segment parameters (S.unit / S.o_lo hold group-local values until here)
                 NSeg &S = segs[tid];
                 const NUnit t = units[S.unit];
@@ -805,6 +861,7 @@ __global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const 
                         double wrow[4], drow[4];
                         if (obs_phase(mp, S, __ldg(P.time + o), rb, wrow, drow)) {
                             const int key = b * nq + (rb * nq) / (nP - 3);
+                            SB_CHECK(rb >= 0 && rb <= nP - 4 && key >= 0 && key < kBins);
                             atomicAdd(&hist[key], 1);
                             rec_key[k] = key;
                             rec_sr[k] = lo | (rb << 8);
@@ -871,6 +928,7 @@ __global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const 
                 const int b = rec_key[k] / nq;
                 const int slot = (b % bps) * n_seg + sg; // item slot inside the band's stage
                 const int pos = atomicAdd(&hist[rec_key[k]], 1);
+                SB_CHECK(pos >= 0 && pos < n_ev && n_ev <= CAP && slot >= 0 && slot < NSL && sg < n_seg && e < n_ev);
                 s_ws[pos] = rec_w[k];
                 if (GRAD) s_ws[CAP + pos] = rec_d[k];
                 s_info[pos] = (uint32_t)slot | ((uint32_t)rb << 5) | ((uint32_t)e << 17);
@@ -932,7 +990,8 @@ __global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const 
                             const int np_b = (len + 31) >> 5;
                             const int q_lo = ws_n * kPassSeg, q_hi = min(q_lo + kPassSeg, np_b);
                             if (q_lo >= q_hi) continue;
-                            phase_a_item<NCL, GRAD>(mp, segs[sg], items_all[b0 * n_seg + it], w_lo, q_lo, q_hi, a_w,
+                            SB_CHECK(it < NSL && sg < n_seg && b0 + bl < n_bands && b0 * n_seg + it < n_bands * NSL);
+                            phase_a_item<NCL, GRAD, NU>(mp, segs[sg], items_all[b0 * n_seg + it], w_lo, q_lo, q_hi, a_w,
                                                     at_buf + (uint32_t)(it * ATS) * 4u, lane);
                         }
                     } else {
@@ -950,6 +1009,7 @@ __global__ void __launch_bounds__(NW * 32, NW == 16 ? 1 : 2) sb_nw_kernel(const 
                             const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
                             if (i_lo >= i_hi) continue;
                             const int n0 = w_lo + ws_c * kSlotW;
+                            SB_CHECK(n0 >= -4 && n0 + width <= mp.n_wave + 4 && i_hi <= n_ev && (n0 & 3) == 0);
                             const int nb64 = (width + 63) >> 6;
                             const bool first = ws_c == 0; // first sweep of these observations: results are stored, not added
                             // slot numbers in the records are (b % bps) * n_seg + sg = bl * n_seg + sg

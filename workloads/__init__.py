@@ -10,6 +10,7 @@ from .generators import (  # noqa: F401
     CONFIG_IDS,
     Workload,
     attach_data,
+    jitter_band_grids,
     make_bands,
     make_colour_law,
     make_model,

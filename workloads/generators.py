@@ -134,6 +134,27 @@ def pack_bands(bands) -> Dict[str, np.ndarray]:
     return {"offset": offset, "wave": np.ascontiguousarray(wave), "trans": np.ascontiguousarray(trans)}
 
 
+def jitter_band_grids(bands: Dict[str, np.ndarray], jitter: float, seed: int = 1003) -> Dict[str, np.ndarray]:
+    """Non-uniformly sampled copies of the band tables: every interior grid point is moved by U(-jitter,
+    +jitter) x the local step (jitter < 0.5 keeps the grid strictly increasing; the end points stay), and the
+    Gaussian transmission is re-tabulated at the moved wavelengths.  Real filter tables are not
+    uniformly sampled; this is their synthetic stand-in.  Table generation only."""
+    if not 0.0 <= jitter < 0.5:
+        raise ValueError("jitter must be in [0, 0.5)")
+    rng = np.random.default_rng(seed)
+    wave, trans = bands["wave"].copy(), bands["trans"].copy()
+    off = bands["offset"]
+    for b in range(len(off) - 1):
+        lo, hi = int(off[b]), int(off[b + 1])
+        w = wave[lo:hi]
+        step = (w[-1] - w[0]) / (len(w) - 1)
+        centre = 0.5 * (w[0] + w[-1])
+        sigma = (w[-1] - w[0]) / 3.0 / FWHM_TO_SIGMA  # the grid spans centre +- 1.5 FWHM (gaussian_band)
+        w[1:-1] += rng.uniform(-jitter, jitter, size=len(w) - 2) * step
+        trans[lo:hi] = np.exp(-0.5 * ((w - centre) / sigma) ** 2)
+    return {"offset": off.copy(), "wave": wave, "trans": trans}
+
+
 def make_bands(config: int) -> Dict[str, np.ndarray]:
     if config in (1, 3):
         centres = np.array([4800.0, 6200.0, 7500.0, 8700.0])
@@ -214,7 +235,7 @@ _FULL = {  # n_sn, n_samples, n_obs per SN
 
 
 def make_workload(config: int, n_sn: Optional[int] = None, n_samples: Optional[int] = None,
-                  ragged: bool = False, seed_offset: int = 0) -> Workload:
+                  ragged: bool = False, seed_offset: int = 0, band_jitter: float = 0.0) -> Workload:
     """Build config `config` (1..5).  `n_sn` / `n_samples` shrink it for parity tests.
 
     The shrunk workload is a prefix of the same random streams only in distribution, not
@@ -222,6 +243,7 @@ def make_workload(config: int, n_sn: Optional[int] = None, n_samples: Optional[i
     `ragged=True` draws a different observation count per supernova (between half and the
     full count) to exercise the CSR layout; BASELINE.json's configs are all regular.
     `seed_offset` shifts the config's seed (one shard per rank in multi-GPU weak scaling).
+    `band_jitter` > 0 replaces the 5 A band grids by non-uniform ones (jitter_band_grids).
     """
     if config not in CONFIG_IDS:
         raise ValueError(f"unknown config {config}")
@@ -233,6 +255,8 @@ def make_workload(config: int, n_sn: Optional[int] = None, n_samples: Optional[i
     model = make_model(nir=(config == 5))
     model.update(make_colour_law())
     bands = make_bands(config)
+    if band_jitter > 0.0:
+        bands = jitter_band_grids(bands, band_jitter)
     n_bands = len(bands["offset"]) - 1
 
     if ragged:
