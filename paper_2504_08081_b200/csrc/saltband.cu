@@ -234,6 +234,20 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
             return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
         }
     }
+    if ((size_t)n_phase * p.ld * sizeof(float) <= (size_t)SBN_M1_OFF) { // tables of the node-weight kernel (sb_internal.h)
+        const size_t m1_at = SBN_M1_OFF / sizeof(float);
+        std::vector<float> tx(m1_at + (size_t)n_phase * p.ld, 0.f);
+        for (int k = 0; k < n_phase; ++k)
+            for (int l = 0; l < n_wave; ++l) {
+                const size_t at = (size_t)k * p.ld + SB_PAD_L + l;
+                tx[at] = (float)m0[(size_t)k * n_wave + l];
+                tx[m1_at + at] = (float)m1[(size_t)k * n_wave + l];
+            }
+        if (!upload(&h->mx_f32, tx)) {
+            sb_free_model(h);
+            return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
+        }
+    }
     *out = h;
     return SB_OK;
 }
@@ -246,6 +260,7 @@ void sb_free_model(sb_model *m)
     cudaFree(m->m0_f64);
     cudaFree(m->m1_f64);
     cudaFree(m->m01_f32);
+    cudaFree(m->mx_f32);
     delete m;
 }
 
@@ -557,7 +572,7 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
               const void *fluxerr, void *out_flux, void *out_chi2, void *out_dflux, void *out_dchi2, cudaStream_t st,
               const RunLive &lv)
 {
-    if (m->prm.n_cl > SB_MAX_CL || b->n_bands > sbn::kMaxBands) return 1;
+    if (m->prm.n_cl > SB_MAX_CL || b->n_bands > sbn::kMaxBands || !m->mx_f32) return 1;
     if (m->prm.n_phase < 4 || m->prm.n_phase > 4096) return 1;
     const int smem_max = m->smem_optin, n_sm = m->n_sm;
     const long long n_units = (long long)bt->n_sn * bt->n_samples;
@@ -600,8 +615,7 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     sbn::SbNParams np;
     memset(&np, 0, sizeof(np));
     np.mp = m->prm;
-    np.m0 = m->m0_f32;
-    np.m1 = m->m1_f32;
+    np.mx = m->mx_f32;
     np.n_bands = b->n_bands;
     np.n_band_total = b->n_total;
     np.band_off = b->d_off;

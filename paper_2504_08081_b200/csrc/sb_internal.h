@@ -38,11 +38,18 @@ struct SbModelParams {
 #define SBH_PAD_L 16
 #define SBH_LDN 1856
 
+// fp32 tables of the node-weight kernel (sb_nw.cuh) in ONE allocation: M0 [n_phase][ld] at byte 0 and M1
+// [n_phase][ld] at the compile-time byte offset SBN_M1_OFF (node l at column l + SB_PAD_L, zero padded), so
+// that the M1 row of a phase is reached from the pointer to its M0 row with an immediate offset (global loads
+// take signed 24-bit immediates: < 8 MB).  Models whose M0 table exceeds SBN_M1_OFF run the direct kernel.
+#define SBN_M1_OFF (4 << 20)
+
 struct sb_model {
     SbModelParams prm;
     float *m0_f32, *m1_f32;   // [n_phase][ld], zero padded (SB_PAD_L)
     double *m0_f64, *m1_f64;  // [n_phase][ld]
     float2 *m01_f32;          // [n_phase][SBH_LDN] or NULL when n_wave + 34 > SBH_LDN
+    float *mx_f32;            // M0 table, M1 table SBN_M1_OFF bytes further (see above); NULL if M0 exceeds the offset
     int device;
     int n_sm, smem_optin;     // of `device`, read once at load
 };

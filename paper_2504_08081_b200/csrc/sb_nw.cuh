@@ -138,7 +138,7 @@ struct NSmem {
 // Kernel parameter block.
 struct SbNParams {
     SbModelParams mp;
-    const float *m0, *m1;             // [n_phase][mp.ld]
+    const float *mx;                  // M0 [n_phase][mp.ld]; M1 the same SBN_M1_OFF bytes further (sb_internal.h)
     int32_t n_bands, n_band_total;
     const int32_t *band_off;
     const double *band_lam_first, *band_zpab_inv, *band_h, *band_dlam;
@@ -189,6 +189,25 @@ __device__ __forceinline__ uint32_t lds32u(uint32_t a)
     return v;
 }
 __device__ __forceinline__ void sts32(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v)); }
+
+// Read-only global loads at a compile-time byte offset from a pointer.  TAG (the register slot the row goes
+// to) is spelled into the instruction text so that the loads of different switch cases are different
+// instructions for the compiler: it then writes each case's rows straight into that case's registers
+// instead of merging the cases into one load followed by predicated register moves.
+template <int TAG, int OFF> __device__ __forceinline__ float4 ldg128_at(const float *p)
+{
+    float4 v;
+    asm volatile("{\n\t// row slot %5\n\tld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4+%6];\n\t}"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "n"(TAG), "n"(OFF));
+    return v;
+}
+template <int TAG, int OFF> __device__ __forceinline__ float2 ldg64_at(const float *p)
+{
+    float2 v;
+    asm volatile("{\n\t// row slot %3\n\tld.global.nc.v2.f32 {%0, %1}, [%2+%4];\n\t}"
+                 : "=f"(v.x), "=f"(v.y) : "l"(p), "n"(TAG), "n"(OFF));
+    return v;
+}
 
 struct NShared { // shared-state-space addresses of the arrays phase B reads
     uint32_t info, ws, wd, x1, res;
@@ -511,59 +530,67 @@ __device__ __forceinline__ void phase_b_window(const SbNParams &P, int n0, uint3
     constexpr int NQ = 2 * N128 + (T64 ? 1 : 0); // packed node pairs per lane
     constexpr uint32_t ATS = (GRAD ? 2 * kSlotW : kSlotW) * 4u; // bytes per item slot
     constexpr int NV = GRAD ? 4 : 1;
-    const int ld = P.mp.ld;
     float2 M0[4][NQ], M1[4][NQ]; // [slot = row mod 4][node pair]
 #pragma unroll
     for (int s = 0; s < 4; ++s)
 #pragma unroll
         for (int q = 0; q < NQ; ++q) { M0[s][q] = make_float2(0.f, 0.f); M1[s][q] = make_float2(0.f, 0.f); }
     // the table rows are zero padded on the right by a whole window (saltband.cu: ld), so every load of a
-    // window that starts at a node of the grid stays inside its row: no bounds predicates
-    const float *p0 = P.m0 + (n0 + SB_PAD_L + 4 * lane), *p1 = P.m1 + (n0 + SB_PAD_L + 4 * lane);
+    // window that starts at a node of the grid stays inside its row: no bounds predicates.  One pointer per
+    // lane: its nodes of the M0 row of phase row r are at pb + r ld, those of the M1 row SBN_M1_OFF bytes further.
+    const float *pb = P.mx + (n0 + SB_PAD_L + 4 * lane);
+    const unsigned ld = (unsigned)P.mp.ld;
     const int toff = 128 * N128 - 2 * lane; // tail pair: column n0 + PAD + 128 N128 + 2 lane
     int rb_held = -64; // rows rb_held .. rb_held + 3 are in the registers
-    const uint32_t a_lane = a_at + (uint32_t)lane * 16u, a_tail = a_at + 512u * N128 + (uint32_t)lane * 8u;
+    // per-lane shared addresses of the node weights and of the sorted records, made opaque so that they
+    // stay in registers (re-materialising them from the thread index costs ~10 instructions per observation)
+    uint32_t a_lane = a_at + (uint32_t)lane * 16u, a_rec = SA.info;
+    asm volatile("" : "+r"(a_lane), "+r"(a_rec));
+    const uint32_t a_tail = a_lane + 512u * N128 - (uint32_t)lane * 8u;
+    const uint32_t d_ws = SA.ws - SA.info; // the row weights of record i are at a_rec + d_ws + 16 i
 
-    auto load_slot = [&](auto s_tag, int row) {
+    auto load_slot = [&](auto s_tag, const float *base, int row) {
         constexpr int s = decltype(s_tag)::value;
-        const ptrdiff_t ro = (ptrdiff_t)row * ld;
+        const float *pr = base + (size_t)(unsigned)row * ld;
+        static_assert(N128 <= 2, "row loads are written out for at most two 128-node blocks");
 #pragma unroll
         for (int h = 0; h < N128; ++h) {
-            const float4 a = __ldg(reinterpret_cast<const float4 *>(p0 + ro + 128 * h));
-            const float4 c = __ldg(reinterpret_cast<const float4 *>(p1 + ro + 128 * h));
+            const float4 a = h == 0 ? ldg128_at<s, 0>(pr) : ldg128_at<s, 512>(pr);
+            const float4 c = h == 0 ? ldg128_at<s, SBN_M1_OFF>(pr) : ldg128_at<s, SBN_M1_OFF + 512>(pr);
             M0[s][2 * h] = make_float2(a.x, a.y); M0[s][2 * h + 1] = make_float2(a.z, a.w);
             M1[s][2 * h] = make_float2(c.x, c.y); M1[s][2 * h + 1] = make_float2(c.z, c.w);
         }
         if constexpr (T64) {
-            M0[s][2 * N128] = __ldg(reinterpret_cast<const float2 *>(p0 + ro + toff));
-            M1[s][2 * N128] = __ldg(reinterpret_cast<const float2 *>(p1 + ro + toff));
+            M0[s][2 * N128] = ldg64_at<s, 0>(pr + toff);
+            M1[s][2 * N128] = ldg64_at<s, SBN_M1_OFF>(pr + toff);
         }
     };
     auto rows = [&](int rb) { // make rows rb .. rb+3 resident; the sorted order makes rb grow slowly
         const int d = rb - rb_held;
-        int r = (d > 0 && d < 4) ? rb_held + 4 : rb; // first row that is not in the registers yet
+        const int first = (d > 0 && d < 4) ? rb_held + 4 : rb; // first row that is not in the registers yet
         rb_held = rb;
-#pragma unroll 1
-        for (; r < rb + 4; ++r) { // warp-uniform row -> its register slot
-            switch (r & 3) {
-            case 0: load_slot(std::integral_constant<int, 0>{}, r); break;
-            case 1: load_slot(std::integral_constant<int, 1>{}, r); break;
-            case 2: load_slot(std::integral_constant<int, 2>{}, r); break;
-            default: load_slot(std::integral_constant<int, 3>{}, r); break;
-            }
-        }
+        // the lane's pointer, made opaque so that it is formed once per call and not once per slot (the
+        // compiler re-materialises it instead of keeping it: 127 live registers)
+        const float *base;
+        asm volatile("mov.u64 %0, %1;" : "=l"(base) : "l"(pb));
+        // one predicated block per register slot (no loop, no switch: the four blocks are straight-line code
+        // that writes its own registers): slot s takes the row of [rb, rb + 4) congruent to s mod 4
+        { const int row = rb + ((0 - rb) & 3); if (row >= first) load_slot(std::integral_constant<int, 0>{}, base, row); }
+        { const int row = rb + ((1 - rb) & 3); if (row >= first) load_slot(std::integral_constant<int, 1>{}, base, row); }
+        { const int row = rb + ((2 - rb) & 3); if (row >= first) load_slot(std::integral_constant<int, 2>{}, base, row); }
+        { const int row = rb + ((3 - rb) & 3); if (row >= first) load_slot(std::integral_constant<int, 3>{}, base, row); }
     };
 
     struct Vals { float v[NV]; };
     auto one = [&](int i) { // value [, d/dx1, d/dc, d/dt0] shares of observation i
         Vals out;
         SB_CHECK(i >= 0 && i < SA.cap);
-        const uint32_t info = lds32u(SA.info + (uint32_t)i * 4u);
+        const uint32_t info = lds32u(a_rec + (uint32_t)i * 4u);
         const uint32_t slot = info & 31u;
         SB_CHECK(slot < (uint32_t)SA.n_slots && (int)(info >> 17) < SA.cap);
         const int rb = (int)((info >> 5) & 4095u);
         if (rb != rb_held) rows(rb);
-        const float4 w4 = lds128(SA.ws + (uint32_t)i * 16u);
+        const float4 w4 = lds128(a_rec + d_ws + (uint32_t)i * 16u);
         const float2 xx = lds64(SA.x1 + slot * 8u);
         const uint32_t so = slot * ATS;
         float2 at[NQ], ac[GRAD ? NQ : 1];
