@@ -354,8 +354,16 @@ __device__ __forceinline__ void phase_a_passes(const SbModelParams &mp, const NS
                     const float kf = (float)k;
                     return __fmaf_rn(kf, ha_hi, __fmaf_rn(kf, ha_lo, lds64(wbase + (uint32_t)k * 8u).y * acell));
                 };
-                while (j > 0 && uk(j - 1) >= xf) --j;
-                while (j < n_in && uk(j) < xf) ++j;
+                // the guess's two neighbours are tested at once (independent loads); the loops only run on
+                // grids further than one sample from their mean-step grid
+                const float below = j > 0 ? uk(j - 1) : -3.0e38f, at = j < n_in ? uk(j) : 3.0e38f;
+                if (below >= xf) {
+                    --j;
+                    while (j > 0 && uk(j - 1) >= xf) --j;
+                } else if (at < xf) {
+                    ++j;
+                    while (j < n_in && uk(j) < xf) ++j;
+                }
             }
         }
         return j;
