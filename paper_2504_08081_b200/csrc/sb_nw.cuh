@@ -818,67 +818,82 @@ __global__ void __launch_bounds__(16 * 32, 1) sb_nw_kernel(const __grid_constant
             if (cur_u >= npos) break;
             // ---- round: consecutive units whose observations fit the result array (a unit larger
             // than the array is processed alone, CAP observations at a time)
-            if (tid == 0) {
-                int u = misc[3], off = misc[4], n_ev = 0, n_seg = 0;
-                while (u < npos && n_seg < NSL) {
-                    const int rem = units[u].n - off;
-                    NSeg &S = segs[n_seg];
-                    if (rem <= CAP - n_ev) {
-                        S.unit = u; S.o_lo = off; S.n = rem; S.e_begin = n_ev; S.first = (off == 0); S.last = 1;
-                        n_ev += rem; ++n_seg; ++u; off = 0;
-                    } else if (n_ev == 0) {
-                        S.unit = u; S.o_lo = off; S.n = CAP; S.e_begin = 0; S.first = (off == 0); S.last = 0;
-                        n_ev = CAP; ++n_seg; off += CAP;
-                        break;
-                    } else {
-                        break;
-                    }
+            // built by warp 0, one lane per unit: an inclusive scan of the observation counts decides how many
+            // units fit; the same lanes then fill in their segment's parameters
+            if (warp == 0) {
+                const int u0 = misc[3], off0 = misc[4];
+                __syncwarp(); // every lane has read the cursor before lane 0 advances it
+                const int u = u0 + lane;
+                const bool have = u < npos && lane < NSL;
+                const int n = have ? units[u].n - (lane == 0 ? off0 : 0) : 0;
+                int incl = n;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int v = __shfl_up_sync(FULL, incl, o);
+                    if (lane >= o) incl += v;
                 }
-                misc[1] = n_seg; misc[2] = n_ev; misc[3] = u; misc[4] = off;
+                const unsigned fits = __ballot_sync(FULL, have && incl <= CAP);
+                const int n_fit = fits == FULL ? 32 : __ffs(~fits) - 1; // leading run of units that fit (counts >= 0: monotone)
+                const bool split = n_fit == 0;      // the first unit alone exceeds the round: CAP observations of it
+                const int n_seg_w = split ? 1 : n_fit;
+                const int n_ev_w = split ? CAP : __shfl_sync(FULL, incl, max(n_fit - 1, 0));
+                if (lane == 0) {
+                    misc[1] = n_seg_w; misc[2] = n_ev_w;
+                    misc[3] = split ? u0 : u0 + n_fit;
+                    misc[4] = split ? off0 + CAP : 0;
+                }
+                if (lane < n_seg_w) {
+                    NSeg &S = segs[lane];
+                    const NUnit t = units[u];
+                    const int off = lane == 0 ? off0 : 0;
+                    const int ks = t.unit - t.sn * P.n_samples;
+                    S.n = split ? CAP : n;
+                    S.e_begin = split ? 0 : incl - n;
+                    S.first = off == 0;
+                    S.last = split ? 0 : 1;
+                    S.unit = t.unit;
+                    S.sn = t.sn;
+                    S.o_lo = t.o_lo + off;
+                    S.out_base = (long long)t.o_lo * P.n_samples + (long long)ks * t.n + off;
+                    const double cc = (double)t.c;
+                    S.opz = 1.0 + (double)t.z;
+                    S.inv_opz = 1.0 / S.opz;
+                    S.x0 = (double)t.x0;
+                    S.x1 = t.x1;
+                    S.t0 = (double)t.t0;
+                    S.cc = cc;
+                    const double cscale = cc * 1.4426950408889634; // exponent in log2 units (ex2)
+#pragma unroll
+                    for (int q = 0; q < SB_MAX_CL; ++q) S.cl[q] = (float)(mp.cl[q] * cscale);
+                    S.s_lo = (float)(mp.s_lo * cscale);
+                    S.s_hi = (float)(mp.s_hi * cscale);
+                    S.cs = (float)cscale;
+                }
             }
             for (int i = tid; i < kBins; i += kThreads) hist[i] = 0;
             if (tid < kMaxBands) { win_all[tid] = 0x7fffffff; win_all[kMaxBands + tid] = -0x7fffffff; }
-            __syncthreads();
-            const int n_seg = misc[1], n_ev = misc[2];
-            SB_CHECK(n_seg >= 0 && n_seg <= NSL && n_ev >= 0 && n_ev <= CAP && n_bands * n_seg <= n_bands * NSL);
-            if (tid < n_seg) { // segment parameters (S.unit / S.o_lo hold group-local values until here)
-                NSeg &S = segs[tid];
-                const NUnit t = units[S.unit];
-                const int off = S.o_lo;
-                const int ks = t.unit - t.sn * P.n_samples;
-                S.unit = t.unit;
-                S.sn = t.sn;
-                S.o_lo = t.o_lo + off;
-                S.out_base = (long long)t.o_lo * P.n_samples + (long long)ks * t.n + off;
-                const double cc = (double)t.c;
-                S.opz = 1.0 + (double)t.z;
-                S.inv_opz = 1.0 / S.opz;
-                S.x0 = (double)t.x0;
-                S.x1 = t.x1;
-                S.t0 = (double)t.t0;
-                S.cc = cc;
-                const double cscale = cc * 1.4426950408889634; // exponent in log2 units (ex2)
-#pragma unroll
-                for (int q = 0; q < SB_MAX_CL; ++q) S.cl[q] = (float)(mp.cl[q] * cscale);
-                S.s_lo = (float)(mp.s_lo * cscale);
-                S.s_hi = (float)(mp.s_hi * cscale);
-                S.cs = (float)cscale;
-            }
-            for (int e = tid; e < n_ev; e += kThreads) {
+            for (int e = tid; e < CAP; e += kThreads) { // results of observations outside the grid stay 0
                 res[e] = 0.f;
                 if (GRAD) { res[CAP + e] = 0.f; res[2 * CAP + e] = 0.f; res[3 * CAP + e] = 0.f; }
             }
             __syncthreads();
+            const int n_seg = misc[1], n_ev = misc[2];
+            SB_CHECK(n_seg >= 1 && n_seg <= NSL && n_ev >= 0 && n_ev <= CAP);
 
             // ---- a1: every observation once: phase -> (rb, row weights); counting sort by (band, rb)
             float4 rec_w[KPT], rec_d[GRAD ? KPT : 1];
             int rec_key[KPT];                 // bin, or -1
             int rec_sr[KPT];                  // segment | rb << 8
+            int rec_b[KPT];                   // band of the observation
+            float rec_t[KPT];                 // its time
+            // first pass: segment of every observation of this thread and its global loads, all in flight at once
 #pragma unroll
             for (int k = 0; k < KPT; ++k) {
                 const int e = tid + k * kThreads;
                 rec_key[k] = -1;
                 rec_sr[k] = 0;
+                rec_b[k] = -1;
+                rec_t[k] = 0.f;
                 rec_w[k] = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (GRAD) rec_d[k] = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (e < n_ev) {
@@ -888,13 +903,23 @@ __global__ void __launch_bounds__(16 * 32, 1) sb_nw_kernel(const __grid_constant
                         if (segs[mid].e_begin <= e) lo = mid;
                         else hi = mid - 1;
                     }
+                    const int o = segs[lo].o_lo + (e - segs[lo].e_begin);
+                    rec_sr[k] = lo;
+                    rec_b[k] = __ldg(P.band + o);
+                    rec_t[k] = __ldg(P.time + o);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < KPT; ++k) {
+                const int e = tid + k * kThreads;
+                if (e < n_ev) {
+                    const int lo = rec_sr[k];
                     const NSeg &S = segs[lo];
-                    const int o = S.o_lo + (e - S.e_begin);
-                    const int b = __ldg(P.band + o);
+                    const int b = rec_b[k];
                     if ((unsigned)b < (unsigned)n_bands) {
                         int rb;
                         double wrow[4], drow[4];
-                        if (obs_phase(mp, S, __ldg(P.time + o), rb, wrow, drow)) {
+                        if (obs_phase(mp, S, rec_t[k], rb, wrow, drow)) {
                             const int key = b * nq + (rb * nq) / (nP - 3);
                             SB_CHECK(rb >= 0 && rb <= nP - 4 && key >= 0 && key < kBins);
                             atomicAdd(&hist[key], 1);

@@ -145,3 +145,25 @@ def test_full_size_config5_host_buffer_call_in_chunks(cuda_device):
     assert np.all(err <= tol), f"worst flux err/tol {np.max(err / np.maximum(tol, 1e-300)):.3g}"
     tolc = sbgpu.chi2_tolerance(sub, ref["flux"], tol, 1, False)
     assert np.all(np.abs(_gather_units(wl, idx, got_chi, False) - ref["chi2"]) <= tolc)
+
+
+def test_full_size_config5_nonuniform_band_grids(cuda_device):
+    """The whole of config 5 with band grids jittered by +-30 % of the step (bench.py --band-jitter 0.3):
+    the node-weight kernel's NU variant on sampled units against the oracle and on ALL units against the
+    direct kernel."""
+    wl = workloads.make_workload(5, band_jitter=0.3)
+    idx = _sample_indices(wl.n_sn, 600, 123)
+    sub = _attach_sampled(wl, idx)
+    ref = oracle.run_workload(sub, want_flux=True, want_chi2=True)
+    got = sbgpu.run_gpu(wl, mode="chi2")
+    assert got["form"] == "tiled"
+    tol = sbgpu.flux_tolerance(sub, ref["flux"], 1, False)
+    err = np.abs(_gather_units(wl, idx, got["flux"], True) - ref["flux"])
+    assert np.all(err <= tol), f"worst flux err/tol {np.max(err / np.maximum(tol, 1e-300)):.3g}"
+    tolc = sbgpu.chi2_tolerance(sub, ref["flux"], tol, 1, False)
+    assert np.all(np.abs(_gather_units(wl, idx, got["chi2"], False) - ref["chi2"]) <= tolc)
+    direct = sbgpu.run_gpu(wl, mode="chi2", form="direct")
+    peak = sbgpu.unit_peaks(wl, direct["flux"], 1)
+    tol_all = 2.0 * (1e-5 * np.abs(direct["flux"]) + 1e-9 * peak)
+    err_all = np.abs(got["flux"] - direct["flux"])
+    assert np.all(err_all <= tol_all), f"tiled vs direct worst ratio {np.max(err_all / np.maximum(tol_all, 1e-300)):.3g}"

@@ -176,3 +176,23 @@ def test_random_grids_band_steps_and_redshifts(cuda_device, seed):
     if n == 0:
         return
     check_all_forms(attach(wl))
+
+
+def test_groups_of_exactly_32_units(cuda_device):
+    """148 x 32 supernovae: every CTA's group holds exactly 32 units (a full warp of segment lanes in the
+    round builder; the host-buffer calls cut their chunks to such multiples) -- forward and gradient."""
+    import torch
+
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    wl = workloads.make_workload(2, n_sn=32 * n_sm)
+    true = oracle.run_workload(wl, theta={k: v.copy() for k, v in wl.theta_true.items()})["flux"]
+    workloads.attach_data(wl, true)
+    ref = oracle.run_workload(wl, want_flux=True, want_chi2=True)
+    got = sbgpu.run_gpu(wl, mode="chi2", form="tiled")
+    tol = sbgpu.flux_tolerance(wl, ref["flux"], 1, False)
+    assert np.all(np.abs(got["flux"] - ref["flux"]) <= tol)
+    assert np.all(np.abs(got["chi2"] - ref["chi2"]) <= sbgpu.chi2_tolerance(wl, ref["flux"], tol, 1, False))
+    half = workloads.subset(wl, np.arange(16 * n_sm))  # gradient rounds hold 16 units
+    refg = oracle.run_workload(half, want_flux=True, want_dflux=True)
+    gotg = sbgpu.run_gpu(half, mode="grad", form="tiled", with_data=False)
+    assert np.all(np.abs(gotg["dflux"] - refg["dflux"]) <= sbgpu.grad_tolerance(half, refg, half.theta, 1, False))
