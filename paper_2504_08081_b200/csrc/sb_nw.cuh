@@ -1107,42 +1107,61 @@ __global__ void __launch_bounds__(16 * 32, 1) sb_nw_kernel(const __grid_constant
                 double sum[NS];
 #pragma unroll
                 for (int k = 0; k < NS; ++k) sum[k] = 0.0;
-                for (int i = lane; i < S.n; i += 32) {
-                    const int o = S.o_lo + i;
-                    const int b = __ldg(P.band + o);
-                    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
-                    double m = qnan, dm[4] = {qnan, qnan, qnan, qnan};
-                    if ((unsigned)b < (unsigned)P.n_bands) {
-                        double sc = 1.0;
-                        if (P.zp != nullptr) { // 10^(0.4 zp): recomputed only when zp changes (usually never)
-                            const float zpv = __ldg(P.zp + o);
-                            if (zpv != zp_last) {
-                                zp_last = zpv;
-                                zp_pow = exp10(0.4 * (double)zpv);
-                            }
-                            sc = zp_pow * __ldg(P.band_zpab_inv + b);
-                        }
-                        const double raw = (double)res[S.e_begin + i];
-                        m = sc * S.x0 * raw;
-                        if (GRAD) {
-                            dm[0] = sc * raw;
-                            dm[1] = sc * S.x0 * (double)res[CAP + S.e_begin + i];
-                            dm[2] = sc * S.x0 * (double)res[2 * CAP + S.e_begin + i];
-                            dm[3] = sc * S.x0 * (double)res[3 * CAP + S.e_begin + i];
+                // four observations per lane at a time: their global loads are issued together (one latency),
+                // then the arithmetic in the order of the observations (the sums keep their fixed order)
+                for (int i0 = lane; i0 < S.n; i0 += 128) {
+                    int b4[4];
+                    float zp4[4], f4[4], e4[4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int i = i0 + 32 * j;
+                        b4[j] = -1; zp4[j] = 0.f; f4[j] = 0.f; e4[j] = 1.f;
+                        if (i < S.n) {
+                            const int o = S.o_lo + i;
+                            b4[j] = __ldg(P.band + o);
+                            if (P.zp != nullptr) zp4[j] = __ldg(P.zp + o);
+                            if (want_chi) { f4[j] = __ldg(P.flux + o); e4[j] = __ldg(P.fluxerr + o); }
                         }
                     }
-                    if (P.out_flux) P.out_flux[S.out_base + i] = (float)m;
-                    if (GRAD && P.out_dflux)
-                        reinterpret_cast<float4 *>(P.out_dflux)[S.out_base + i] =
-                            make_float4((float)dm[0], (float)dm[1], (float)dm[2], (float)dm[3]);
-                    if (want_chi) {
-                        const double f = (double)__ldg(P.flux + o), e = (double)__ldg(P.fluxerr + o);
-                        const double qv = (f - m) / e;
-                        sum[0] += qv * qv;
-                        if (GRAD) {
-                            const double g = -2.0 * (f - m) / (e * e);
 #pragma unroll
-                            for (int k = 0; k < 4; ++k) sum[1 + k] += g * dm[k];
+                    for (int j = 0; j < 4; ++j) {
+                        const int i = i0 + 32 * j;
+                        if (i >= S.n) break;
+                        const int b = b4[j];
+                        const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+                        double m = qnan, dm[4] = {qnan, qnan, qnan, qnan};
+                        if ((unsigned)b < (unsigned)P.n_bands) {
+                            double sc = 1.0;
+                            if (P.zp != nullptr) { // 10^(0.4 zp): recomputed only when zp changes (usually never)
+                                const float zpv = zp4[j];
+                                if (zpv != zp_last) {
+                                    zp_last = zpv;
+                                    zp_pow = exp10(0.4 * (double)zpv);
+                                }
+                                sc = zp_pow * __ldg(P.band_zpab_inv + b);
+                            }
+                            const double raw = (double)res[S.e_begin + i];
+                            m = sc * S.x0 * raw;
+                            if (GRAD) {
+                                dm[0] = sc * raw;
+                                dm[1] = sc * S.x0 * (double)res[CAP + S.e_begin + i];
+                                dm[2] = sc * S.x0 * (double)res[2 * CAP + S.e_begin + i];
+                                dm[3] = sc * S.x0 * (double)res[3 * CAP + S.e_begin + i];
+                            }
+                        }
+                        if (P.out_flux) P.out_flux[S.out_base + i] = (float)m;
+                        if (GRAD && P.out_dflux)
+                            reinterpret_cast<float4 *>(P.out_dflux)[S.out_base + i] =
+                                make_float4((float)dm[0], (float)dm[1], (float)dm[2], (float)dm[3]);
+                        if (want_chi) {
+                            const double f = (double)f4[j], e = (double)e4[j];
+                            const double qv = (f - m) / e;
+                            sum[0] += qv * qv;
+                            if (GRAD) {
+                                const double g = -2.0 * (f - m) / (e * e);
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) sum[1 + k] += g * dm[k];
+                            }
                         }
                     }
                 }
