@@ -23,6 +23,9 @@
  *       first/last cell of each axis, zero outside the closed grid range                [G1-G3]
  *   CL(l): polynomial in (l - cl_wave_b)/(cl_wave_v - cl_wave_b) on [cl_lo, cl_hi], continued
  *       linearly (value and slope) outside                                                 [G5]
+ *   Conventions against SNCosmo-style SALT code (readings G5, G6): the exponent is NATURAL, exp(c CL) -- a
+ *       colour law given for 10^(-0.4 c CL') is passed as cl_coef[q] = -0.4 ln(10) a'_q; and there is NO
+ *       1/(1+z) flux-dilution factor -- the x0 of this library is such a code's x0/(1+z).
  *
  * Conventions
  *   - Loaders take HOST pointers and copy; compute calls take DEVICE pointers owned by the caller

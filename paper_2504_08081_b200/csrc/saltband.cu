@@ -648,7 +648,7 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     np.n_live = lv.n_live;
     np.n_groups = (int32_t)n_groups;
     np.cap = cap;
-    { const char *e = getenv("SB_NW_MIX"); np.mix = e ? atoi(e) : 2; }
+    { const char *e = getenv("SB_NW_MIX"); np.mix = e ? atoi(e) : 3; }
     const int grid = (int)(n_groups < (long long)n_cta ? n_groups : (long long)n_cta);
     const bool small_cl = m->prm.n_cl <= 5;
     if (nu) {

@@ -1032,17 +1032,23 @@ __global__ void __launch_bounds__(16 * 32, 1) sb_nw_kernel(const __grid_constant
             int st_n = 0, ws_n = 0, nws_n = 0, st_c = n_bst, ws_c = 0;
             while (st_n < n_bst && (nws_n = n_wseg_of(st_n)) == 0) ++st_n;
             int buf = 0;
-            // which warps start a super-step with phase A: 0 all, 1 the warps of two schedulers, 2 two warps of every scheduler
-            const bool a_first = P.mix == 0 ? true : P.mix == 1 ? (warp & 2) == 0 : ((warp >> 2) & 1) == 0;
+            // A super-step of a warp is three tasks: its (up to) two items of phase A and its chunk of phase B.
+            // Where the chunk sits among them depends on the warp (P.mix: 0 last in all warps; 1 first in the
+            // warps of two schedulers; 2 first in two warps of every scheduler; 3 first / middle / last / middle in
+            // the four warps of a scheduler), so that both kinds of work are in flight on every scheduler
+            const int wsch = (warp >> 2) & 3; // index of the warp among the warps of its scheduler
+            const int bpos = P.mix == 0 ? 2 : P.mix == 1 ? ((warp & 2) ? 0 : 2) : P.mix == 2 ? ((wsch & 1) ? 0 : 2)
+                                                                               : (wsch == 0 ? 0 : wsch == 2 ? 2 : 1);
             while (st_n < n_bst || st_c < n_bst) {
 #pragma unroll 1
-                for (int ph = 0; ph < 2; ++ph) {
-                    if ((ph == 0) == a_first) {
+                for (int task = 0; task < 3; ++task) {
+                    if (task != bpos) {
+                        const int slice = task < bpos ? task : task - 1; // first or second item of this warp
                         // ---- phase A of stage (st_n, ws_n): node weights of its items -> buffer buf
                         if (st_n >= n_bst) continue;
                         const uint32_t at_buf = a_at + (uint32_t)(buf * BUF) * 4u;
                         const int b0 = st_n * bps, nbs = min(bps, n_bands - b0), n_items = nbs * n_seg;
-                        for (int it = warp; it < n_items; it += kWarps) {
+                        for (int it = warp + slice * kWarps; it < n_items; it += 2 * kWarps) {
                             const int tb = slot_tab[it];
                             const int bl = tb & 255, sg = tb >> 8;
                             const int w_lo = win_all[b0 + bl], len = win_len(b0 + bl);
