@@ -105,3 +105,28 @@ def test_product_does_not_import_oracle():
         if f.endswith((".py", ".c")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2504_08081_b200" not in txt and "saltband.h\"" not in txt
+
+
+def test_fit_options_defaults_and_host_side_validation(lib):
+    """sb_fit_default_opts fills the documented defaults; sb_fit_lbfgs rejects NULL handles, missing
+    photometry and out-of-range options with SB_EINVAL before any CUDA call (runs without a GPU)."""
+    from paper_2504_08081_b200 import api
+
+    o = api._FitOpts()
+    lib.sb_fit_default_opts(C.byref(o))
+    assert (o.memory, o.max_eval, o.max_iter, o.trace_len) == (8, 60, 1000, 0)
+    assert o.ftol == 1e-12 and o.gtol == 0.0 and not o.lo and not o.hi
+    bt = api._Batch(api.SB_F32, 1, 1, 0, None, None, None, None, None, None, None, None, None, None)
+    res = api._FitResult(None, None, None, None, None, None)
+    assert lib.sb_fit_lbfgs(None, None, C.byref(bt), None, None, C.byref(o), C.byref(res), None) == -1
+    assert lib.sb_fit_lbfgs_host(None, None, C.byref(bt), None, None, C.byref(o), C.byref(res)) == -1
+    assert lib.sb_pack_observations(None, None, C.byref(bt), None, C.byref(C.c_void_p())) == -1
+    lib.sb_free_pack(None)  # NULL is allowed
+
+
+def test_binding_exposes_the_same_names_as_the_header():
+    import paper_2504_08081_b200 as sb
+
+    for n in ("sb_load_model", "sb_load_bandpasses", "sb_bandflux", "sb_chi2", "sb_bandflux_grad", "sb_pack_observations",
+              "sb_fit_lbfgs", "sb_chi2_host", "sb_bandflux_grad_host", "sb_fit_lbfgs_host"):
+        assert callable(getattr(sb, n)), n
