@@ -1071,8 +1071,13 @@ __global__ void __launch_bounds__(16 * 32, 1) sb_nw_kernel(const __grid_constant
                             const int width = min(kSlotW, len - ws_c * kSlotW);
                             if (width <= 0) continue;
                             const int lo = bstart[b0 + bl], n = bstart[b0 + bl + 1] - lo;
+                            if (n <= 0) continue;
                             const int per = (((n + kWarps - 1) / kWarps) + (GRAD ? 3 : 7)) & (GRAD ? ~3 : ~7);
-                            const int i_lo = lo + warp * per, i_hi = min(i_lo + per, lo + n);
+                            // chunk -> warp: in stages of several bands (small batches: few observations per band)
+                            // rotated from band to band, starting after the warps that carry one item more in
+                            // phase A, so that every warp gets chunks; one band per stage: chunk c on warp c
+                            const int rot = nbs > 1 ? (nbs * n_seg + 5 * bl) & (kWarps - 1) : 0;
+                            const int i_lo = lo + ((warp - rot) & (kWarps - 1)) * per, i_hi = min(i_lo + per, lo + n);
                             if (i_lo >= i_hi) continue;
                             const int n0 = w_lo + ws_c * kSlotW;
                             SB_CHECK(n0 >= -4 && n0 + width <= mp.n_wave + 4 && i_hi <= n_ev && (n0 & 3) == 0);
