@@ -48,7 +48,7 @@ FLOPS_PER_EVAL_GRAD = 120
 # per model cell of a chunk: sample range 9, moments -> node weights 20, x1 1; per node per
 # observation: 8 FFMA; per eval: phase weights, zero point, chi^2 term, reduction.
 FLOPS_G_SAMPLE, FLOPS_G_CELL, FLOPS_G_NODE_OBS, FLOPS_G_EVAL = 21, 30, 16, 60
-# Tiled formulation, csrc/sb_tiled.cuh: the same per-sample and per-cell work once per (unit, band)
+# Node-weight ("tiled") formulation, csrc/sb_nw.cuh: the same per-sample and per-cell work once per (unit, band)
 # ITEM (all its observations share it); per node per observation 8 FFMA (phase collapse of M0, M1
 # with x1 folded into the weights) + 1 FFMA (node weight) = 18.  Only nodes of the item's window count;
 # the zero-padded remainder of the 128-node half windows the kernel also multiplies is not counted.

@@ -111,7 +111,7 @@ struct SbKParams {
 struct SbHParams {
     SbModelParams mp;
     const float2 *m01;                // [n_phase][SBH_LDN] {M0, M1}
-    const float *m0, *m1;             // [n_phase][mp.ld] (sb_tiled.cuh)
+    const float *m0, *m1;             // [n_phase][mp.ld] (unused by the grouped kernel; kept for layout)
     int32_t n_bands, n_band_total;
     const int32_t *band_off;
     const double *band_lam_first, *band_zpab_inv, *band_h, *band_dlam;
