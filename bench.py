@@ -131,7 +131,8 @@ def flops_per_call(wl, grad: bool, form: str = "direct"):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 20 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 20 ms.  Started before the warm-up (the tool needs
+    tens of milliseconds to come up); stop(t0, t1) keeps the samples that arrived inside the timed region."""
 
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
@@ -152,9 +153,9 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.perf_counter(), line.strip()))
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -164,7 +165,10 @@ class ClockSampler:
             self.proc.kill()
         sm, smax, reasons, power = [], [], set(), []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
+        lines = [ln for t, ln in self.lines if t0 is None or (t0 <= t <= t1 + 0.02)]
+        if not lines:  # region shorter than one sampling period: the samples nearest to it
+            lines = [ln for _, ln in self.lines[-3:]]
+        for ln in lines:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
@@ -341,18 +345,19 @@ def run_fit(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local_rank)
+    sampler.start()
     for _ in range(warmup):
         step()
     barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    wall0 = time.perf_counter()
     for a, b in ev:
         a.record()
         step()
         b.record()
     barrier()
-    clocks = sampler.stop()
+    clocks = sampler.stop(wall0, time.perf_counter())
     total_ms = float(sum(a.elapsed_time(b) for a, b in ev))
     if dist is not None:
         tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
@@ -528,11 +533,11 @@ def main():
         torch.cuda.synchronize()
 
     # ---- device-resident timing: K steps, CUDA events per step on the launching (current) stream
+    sampler = ClockSampler(local_rank)
+    sampler.start()
     for _ in range(warmup):
         step(d)
     barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     wall0 = time.perf_counter()
     for a, b in ev:
@@ -542,8 +547,9 @@ def main():
         step(d)
         b.record()
     barrier()
-    wall = time.perf_counter() - wall0
-    clocks = sampler.stop()
+    wall1 = time.perf_counter()
+    wall = wall1 - wall0
+    clocks = sampler.stop(wall0, wall1)
     per_step_ms = np.array([a.elapsed_time(b) for a, b in ev])
     total_ms = float(per_step_ms.sum())
     if dist is not None:
