@@ -105,7 +105,9 @@ bool device_limits(int *n_sm, int *smem_optin)
 }
 
 // Opt-in dynamic shared memory of a kernel: set once per (kernel, device) to the device maximum.
-bool allow_max_smem(const void *kern, int device, int smem_optin)
+// `carve`: also prefer the largest shared-memory carveout (kernels that fill shared memory; the others keep
+// the default split so that their model-table reads stay in L1).
+bool allow_max_smem(const void *kern, int device, int smem_optin, bool carve = false)
 {
     static std::mutex mu;
     static std::vector<std::pair<const void *, int>> done;
@@ -116,7 +118,7 @@ bool allow_max_smem(const void *kern, int device, int smem_optin)
     if (!cuda_ok(cudaFuncGetAttributes(&fa, kern))) return false;
     const int dyn = smem_optin - (int)fa.sharedSizeBytes; // static + dynamic <= the opt-in limit
     if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn))) return false;
-    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (carve) cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     done.emplace_back(kern, device);
     return true;
 }
@@ -556,7 +558,7 @@ template <int NCL, bool GRAD, bool NU>
 int launch_nw_inst(const sb_model *m, const sbn::SbNParams &np, size_t smem, int grid, cudaStream_t st)
 {
     auto kern = sbn::sb_nw_kernel<NCL, GRAD, NU>;
-    if (!allow_max_smem((const void *)kern, m->device, m->smem_optin)) return SB_ECUDA;
+    if (!allow_max_smem((const void *)kern, m->device, m->smem_optin, true)) return SB_ECUDA;
     kern<<<grid, 16 * 32, smem, st>>>(np);
     if (!cuda_ok(cudaGetLastError())) return SB_ECUDA;
     tl_launches += 1;
