@@ -75,3 +75,40 @@ def test_recovers_theta_true_on_noise_free_salt_photometry():
     assert np.all(res["chi2"] <= 1e-8 * start)
     for tr in res["trace"]:
         assert np.all(np.diff(tr) <= 0.0)  # monotone chi^2
+
+
+def _pairs(rng, n, m):
+    """m curvature pairs of a random SPD quadratic (y = H s, so s.y > 0), oldest first."""
+    A = rng.normal(size=(n, n))
+    H = A @ A.T + n * np.eye(n)
+    S = [rng.normal(size=n) for _ in range(m)]
+    return S, [H @ s for s in S]
+
+
+def test_two_loop_satisfies_the_secant_equation():
+    """The inverse-Hessian approximation built from pairs (s_i, y_i) maps the NEWEST y to its s, whatever
+    the memory length (Nocedal & Wright eq. 6.6/7.16: H_{k+1} y_k = s_k); two_loop returns -H g."""
+    rng = np.random.default_rng(11)
+    for n, m in ((2, 1), (4, 3), (4, 8), (7, 5)):
+        S, Y = _pairs(rng, n, m)
+        d = lbfgs.two_loop(Y[-1], S, Y)
+        assert np.allclose(d, -S[-1], rtol=0, atol=1e-12 * np.abs(S[-1]).max())
+
+
+def test_two_loop_equals_the_dense_bfgs_update():
+    """two_loop against the definition it is a fast form of: H_0 = gamma I with gamma of the newest pair, then
+    H <- (I - rho s y')H(I - rho y s') + rho s s' for every pair, oldest first (Nocedal & Wright eq. 7.16 and
+    7.20).  A wrong index, sign or loop order in the recursion changes H g for a generic g."""
+    rng = np.random.default_rng(12)
+    for n, m in ((3, 1), (4, 4), (6, 8)):
+        S, Y = _pairs(rng, n, m)
+        gamma = (S[-1] @ Y[-1]) / (Y[-1] @ Y[-1])
+        H = gamma * np.eye(n)
+        for s, y in zip(S, Y):
+            rho = 1.0 / (y @ s)
+            V = np.eye(n) - rho * np.outer(y, s)
+            H = V.T @ H @ V + rho * np.outer(s, s)
+        for _ in range(3):
+            g = rng.normal(size=n)
+            want = -H @ g
+            assert np.allclose(lbfgs.two_loop(g, S, Y), want, rtol=0, atol=1e-11 * np.abs(want).max())
