@@ -194,6 +194,35 @@ int sb_bandflux_grad_host(const sb_model *m, const sb_bands *b, const sb_batch *
                           const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2,
                           void *out_dchi2);
 
+/* sb_chi2_noalloc -- sb_chi2 (same arguments, same outputs, same error codes) for callers that must not
+ * allocate device memory.  Two kinds of caller are meant: a process whose GPU memory has been handed, all of
+ * it, to another component's pool at start-up (an inference server, a framework's caching allocator with the
+ * device filled), so that a cudaMalloc issued from inside this library would fail; and a latency-bound loop
+ * that cannot afford the device-wide synchronisation a cudaMalloc may imply.  sb_chi2 keeps its scratch (the
+ * redshift order of the batch, a few hundred KB) in a workspace it allocates on the first call per stream;
+ * this call keeps the same scratch in a fixed array that is part of the library image instead, so it never
+ * calls cudaMalloc, cudaFree or any allocating library routine.
+ *   Limits       SB_F32 batches only, node-weight formulation only (SB_FORM_TILED is implied; another
+ *                formulation bit -> SB_EINVAL; calls of fewer than 4096 evaluations run the direct kernel,
+ *                which has no scratch, as they do in sb_chi2), batch->pack must be NULL (SB_EINVAL: a pack already makes
+ *                sb_chi2 allocation-free), and batch->n_sn <= SB_NOALLOC_MAX_SN -- a larger batch is refused
+ *                with SB_ELIMIT before anything is enqueued (cut it into several calls).  A model or band set
+ *                the node-weight kernel does not take (more than 64 bands, ...) also gives SB_ELIMIT: there
+ *                is no fall-back to a kernel that would allocate.
+ *   Cost         the array (about 1 MB for SB_NOALLOC_MAX_SN = 131072) is reserved on every GPU on which the
+ *                process loads this library, from load until the process exits, whether or not the call is
+ *                ever made.
+ *   First call   the first call on each device looks up the array's device address (with that device
+ *                current) and remembers it; make that first call during set-up, before starting any stream
+ *                capture.  Later calls on that device do no set-up.
+ *   Sharing      every call on a device uses the SAME array, whatever its stream or host thread, and the
+ *                array keeps what the previous call left in it (the call clears the part that must start at
+ *                zero itself).  Two calls whose GPU work can overlap -- distinct streams with no dependency
+ *                between them -- race on it and give wrong results; order them (same stream, or an event). */
+#define SB_NOALLOC_MAX_SN 131072
+int sb_chi2_noalloc(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+                    const void *fluxerr, void *out_chi2, void *out_flux, void *stream);
+
 /* sb_fit_lbfgs -- device-resident batched fit of (x0, x1, c, t0): every unit (supernova, parameter sample)
  * is one optimiser LANE that minimises its own chi^2 ("fmin_bfgs.py ... optimisation via
  * L-BFGS-B" is one of the paper's two workloads; the paper gives no algorithmic detail, the algorithm is

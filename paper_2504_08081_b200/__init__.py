@@ -11,6 +11,7 @@ from .api import (  # noqa: F401
     SB_FORM_DIRECT,
     SB_FORM_GROUPED,
     SB_FORM_TILED,
+    SB_NOALLOC_MAX_SN,
     FIT_CONVERGED,
     FIT_EXHAUSTED,
     FIT_RUNNING,
@@ -27,6 +28,7 @@ from .api import (  # noqa: F401
     sb_bandflux_grad_host,
     sb_chi2,
     sb_chi2_host,
+    sb_chi2_noalloc,
     sb_fit_lbfgs,
     sb_fit_lbfgs_host,
     sb_load_bandpasses,

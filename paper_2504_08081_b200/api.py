@@ -13,6 +13,7 @@ import numpy as np
 
 SB_F32, SB_F64 = 0, 1
 SB_FORM_DIRECT, SB_FORM_GROUPED, SB_FORM_TILED = 0x100, 0x200, 0x400  # optional formulation bits OR-ed into dtype
+SB_NOALLOC_MAX_SN = 131072  # include/saltband.h: largest n_sn sb_chi2_noalloc accepts
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
 # SALTBAND_LIB=checked loads the bounds-checked build of the same sources (build.py --checked)
@@ -74,6 +75,8 @@ def _load():
     L.sb_bandflux.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp]
     L.sb_chi2.restype = C.c_int
     L.sb_chi2.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp, vp]
+    L.sb_chi2_noalloc.restype = C.c_int
+    L.sb_chi2_noalloc.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp, vp]
     L.sb_bandflux_grad.restype = C.c_int
     L.sb_bandflux_grad.argtypes = [vp, vp, C.POINTER(_Batch), vp, vp, vp, vp, vp, vp, vp]
     L.sb_pack_observations.restype = C.c_int
@@ -281,6 +284,27 @@ def sb_chi2(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int
                          _ptr(out_chi2, ft, n_sn * n_samples, "out_chi2"),
                          _ptr(out_flux, ft, n_obs_total * n_samples, "out_flux", allow_none=True), _stream())
     _check(rc, "sb_chi2")
+
+
+def sb_chi2_noalloc(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,
+                    obs_offset, time, band, zp, z, x0, x1, c, t0, flux, fluxerr, out_chi2, out_flux=None) -> None:
+    """include/saltband.h: sb_chi2_noalloc -- sb_chi2 for a caller that must not allocate device memory (its
+    GPU memory all belongs to another pool, or it cannot take cudaMalloc's synchronisation).  fp32 only, no
+    pack, n_sn <= SB_NOALLOC_MAX_SN (SaltbandError 'table exceeds ...' beyond).  All calls on a device share
+    one fixed scratch array inside the library: keep them ordered on the GPU (one stream, or events) -- calls
+    that overlap there race.  The first call on a device also looks up that array's address; make it during
+    set-up.  The tensors passed here are the caller's own, as for sb_chi2."""
+    import torch
+
+    if (dtype & 0xFF) != SB_F32:
+        raise ValueError("sb_chi2_noalloc is fp32 only")
+    ft = torch.float32
+    bt = _batch(dtype, n_sn, n_samples, obs_offset, time, band, zp, z, x0, x1, c, t0, n_obs_total, None)
+    rc = _load().sb_chi2_noalloc(model._h, bands._h, C.byref(bt), _ptr(flux, ft, n_obs_total, "flux"),
+                                 _ptr(fluxerr, ft, n_obs_total, "fluxerr"),
+                                 _ptr(out_chi2, ft, n_sn * n_samples, "out_chi2"),
+                                 _ptr(out_flux, ft, n_obs_total * n_samples, "out_flux", allow_none=True), _stream())
+    _check(rc, "sb_chi2_noalloc")
 
 
 def sb_bandflux_grad(model: Model, bands: Bands, *, dtype: int, n_sn: int, n_samples: int, n_obs_total: int,

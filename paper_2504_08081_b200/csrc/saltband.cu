@@ -811,6 +811,94 @@ int sb_chi2(const sb_model *m, const sb_bands *b, const sb_batch *batch, const v
     return run(m, b, batch, flux, fluxerr, out_flux, nullptr, out_chi2, nullptr, stream, false);
 }
 
+} // extern "C"
+
+// ---------------------------------------------------------------- sb_chi2_noalloc
+// Scratch of the allocation-free chi^2 call: the z-order workspace (ZWork layout) of a batch of up to
+// SB_NOALLOC_MAX_SN supernovae, as a fixed array in the library image.  Each GPU that loads the library holds
+// its own copy until the process exits.  In HOST code the name below is only a handle for the runtime -- it is
+// not a device address and must never be handed to a kernel or to cudaMemsetAsync; noalloc_scratch() asks the
+// runtime for the real address on the current device.
+constexpr size_t kNoAllocBytes = 4096 + (((sizeof(int32_t) * (size_t)SB_NOALLOC_MAX_SN) + 255) & ~(size_t)255) +
+                                 sizeof(uint32_t) * (size_t)sbh::kZSegs * sbh::kZBins;
+static __device__ __align__(256) unsigned char sb_noalloc_scratch[kNoAllocBytes];
+
+namespace {
+
+// Device address of sb_noalloc_scratch on `device`, which must be the current device.  Looked up once per
+// device (cudaGetSymbolAddress; the first lookup also makes the runtime load this module on that device) and
+// cached; NULL on failure, with the CUDA error left in tl_cuda_err.
+unsigned char *noalloc_scratch(int device)
+{
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static unsigned char *addr[kMaxDev] = {};
+    if (device < 0 || device >= kMaxDev) { tl_cuda_err = (int32_t)cudaErrorInvalidDevice; return nullptr; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[device]) {
+        void *p = nullptr;
+        if (!cuda_ok(cudaGetSymbolAddress(&p, sb_noalloc_scratch)) || !p) return nullptr;
+        addr[device] = static_cast<unsigned char *>(p);
+    }
+    return addr[device];
+}
+
+} // namespace
+
+extern "C" {
+
+int sb_chi2_noalloc(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
+                    const void *fluxerr, void *out_chi2, void *out_flux, void *stream)
+{
+    NvtxRange nvtx("sb_chi2_noalloc");
+    tl_launches = 0;
+    tl_form = 0;
+    if (!m || !b || !batch) return SB_EINVAL;
+    // the size limit of the fixed array comes first: refused before anything else is looked at or enqueued
+    if (batch->n_sn > SB_NOALLOC_MAX_SN) return SB_ELIMIT;
+    if ((!out_chi2 || !flux || !fluxerr) && batch->n_sn != 0) return SB_EINVAL;
+    if (batch->pack) return SB_EINVAL; // with a pack sb_chi2 itself allocates nothing
+    constexpr int32_t kForms = SB_FORM_DIRECT | SB_FORM_GROUPED | SB_FORM_TILED;
+    const int32_t form = batch->dtype & kForms;
+    if ((batch->dtype & ~kForms) != SB_F32 || (form != 0 && form != SB_FORM_TILED)) return SB_EINVAL;
+    if (batch->n_sn < 0) return SB_EINVAL;
+    if (ZWork(batch->n_sn).bytes > kNoAllocBytes) return SB_ELIMIT; // cannot happen while the layouts agree
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return SB_ECUDA;
+    if (dev != m->device || dev != b->device) return SB_EINVAL;
+    unsigned char *ws = noalloc_scratch(dev);
+    if (!ws) return SB_ECUDA;
+    // Run the unchanged sb_chi2 path with the fixed array standing where a pack's redshift order stands: the
+    // permutation is rebuilt into the array by this call (enqueue_zorder clears the counters it needs at zero
+    // and overwrites the rest), there is no item geometry (d_geom NULL: the kernel computes it, as it does
+    // without a pack), and SB_FORM_TILED makes run() return SB_ELIMIT rather than fall through to a kernel
+    // that would take a workspace from scratch_for().  A single supernova needs no order at all.
+    // Batches too small for that kernel (the same threshold as sb_chi2's own choice) go to the direct kernel,
+    // which uses no scratch.
+    sb_pack view;
+    memset(&view, 0, sizeof(view));
+    sb_batch bt = *batch;
+    const bool tiny = (long long)bt.n_obs_total * bt.n_samples < 4096;
+    bt.dtype = SB_F32 | (tiny ? SB_FORM_DIRECT : SB_FORM_TILED);
+    int32_t sort_launches = 0;
+    if (bt.n_sn > 1 && !tiny) {
+        if (!bt.z) return SB_EINVAL;
+        view.n_sn = bt.n_sn;
+        view.n_bands = b->n_bands;
+        view.model = m;
+        view.bands = b;
+        view.z = bt.z;
+        view.device = dev;
+        view.d_perm = reinterpret_cast<int32_t *>(ws + ZWork(bt.n_sn).perm_off);
+        const int rc = enqueue_zorder((const float *)bt.z, bt.n_sn, ws, (cudaStream_t)stream, &sort_launches);
+        if (rc != SB_OK) return rc;
+        bt.pack = &view;
+    }
+    const int rc = run(m, b, &bt, flux, fluxerr, out_flux, nullptr, out_chi2, nullptr, stream, false);
+    if (rc == SB_OK) tl_launches += sort_launches;
+    return rc;
+}
+
 int sb_bandflux_grad(const sb_model *m, const sb_bands *b, const sb_batch *batch, const void *flux,
                      const void *fluxerr, void *out_flux, void *out_dflux, void *out_chi2, void *out_dchi2,
                      void *stream)
