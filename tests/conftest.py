@@ -15,13 +15,9 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: test needs a CUDA device (run with -m gpu on a B200)")
 
 
-def pytest_collection_modifyitems(config, items):
-    """GPU tests fail loudly (not skip) on a GPU box; on a CPU box they are deselected by -m."""
-    return
-
-
 @pytest.fixture(scope="session")
 def cuda_device():
+    """GPU tests fail loudly (never skip) without a device; on a CPU box they are deselected by -m "not gpu"."""
     import torch
 
     if not torch.cuda.is_available():

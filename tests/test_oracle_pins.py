@@ -218,7 +218,9 @@ def test_p9_zero_point_ratios():
     m25 = oracle.eval_one(m, bd, 0.1, 1.3, 0, 25.0, 1e-5, 0.4, 0.03, 0.0)
     m275 = oracle.eval_one(m, bd, 0.1, 1.3, 0, 27.5, 1e-5, 0.4, 0.03, 0.0)
     assert rel(m275, 10.0 * m25) < 1e-14
-    # ZPAB written out independently with numpy's trapezoid of (AB_FNU/h) T / lam
+    # ZPAB written out with numpy's trapezoid of (AB_FNU/h) T / lam.  This restates the oracle's own formula
+    # with a library routine, so it only guards the plumbing (band indexing, constants); the PIN of sbo_zpab is
+    # P10 below (closed form of the top-hat integral), and the 10^(0.4 zp) / ZPAB ratios asserted here.
     zpab = np.trapezoid(AB_FNU / H_PLANCK * tr / w, w)
     assert rel(bd.zpab(0), zpab) < 1e-14
     assert rel(m25 / raw, 10.0 ** 10 / zpab) < 1e-14
