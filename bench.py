@@ -674,8 +674,9 @@ def main():
         cpu["single_thread"] = {"value": v1, "unit": UNIT, "cores": 1, "sample": sample1, "seconds": sec1}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-        "data": "synthetic",
+        "ms_per_step": ms_per_step, "ms_per_step_median": float(np.median(per_step_ms)),
+        "ms_per_step_min": float(per_step_ms.min()), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": wl.name, "n_sn": wl.n_sn, "n_samples": ns, "n_obs_total": n_tot, "n_evals": n_ev,
                    "mode": args.mode, "form": form_run, "pack": bool(args.pack), "band_jitter": args.band_jitter, "chi2_evals_per_sec": n_units * world * steps / (total_ms * 1e-3),
                    "l2": "inputs+outputs %.0f MB > 126 MB L2, no flush" % ((in_bytes + out_bytes) / 1e6) if not need_flush

@@ -76,8 +76,8 @@ typedef enum { SB_F32 = 0, SB_F64 = 1 } sb_dtype;
  *   SB_FORM_TILED    the node-weight kernel (csrc/sb_nw.cuh): as SB_FORM_GROUPED, and the observations
  *                    of a group of units that are neighbours in redshift are ordered by phase so
  *                    that the model rows they read stay in registers; fp32
- *                    forward AND gradient calls with uniform band grids, same error behaviour.
- *                    The only formulation that uses sb_batch.pack. */
+ *                    forward AND gradient calls, uniform or non-uniform band grids, at most 64 bands;
+ *                    same error behaviour.  The only formulation that uses sb_batch.pack. */
 enum { SB_FORM_DIRECT = 0x100, SB_FORM_GROUPED = 0x200, SB_FORM_TILED = 0x400 };
 
 typedef enum {
@@ -139,9 +139,11 @@ typedef struct {
  * only) and the DEVICE array batch->z; the other fields are ignored.  Allocates the pack's device
  * memory and enqueues its build on `stream` (no host synchronisation: use the pack on the same
  * stream, or synchronise first).  A compute call whose batch points to the pack must pass the
- * same n_sn, model and bands (else SB_EINVAL) and the same z values (not checked).  Kernels that
- * do not use a pack (fp64, SB_FORM_DIRECT, SB_FORM_GROUPED) ignore it.  SB_ELIMIT when the band set is
- * one the node-weight kernel does not handle (non-uniform band grids, more than 64 bands). */
+ * same n_sn, model and bands and the same device array z it was built from (else SB_EINVAL: the
+ * pack holds geometry computed from those redshifts; the pointer is compared, the values are not, so do
+ * not overwrite z in place between the build and the last use).  Kernels that do not use a pack (fp64,
+ * SB_FORM_DIRECT, SB_FORM_GROUPED) ignore it.  SB_ELIMIT when the band set is one the node-weight kernel
+ * does not handle (more than 64 bands); non-uniform band grids are fine. */
 int sb_pack_observations(const sb_model *m, const sb_bands *b, const sb_batch *batch, void *stream,
                          sb_pack **out);
 void sb_free_pack(sb_pack *p); /* NULL is allowed; free after the work that uses it has finished */
@@ -245,7 +247,11 @@ int sb_chi2_noalloc(const sb_model *m, const sb_bands *b, const sb_batch *batch,
  *                  fp64: chi^2 after i accepted steps (row 0: start point; NaN where not reached).
  * A lane converges when an accepted step lowers chi^2 by <= ftol * max(|chi2_old|, |chi2_new|, 1) or
  * when max_k |d chi^2 / d u_k| <= gtol.  In SB_F32 batches every trial point is rounded to fp32 (the
- * kernels take fp32 parameters); lane state and all optimiser arithmetic are fp64.  Lane state lives in a
+ * kernels take fp32 parameters) and chi^2 comes back in fp32, so a decrease below a few fp32 ulps cannot be
+ * observed: there a positive ftol below 2^-21 (4.8e-7) is raised to 2^-21 (the default 1e-12 included);
+ * ftol = 0 switches the test off in either precision.  Lane state and all optimiser arithmetic are fp64.
+ * With a box, every evaluated and every returned theta satisfies lo <= theta <= hi exactly in the batch's
+ * element type (the point is clamped again after scaling and rounding).  Lane state lives in a
  * workspace owned by the sb_bands handle (one per stream, as for the compute calls; ~0.7 KB per lane).
  * Errors as for the compute calls; SB_EINVAL for out-of-range options. */
 typedef struct {
@@ -253,7 +259,7 @@ typedef struct {
     int32_t max_eval;  /* evaluations per lane = steps enqueued, >= 1 (default 60) */
     int32_t max_iter;  /* accepted steps per lane, >= 1 (default 1000) */
     int32_t trace_len; /* rows of result->trace (0: no trace) */
-    double ftol, gtol; /* >= 0 (defaults 1e-12, 0) */
+    double ftol, gtol; /* >= 0 (defaults 1e-12, 0; SB_F32 batches: see the ftol floor above) */
     const double *lo, *hi; /* HOST [4] box on (x0, x1, c, t0) in theta units, or NULL: no bound on that side */
 } sb_fit_opts;
 

@@ -250,6 +250,9 @@ int sb_load_model(const double *phase, int32_t n_phase, const double *wave, int3
             return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
         }
     }
+    // the uploads above are cudaMemcpy from pageable memory (they may return once the data is staged): make the
+    // tables complete before a compute call on a non-blocking stream, which is not ordered after them, reads them
+    if (!cuda_ok(cudaDeviceSynchronize())) { sb_free_model(h); return SB_ECUDA; }
     *out = h;
     return SB_OK;
 }
@@ -342,6 +345,7 @@ int sb_load_bandpasses(int32_t n_bands, const int64_t *offset, const double *wav
         sb_free_bands(h);
         return tl_cuda_err == (int32_t)cudaErrorMemoryAllocation ? SB_ENOMEM : SB_ECUDA;
     }
+    if (!cuda_ok(cudaDeviceSynchronize())) { sb_free_bands(h); return SB_ECUDA; } // as in sb_load_model
     *out = h;
     return SB_OK;
 }
@@ -604,6 +608,7 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     if (pk) {
         if (pk->model != m || pk->bands != b || pk->n_sn != bt->n_sn || pk->n_bands != b->n_bands || pk->device != m->device)
             return SB_EINVAL;
+        if (pk->z != bt->z) return SB_EINVAL; // the pack's geometry belongs to the redshift array it was built from
         perm = pk->d_perm;
         geom = reinterpret_cast<const sbn::NItem *>(pk->d_geom);
     } else if (bt->n_sn > 1) {
@@ -650,7 +655,6 @@ int launch_nw(bool grad, const sb_model *m, const sb_bands *b, const sb_batch *b
     np.n_live = lv.n_live;
     np.n_groups = (int32_t)n_groups;
     np.cap = cap;
-    { const char *e = getenv("SB_NW_MIX"); np.mix = e ? atoi(e) : 3; }
     const int grid = (int)(n_groups < (long long)n_cta ? n_groups : (long long)n_cta);
     const bool small_cl = m->prm.n_cl <= 5;
     if (nu) {
@@ -1113,6 +1117,8 @@ int sb_bandflux_grad_host(const sb_model *m, const sb_bands *b, const sb_batch *
 // ------------------------------------------------------------------------------------------
 namespace {
 
+constexpr double kFtolFloorF32 = 4.76837158203125e-7; // 2^-21 = 8 fp32 ulps of chi^2 (include/saltband.h: sb_fit_lbfgs)
+
 struct FitLayout { // carve-up of the fit workspace (kScratchFit slot of the call's stream)
     size_t theta[4], chi2, dchi2, u, g, d, ut, f, alpha, scale, S, Y, ints[7], n_live, bytes;
     FitLayout(size_t n, size_t es, int memory)
@@ -1179,6 +1185,9 @@ int fit_device(const sb_model *m, const sb_bands *b, const sb_batch *bt_in, cons
     F.n = (int32_t)n_units;
     F.memory = opts->memory; F.max_eval = opts->max_eval; F.max_iter = opts->max_iter; F.trace_len = opts->trace_len;
     F.ftol = opts->ftol; F.gtol = opts->gtol;
+    // SB_F32: chi^2 comes back from the kernels in fp32, so a decrease of less than a few of its ulps cannot be
+    // observed; a positive ftol below that resolution would never be met before the line search stalls
+    if (base == SB_F32 && F.ftol > 0.0 && F.ftol < kFtolFloorF32) F.ftol = kFtolFloorF32;
     F.has_box = (opts->lo || opts->hi) ? 1 : 0;
     for (int k = 0; k < 4; ++k) {
         F.lo[k] = opts->lo ? opts->lo[k] : -INFINITY;
@@ -1313,7 +1322,10 @@ int sb_fit_lbfgs_host(const sb_model *m, const sb_bands *b, const sb_batch *hb, 
     if (hb->zp) h2d(o_zp, hb->zp, es * nob);
     h2d(o_flux, flux, es * nob); h2d(o_err, fluxerr, es * nob); h2d(o_z, hb->z, es * nsn);
     h2d(o_x0, hb->x0, es * nun); h2d(o_x1, hb->x1, es * nun); h2d(o_c, hb->c, es * nun); h2d(o_t0, hb->t0, es * nun);
-    if (rc != SB_OK) return rc;
+    if (rc != SB_OK) { // copies enqueued before the failing one may still read the caller's buffers: drain first
+        cudaStreamSynchronize(st);
+        return rc;
+    }
     sb_batch db = *hb;
     db.obs_offset = (const int32_t *)(D + o_off); db.band = (const int32_t *)(D + o_band); db.time = D + o_time;
     db.zp = hb->zp ? D + o_zp : nullptr; db.z = D + o_z; db.x0 = D + o_x0; db.x1 = D + o_x1; db.c = D + o_c; db.t0 = D + o_t0;

@@ -79,12 +79,28 @@ __device__ __forceinline__ void project(const FitParams &F, const double (&sc)[4
     }
 }
 
+// theta_k = u_k s_k in the batch's element type, INSIDE the box: the projection above works in u, and both
+// (lo/s) s and the rounding to T can land one ulp outside [lo, hi]; clamp in theta units and, where the cast
+// crosses a bound, step to the neighbouring value of T on the inside.
+template <typename T> __device__ __forceinline__ T to_theta(const FitParams &F, int k, double u, double s)
+{
+    double th = mul(u, s);
+    if (!F.has_box) return (T)th;
+    th = fmin(fmax(th, F.lo[k]), F.hi[k]);
+    T r = (T)th;
+    if constexpr (sizeof(T) == 4) {
+        if ((double)r < F.lo[k]) r = nextafterf(r, INFINITY);
+        else if ((double)r > F.hi[k]) r = nextafterf(r, -INFINITY);
+    }
+    return r;
+}
+
 template <typename T> __device__ __forceinline__ void store_theta(const FitParams &F, int i, const double (&v)[4], const double (&sc)[4])
 {
-    static_cast<T *>(F.x0)[i] = (T)mul(v[0], sc[0]);
-    static_cast<T *>(F.x1)[i] = (T)mul(v[1], sc[1]);
-    static_cast<T *>(F.c)[i] = (T)mul(v[2], sc[2]);
-    static_cast<T *>(F.t0)[i] = (T)mul(v[3], sc[3]);
+    static_cast<T *>(F.x0)[i] = to_theta<T>(F, 0, v[0], sc[0]);
+    static_cast<T *>(F.x1)[i] = to_theta<T>(F, 1, v[1], sc[1]);
+    static_cast<T *>(F.c)[i] = to_theta<T>(F, 2, v[2], sc[2]);
+    static_cast<T *>(F.t0)[i] = to_theta<T>(F, 3, v[3], sc[3]);
 }
 
 // Start: u = P(theta_start / s), trial theta = u s; every lane live.
@@ -260,7 +276,7 @@ template <typename T> __global__ void __launch_bounds__(128) sb_fit_update_kerne
         if (F.theta_out) {
             T *o = static_cast<T *>(F.theta_out) + 4 * (size_t)i;
 #pragma unroll
-            for (int k = 0; k < 4; ++k) o[k] = (T)mul(u[k], sc[k]);
+            for (int k = 0; k < 4; ++k) o[k] = to_theta<T>(F, k, u[k], sc[k]);
         }
         if (F.chi2_out) static_cast<T *>(F.chi2_out)[i] = (T)f;
         if (F.status_out) F.status_out[i] = status;

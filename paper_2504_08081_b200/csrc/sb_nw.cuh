@@ -8,7 +8,7 @@
 // observation).  At depends on (unit, band) only -- an ITEM -- and is shared by all
 // observations of the item.
 //
-// Work decomposition.  The units (supernova x sample) are taken in redshift order (sb_pack.cuh) and cut
+// Work decomposition.  The units (supernova x sample) are taken in redshift order (sb_zorder_* kernels of sb_hoist.cuh) and cut
 // into GROUPS of z-neighbours; CTA c of a persistent grid owns groups c, c + gridDim, ... (static: no
 // counter, no per-call mutable state).  A group is processed in ROUNDS of at most `cap` observations and
 // `NSL` units.  Per round:
@@ -73,7 +73,7 @@ template <int NW> struct Cfg {
 };
 
 // Geometry of one item (supernova, band): depends on z and the band only (never on theta), so the pack
-// (sb_pack.cuh) can hold it.  64 bytes, loaded as four 16-byte words.
+// (sb_pack_observations, saltband.cu) can hold it.  64 bytes, loaded as four 16-byte words.
 struct __align__(16) NItem {
     int32_t n_in;    // in-range band samples (0: nothing to do)
     int32_t ncell;   // model cells spanned
@@ -156,7 +156,6 @@ struct SbNParams {
     const int32_t *live, *n_live;     // fit driver: [n_units] 0 = skip the unit; [1] 0 = nothing to do (or NULL)
     int32_t n_groups;                 // groups: unit range of group i = [i n_units / n_groups, (i+1) n_units / n_groups)
     int32_t cap;                      // observations per round
-    int32_t mix;                      // which warps start a super-step with phase A (experiment knob)
 };
 
 // Shared-memory accesses of the hot loops go through 32-bit shared-state-space addresses (one cvta at
@@ -1033,12 +1032,11 @@ __global__ void __launch_bounds__(16 * 32, 1) sb_nw_kernel(const __grid_constant
             while (st_n < n_bst && (nws_n = n_wseg_of(st_n)) == 0) ++st_n;
             int buf = 0;
             // A super-step of a warp is three tasks: its (up to) two items of phase A and its chunk of phase B.
-            // Where the chunk sits among them depends on the warp (P.mix: 0 last in all warps; 1 first in the
-            // warps of two schedulers; 2 first in two warps of every scheduler; 3 first / middle / last / middle in
-            // the four warps of a scheduler), so that both kinds of work are in flight on every scheduler
+            // Where the chunk sits among them depends on the warp: first / middle / last / middle in the four
+            // warps of a scheduler, so that both kinds of work are in flight on every scheduler (the measured
+            // best of four orders)
             const int wsch = (warp >> 2) & 3; // index of the warp among the warps of its scheduler
-            const int bpos = P.mix == 0 ? 2 : P.mix == 1 ? ((warp & 2) ? 0 : 2) : P.mix == 2 ? ((wsch & 1) ? 0 : 2)
-                                                                               : (wsch == 0 ? 0 : wsch == 2 ? 2 : 1);
+            const int bpos = wsch == 0 ? 0 : wsch == 2 ? 2 : 1;
             while (st_n < n_bst || st_c < n_bst) {
 #pragma unroll 1
                 for (int task = 0; task < 3; ++task) {

@@ -117,31 +117,113 @@ def chi2_tolerance(wl, flux_ref: np.ndarray, tol_flux: np.ndarray, n_samples: in
     return out
 
 
-def grad_tolerance(wl, ref: Dict[str, np.ndarray], th: Dict[str, np.ndarray], n_samples: int, fp64: bool):
+def _stencil(u_all: np.ndarray, n: int):
+    """Dense interpolation weights of reading G1-G3 for grid coordinates u (in units of the grid step):
+    Keys a = -1/2 in interior cells, linear in the first and last cell, zero outside [0, n-1].  Returns
+    (W, dW), each [len(u), n]: value and d/du weights.  Tolerance helper only (checked against
+    oracle.Model.surface by tests/test_tolerance_helpers.py); no expected value comes from here."""
+    u_all = np.asarray(u_all, dtype=np.float64)
+    W = np.zeros((len(u_all), n))
+    dW = np.zeros_like(W)
+    ok = (u_all >= 0.0) & (u_all <= n - 1)
+    idx = np.nonzero(ok)[0]
+    u = u_all[idx]
+    i = np.minimum(np.floor(u).astype(np.int64), n - 2)
+    t = u - i
+    border = (i == 0) | (i == n - 2)
+    kb, ki = idx[border], idx[~border]
+    W[kb, i[border]] = 1.0 - t[border]
+    W[kb, i[border] + 1] = t[border]
+    dW[kb, i[border]] = -1.0
+    dW[kb, i[border] + 1] = 1.0
+    ti, ii = t[~border], i[~border]
+    t2, t3 = ti * ti, ti * ti * ti
+    for off, w, d in ((-1, (-t3 + 2 * t2 - ti) / 2, (-3 * t2 + 4 * ti - 1) / 2), (0, (3 * t3 - 5 * t2 + 2) / 2, (9 * t2 - 10 * ti) / 2),
+                      (1, (-3 * t3 + 4 * t2 + ti) / 2, (-9 * t2 + 8 * ti + 1) / 2), (2, (t3 - t2) / 2, (3 * t2 - 2 * ti) / 2)):
+        W[ki, ii + off] = w
+        dW[ki, ii + off] = d
+    return W, dW
+
+
+def grad_term_sums(wl, th: Dict[str, np.ndarray], n_samples: int, use_zp: bool = True, row_terms: bool = True) -> np.ndarray:
+    """[n_evals][4]: the sum of ABSOLUTE terms of each derivative's band integral (0 for x0), in out_flux order.
+    With g_r[j] = the wavelength-interpolated model row r at band sample j, W_r / dW_r the phase weights and
+    their derivatives, E = exp(c CL), k = T lam/(hc), w_j the trapezoid weights, S the zero-point factor:
+        A_x1 = S x0 sum_j sum_r w_j |W_r M1_r[j]| E k,   A_c = S x0 sum_j sum_r w_j |W_r (M0 + x1 M1)_r[j] CL_j| E k,
+        A_t0 = S x0/((1+z) dP) sum_j sum_r w_j |dW_r (M0 + x1 M1)_r[j]| E k
+    (a derivative whose terms change sign is held to its sum of absolute term sizes, never to a
+    cancelling total).  The phase rows are terms of their own: sum_r dW_r = 0, so dM/dp is a difference of
+    neighbouring rows and cancels by construction, in ANY evaluation order.  row_terms=False takes the absolute
+    value per sample after summing the rows (a smaller sum that ignores that cancellation; reported, not
+    asserted).  The colour law and ZPAB come from the oracle's exposed pieces; the surfaces are interpolated
+    here with _stencil."""
+    import oracle
+
+    md, bd = wl.model, wl.bands
+    om, ob = oracle.Model.from_dict(md), oracle.Bands.from_dict(bd)
+    phase, wave = np.asarray(md["phase"], dtype=np.float64), np.asarray(md["wave"], dtype=np.float64)
+    m0, m1 = np.asarray(md["m0"], dtype=np.float64), np.asarray(md["m1"], dtype=np.float64)
+    n_p, n_w = len(phase), len(wave)
+    dp, dw = (phase[-1] - phase[0]) / (n_p - 1), (wave[-1] - wave[0]) / (n_w - 1)
+    hc = 6.62607015e-27 * 2.99792458e18
+    off = np.asarray(bd["offset"], dtype=np.int64)
+    n_bands = len(off) - 1
+    zpab = [ob.zpab(b) for b in range(n_bands)]
+    out = np.zeros((int(wl.obs_offset[-1]) * n_samples, 4))
+    for s in range(wl.n_sn):
+        a, e = int(wl.obs_offset[s]), int(wl.obs_offset[s + 1])
+        n_obs = e - a
+        if n_obs == 0:
+            continue
+        opz = 1.0 + float(wl.z[s])
+        bs = np.asarray(wl.band[a:e])
+        tt = np.asarray(wl.time[a:e], dtype=np.float64)
+        for b in np.unique(bs):
+            if b < 0 or b >= n_bands:
+                continue
+            lam, tr = np.asarray(bd["wave"][off[b]:off[b + 1]], dtype=np.float64), np.asarray(bd["trans"][off[b]:off[b + 1]], dtype=np.float64)
+            w = np.zeros_like(lam)
+            w[:-1] += 0.5 * np.diff(lam)
+            w[1:] += 0.5 * np.diff(lam)
+            lr = lam / opz
+            Wl, _ = _stencil((lr - wave[0]) / dw, n_w)            # [n_lam][n_wave]
+            g0, g1 = m0 @ Wl.T, m1 @ Wl.T                          # [n_phase][n_lam]
+            cl = np.array([om.colour_law(float(x)) for x in lr])
+            wk = w * tr * lam / hc
+            sel = np.nonzero(bs == b)[0]
+            for k in range(n_samples):
+                u = s * n_samples + k
+                x0, x1, c, t0 = (float(th[q][u]) for q in ("x0", "x1", "c", "t0"))
+                Wp, dWp = _stencil(((tt[sel] - t0) / opz - phase[0]) / dp, n_p)  # [n_sel][n_phase]
+                ek = np.exp(c * cl) * wk
+                sc = np.ones(len(sel))
+                if use_zp:
+                    sc = 10.0 ** (0.4 * np.asarray(wl.zp[a:e], dtype=np.float64)[sel]) / zpab[b]
+                rows = a * n_samples + k * n_obs + sel
+                g01 = g0 + x1 * g1
+                if row_terms:  # |W_r| |g_r[j]|: absolute value of every (phase row, sample) term
+                    out[rows, 1] = sc * abs(x0) * ((np.abs(Wp) @ np.abs(g1)) @ ek)
+                    out[rows, 2] = sc * abs(x0) * (((np.abs(Wp) @ np.abs(g01)) * np.abs(cl)) @ ek)
+                    out[rows, 3] = sc * abs(x0) / opz * (((np.abs(dWp) @ np.abs(g01)) / dp) @ ek)
+                else:          # |sum_r W_r g_r[j]|: absolute value per sample, rows summed first
+                    out[rows, 1] = sc * abs(x0) * (np.abs(Wp @ g1) @ ek)
+                    out[rows, 2] = sc * abs(x0) * (np.abs((Wp @ g01) * cl) @ ek)
+                    out[rows, 3] = sc * abs(x0) / opz * (np.abs((dWp @ g01) / dp) @ ek)
+    return out
+
+
+def grad_tolerance(wl, ref: Dict[str, np.ndarray], th: Dict[str, np.ndarray], n_samples: int, fp64: bool,
+                   use_zp: bool = True):
     """Tolerance of d m/d(x0, x1, c, t0) (reading G13a): rel * (|dm| + A) + floor * peak/scale.
 
-    The derivative integrands change sign inside the band (CL crosses zero at lambda_B, dM/dp at
-    maximum light, M1 oscillates), so the integral can cancel far below the sum of its absolute
-    terms, and rounding error scales with that sum, not with the total.  A is that non-cancelling
-    magnitude: 0 for x0, |m| for x1 and c (|M1| <~ |M0|, |CL| = O(1)), |m|/(dP (1+z)) for t0."""
+    The derivative integrands change sign inside the band (CL crosses zero at lambda_B, dM/dp at maximum
+    light, M1 oscillates), so the integral can cancel far below the sum of its absolute terms, and rounding
+    error scales with that sum, not with the total.  A is that sum, MEASURED per evaluation by
+    grad_term_sums (0 for x0, whose integrand is the flux integrand itself)."""
     rel, floor = (1e-12, 1e-15) if fp64 else (1e-5, 1e-9)
     peak = unit_peaks(wl, ref["flux"], n_samples)
-    m = np.abs(ref["flux"])
-    dp = float(wl.model["phase"][1] - wl.model["phase"][0])
-    scale = np.empty((len(ref["flux"]), 4))
-    opz = np.empty(len(ref["flux"]))
-    for s in range(wl.n_sn):
-        a, b = int(wl.obs_offset[s]), int(wl.obs_offset[s + 1])
-        n_obs = b - a
-        opz[a * n_samples:b * n_samples] = 1.0 + float(wl.z[s])
-        for k in range(n_samples):
-            u = s * n_samples + k
-            sl = slice(a * n_samples + k * n_obs, a * n_samples + (k + 1) * n_obs)
-            scale[sl, 0] = abs(th["x0"][u])
-            scale[sl, 1] = max(abs(th["x1"][u]), 1.0)
-            scale[sl, 2] = max(abs(th["c"][u]), 1.0)
-            scale[sl, 3] = max(abs(th["t0"][u]), 1.0)
-    A = np.stack([np.zeros_like(m), m, m, m / (dp * opz)], axis=1)
+    scale = _theta_scale(wl, th, n_samples, len(ref["flux"]))
+    A = grad_term_sums(wl, th, n_samples, use_zp)
     return rel * (np.abs(ref["dflux"]) + A) + floor * peak[:, None] / scale
 
 
@@ -156,14 +238,12 @@ def grad_tolerance_strict(wl, ref: Dict[str, np.ndarray], th: Dict[str, np.ndarr
     return rel[None, :] * np.abs(ref["dflux"]) + floor * peak[:, None] / scale
 
 
-def grad_conditioning(wl, ref: Dict[str, np.ndarray], n_samples: int) -> np.ndarray:
-    """|dm/dtheta| / A per evaluation and component (A = the non-cancelling magnitude of grad_tolerance;
-    inf for x0, whose integrand is the flux integrand itself): small values mean the derivative integral
-    cancels and no tolerance relative to the total can hold in fp32 (reading G13a)."""
-    m = np.abs(ref["flux"])
-    dp = float(wl.model["phase"][1] - wl.model["phase"][0])
-    opz = np.repeat(1.0 + wl.z.astype(np.float64), np.diff(wl.obs_offset) * n_samples)
-    A = np.stack([np.zeros_like(m), m, m, m / (dp * opz)], axis=1)
+def grad_conditioning(wl, ref: Dict[str, np.ndarray], th: Dict[str, np.ndarray], n_samples: int) -> np.ndarray:
+    """|dm/dtheta| / A per evaluation and component (A = grad_term_sums, the sum of absolute terms of the
+    derivative integral; inf for x0, whose integrand is the flux integrand itself): 1 means no cancellation,
+    small values mean the integral cancels and no tolerance relative to the total can hold in fp32
+    (reading G13a)."""
+    A = grad_term_sums(wl, th, n_samples)
     with np.errstate(divide="ignore", invalid="ignore"):
         return np.where(A > 0, np.abs(ref["dflux"]) / A, np.inf)
 

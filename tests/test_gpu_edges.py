@@ -180,3 +180,22 @@ def test_p17_scale_invariance_fp32(cuda_device, kappa):
     x0_ratio = th["x0"].astype(np.float64) * kappa / wl.theta["x0"].astype(np.float64)  # fp32 rounding of x0/kappa
     b = b / np.repeat(x0_ratio, np.diff(wl.obs_offset))
     assert np.all(np.abs(a - b) <= 2e-6 * np.abs(a) + 1e-9 * np.max(np.abs(a)))
+
+
+@pytest.mark.parametrize("config", [1, 5])
+def test_zpab_of_the_loader_equals_the_oracle(cuda_device, config):
+    """a0 / reading G7: ZPAB_b as sb_load_bandpasses computes it at load (fp64 host arithmetic, folded
+    weights) against the oracle's literal trapezoid of the AB spectrum through the band, for every band of
+    configs 1 and 5 (optical and NIR), and on jittered (non-uniform) grids of the same bands."""
+    for jitter in (0.0, 0.3):
+        wl = workloads.make_workload(config, **({"n_sn": 4} if config == 5 else {}))
+        if jitter:
+            wl.bands = workloads.jitter_band_grids(wl.bands, jitter)
+        _, bands = sbgpu.load_handles(wl)
+        ob = oracle.Bands.from_dict(wl.bands)
+        n_bands = len(wl.bands["offset"]) - 1
+        assert bands.n_bands == n_bands
+        for b in range(n_bands):
+            want = ob.zpab(b)
+            assert want > 0 and abs(bands.zpab(b) - want) <= 1e-14 * want, (config, jitter, b)
+        assert np.isnan(bands.zpab(n_bands)) and np.isnan(bands.zpab(-1))

@@ -170,3 +170,35 @@ def test_host_call_graph_replay_and_budget(cuda_device):
     stream.synchronize()
     assert np.array_equal(theta.cpu().numpy().astype(np.float64), dev["theta"])
     assert np.array_equal(chi2.cpu().numpy().astype(np.float64), dev["chi2"])
+
+
+def test_fp32_fit_with_the_default_options_converges(cuda_device):
+    """sb_fit_default_opts (ftol 1e-12, gtol 0, 60 evaluations) in an SB_F32 batch: chi^2 comes back in fp32, so
+    the library raises that ftol to 2^-21 (include/saltband.h).  Without the floor a lane near its minimum
+    burns its budget on halvings and ends stalled or exhausted; with it the lanes stop CONVERGED at the minimum
+    the oracle finds."""
+    wl = _prepare(48)
+    got = _gpu_fit(wl, fp64=False, use_pack=True)  # every option left at the library's default
+    assert np.all(got["status"] != 0)
+    assert np.mean(got["status"] == 1) >= 0.9, np.bincount(got["status"].astype(int), minlength=4)
+    ref = lbfgs.fit_workload(wl, round_theta_to=np.float32, memory=8, max_eval=60, max_iter=1000, ftol=2.0 ** -21, gtol=0.0)
+    assert np.allclose(got["chi2"], ref["chi2"], rtol=1e-4), np.max(np.abs(got["chi2"] / ref["chi2"] - 1))
+    # an explicit zero still switches the test off: no lane converges by ftol, every lane spends its budget or stalls
+    off = _gpu_fit(wl, fp64=False, use_pack=True, ftol=0.0, max_eval=30)
+    assert not np.any(off["status"] == 1)
+
+
+def test_fp32_box_holds_exactly_after_rounding(cuda_device):
+    """Bounds that are not fp32 numbers (-0.3, 0.1, 1e-5 x0 scale): every returned theta must satisfy
+    lo <= theta <= hi exactly as fp32 values compared in fp64, although the lane projects in scaled fp64
+    variables and the result is rounded to fp32 afterwards."""
+    wl = _prepare(64)
+    x0 = wl.theta["x0"].astype(np.float64)
+    lo = np.array([0.3 * x0.min(), -0.3, -0.03, -0.7])
+    hi = np.array([1.7 * x0.max(), 0.1, 0.03, 0.3])
+    got = _gpu_fit(wl, fp64=False, use_pack=True, max_eval=40, ftol=1e-6, lo=lo, hi=hi)
+    assert np.all(got["theta"] >= lo[None, :]) and np.all(got["theta"] <= hi[None, :])
+    lo32, hi32 = np.float32(lo), np.float32(hi)
+    edge = np.stack([lo32, hi32, np.nextafter(lo32, np.float32(np.inf)), np.nextafter(hi32, np.float32(-np.inf))]).astype(np.float64)
+    at_bound = np.any(got["theta"][:, None, :] == edge[None, :, :], axis=1)
+    assert at_bound[:, 1:].any()  # some bound is active, so the clamp was exercised
